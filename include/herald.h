@@ -1,0 +1,194 @@
+/* herald.h -- C ABI of the B200-native HERALD per-block sparse-KV hot path.
+ *
+ * HERALD (arxiv/paper_2606_21633; text in PAPER.md) serves block-diffusion LLMs with a
+ * sparse KV cache: once per block a single *representative query* scores the whole
+ * prefix KV cache and a per-KV-head top-k picks the critical entries (PAPER.md:141-163
+ * section IV-A2; section IV-B4), the selected K/V rows are gathered into
+ * the idle one of two sparse KV pools (section IV-B1), and
+ * the block's T-1 denoising steps attend over the active pool plus the block's own
+ * bidirectional KV (section II-A).  Selection for block n+1 overlaps with the
+ * denoising of block n on a second stream; the pools are swapped at the block boundary
+ * (Fig. 11).  The paper runs selection/gather on the CPU;
+ * here every stage is a CUDA kernel for sm_100a.
+ *
+ * Conventions
+ *   - every entry point returns 0 (HERALD_OK) or a negative HERALD_ERR_* code; nothing
+ *     throws or aborts; herald_last_error() returns a thread-local message.
+ *   - the CALLER owns every buffer (caches, pools, indices, outputs, workspaces).  The
+ *     library allocates nothing, frees nothing and never synchronises with the host;
+ *     all work is enqueued on the stream(s) passed in and is CUDA-graph capturable
+ *     (pools are "allocated at initialization and reused across blocks").
+ *   - pointers are DEVICE pointers unless the comment says "host"; all device pointers
+ *     must be 16-byte aligned.  bf16 = IEEE bfloat16 bit patterns (uint16).
+ *   - head_dim must be 128, page_size 16, G = n_q_heads / n_kv_heads an integer <= 8;
+ *     anything else returns HERALD_ERR_UNSUPPORTED.
+ *   - query head hq belongs to KV head hq / G (contiguous groups).
+ *   - device-side integers (seq_lens, page_table, k_per_seq, pool_len) are trusted; they
+ *     are never read back by the host.  Kernels clamp k to min(k, seq_len, pool_capacity).
+ */
+#ifndef HERALD_H
+#define HERALD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HERALD_OK 0
+#define HERALD_ERR_INVALID_ARG (-1)
+#define HERALD_ERR_UNSUPPORTED (-2)
+#define HERALD_ERR_WORKSPACE_TOO_SMALL (-3)
+#define HERALD_ERR_CUDA (-4)
+
+/* GQA aggregation of the G per-head scores of one cached position (reading 1). */
+#define HERALD_AGG_MAX_LOGIT 0   /* a[t] = max_g s[g,t]                      (BASELINE.json north_star) */
+#define HERALD_AGG_SOFTMAX_SUM 1 /* a[t] = sum_g exp(s[g,t]-m_g)/l_g             */
+
+typedef void* herald_stream_t; /* a cudaStream_t  */
+typedef void* herald_event_t;  /* a cudaEvent_t   */
+
+/* Problem shape, host POD.  Notation follows PAPER.md:201: S = seq_len prefix entries, k the
+ * per-KV-head budget, G query heads per KV head; B = block_size. */
+typedef struct herald_shape {
+    int32_t batch;             /* sequences                                                         */
+    int32_t n_q_heads;         /* H_q                                                               */
+    int32_t n_kv_heads;        /* H_kv                                                              */
+    int32_t head_dim;          /* d, must be 128                                                    */
+    int32_t page_size;         /* tokens per KV page, must be 16                                    */
+    int32_t block_size;        /* B, tokens per diffusion block (1..64)                             */
+    int32_t max_seq_len;       /* bound on seq_lens[]; row stride of the score plane; multiple of 16 */
+    int32_t max_pages_per_seq; /* row stride of page_table                                          */
+    int32_t pool_capacity;     /* rows per (sequence, KV head) in one pool buffer; stride of sel_idx */
+    int32_t agg_mode;          /* HERALD_AGG_*                                                      */
+    float sm_scale;            /* logit scale, d^-1/2 (reading 2)                         */
+} herald_shape_t;
+
+/* Paged full KV cache ("full KV pool"; paged).  Token t of sequence b
+ * is slot t % page_size of physical page page_table[b][t / page_size].  Element (page p, slot s,
+ * KV head h, channel c) is at  p*page_stride + s*token_stride + h*head_stride + c  (bf16 elements);
+ * the 128 channels of a row are contiguous and every stride is a multiple of 8 elements.
+ * The canonical layout [n_pages][16][H_kv][128] has strides (16*H_kv*128, H_kv*128, 128).
+ * Slots past seq_lens[b] in the last page and page_table entries past the last page are never read. */
+typedef struct herald_cache {
+    const void* k_pages;
+    const void* v_pages;
+    int64_t page_stride, token_stride, head_stride;
+    const int32_t* page_table; /* [batch][max_pages_per_seq] */
+    const int32_t* seq_lens;   /* [batch]                    */
+} herald_cache_t;
+
+/* Message for the last error returned on this thread ("" if none).  Host only. */
+const char* herald_last_error(void);
+
+/* Budget rows k = min(L, ceil(L * permille / 1000)) in integer arithmetic (reading 5;
+ * BASELINE.json: 5 % of 4096 -> 205, of 32768 -> 1639).  Host only; returns -1 on bad arguments. */
+int32_t herald_budget_rows(int32_t seq_len, int32_t permille);
+
+/* Workspace sizes in bytes for herald_select / herald_sparse_attn with this shape.  Host only;
+ * return 0 on an invalid shape.  The two stages run concurrently in the pipeline, so they need
+ * two distinct workspaces. */
+size_t herald_select_workspace_bytes(const herald_shape_t* shape);
+size_t herald_attn_workspace_bytes(const herald_shape_t* shape);
+
+/* Representative-query selection (Eq.(1)).
+ * For every sequence b and KV head h:
+ *   s[g,t]  = sm_scale * q_rep[b, h*G+g, :] . K[b, t, h, :]      for all t < seq_lens[b]   (fp32 accumulate)
+ *   a[t]    = aggregate_g s[g,t]                                 (shape->agg_mode)
+ *   sel     = the k = min(k_per_seq[b], seq_lens[b], pool_capacity) positions of largest a[t];
+ *             ties -> lower position; written in ASCENDING position order.
+ *   q_rep      bf16 [batch][H_q][128]
+ *   k_per_seq  int32 [batch]
+ *   sel_idx    int32 [batch][H_kv][pool_capacity]  (entries past sel_cnt are left untouched)
+ *   sel_cnt    int32 [batch][H_kv]
+ *   scores_out optional fp32 [batch][H_kv][max_seq_len]: receives a[t] for t < seq_lens[b]; if NULL
+ *              the plane lives in the workspace.
+ *   ws         >= herald_select_workspace_bytes(shape) bytes, 256-byte aligned.
+ * Errors: INVALID_ARG (null / misaligned pointer, bad shape), UNSUPPORTED, WORKSPACE_TOO_SMALL, CUDA. */
+int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep,
+                  const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, float* scores_out,
+                  void* ws, size_t ws_bytes, herald_stream_t stream);
+
+/* Gather of the selected entries into a sparse KV pool (pools PAPER.md:175):
+ *   pool_k[b][h][j][:] = K[b, sel_idx[b][h][j], h, :]   for j < sel_cnt[b][h]   (bit copies; same for V)
+ *   pool_k, pool_v  bf16 [batch][H_kv][pool_capacity][128] -- the IDLE buffer; rows j >= sel_cnt untouched. */
+int herald_gather(const herald_shape_t* shape, const herald_cache_t* cache, const int32_t* sel_idx,
+                  const int32_t* sel_cnt, void* pool_k, void* pool_v, herald_stream_t stream);
+
+/* One denoising step's attention over critical KV + in-block KV:
+ *   out[b][i][hq][:] = softmax_j( sm_scale * q_blk[b][i][hq][:] . K'_j ) . V'_j ,   h = hq / G,
+ *   K' = pool_k[b][h][0 .. pool_len[b][h]) followed by k_blk[b][0..B)[h]  (no mask; V' likewise).
+ *   pool_k/pool_v bf16 [batch][H_kv][pool_capacity][128] (the ACTIVE buffer); pool_len int32 [batch][H_kv]
+ *   q_blk bf16 [batch][B][H_q][128]; k_blk, v_blk bf16 [batch][B][H_kv][128]
+ *   out fp32 [batch][B][H_q][128]; lse optional fp32 [batch][B][H_q] = log sum_j exp(logit_j).
+ *   ws >= herald_attn_workspace_bytes(shape), 256-byte aligned.  bf16 tensor-core products, fp32
+ *   softmax and accumulation; softmax weights are rounded to bf16 for the PV product. */
+int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const void* pool_v,
+                       const int32_t* pool_len, const void* q_blk, const void* k_blk, const void* v_blk,
+                       float* out, float* lse, void* ws, size_t ws_bytes, herald_stream_t stream);
+
+/* Per-layer state of the dual-stream block step.  Host POD holding device pointers. */
+typedef struct herald_layer {
+    herald_cache_t cache;      /* this layer's full KV pool                                                   */
+    const void* q_rep;         /* bf16 [batch][H_q][128]: representative query of the NEXT block              */
+    const int32_t* k_per_seq;  /* int32 [batch]                                                               */
+    const void* q_blk;         /* bf16 [n_steps][batch][B][H_q][128]: denoise step s reads slice s            */
+    const void* k_blk;         /* bf16 [n_steps][batch][B][H_kv][128]                                         */
+    const void* v_blk;         /* bf16 [n_steps][batch][B][H_kv][128]                                         */
+    float* out;                /* fp32 [n_steps][batch][B][H_q][128]                                          */
+    void* pool_k[2];           /* double-buffered sparse KV pools, each [batch][H_kv][cap][128] */
+    void* pool_v[2];
+    int32_t* pool_len[2];      /* int32 [batch][H_kv] per buffer                                              */
+} herald_layer_t;
+
+/* One block step of the dual-stream pipeline (Fig. 11):
+ *   main stream     : for s in [0, n_steps): for each layer: herald_sparse_attn on pools[active]
+ *   retrieval stream: starts once `start_after_step` main-stream steps have been enqueued-and-finished
+ *                     (0 = immediately, the north-star default; 2 = the paper's "waits only for the
+ *                     first two steps"); for each layer: herald_select -> herald_gather into
+ *                     pools[1-active], sel_cnt written to pool_len[1-active]
+ *   join            : main stream waits for the retrieval stream; `active` is flipped (pool swap).
+ * No host synchronisation.  `layers` is a host array.  Events are caller-created cudaEvent_t. */
+typedef struct herald_pipeline {
+    herald_shape_t shape;
+    int32_t n_layers;
+    int32_t n_steps;          /* T-1 attention steps per block (reading 13) */
+    int32_t start_after_step; /* 0 .. n_steps                                           */
+    int32_t active;           /* index of the ACTIVE pool buffer; flipped on success    */
+    herald_layer_t* layers;   /* host array [n_layers]                                  */
+    int32_t* sel_idx;         /* int32 [batch][H_kv][pool_capacity] scratch (retrieval stream) */
+    void* ws_select;
+    size_t ws_select_bytes;
+    void* ws_attn;
+    size_t ws_attn_bytes;
+    herald_stream_t main_stream;
+    herald_stream_t retrieval_stream;
+    herald_event_t ev_fork; /* recorded on the main stream, waited on by the retrieval stream */
+    herald_event_t ev_join; /* recorded on the retrieval stream, waited on by the main stream */
+} herald_pipeline_t;
+
+int herald_pipeline_step(herald_pipeline_t* pipe);
+
+/* Host-buffer variant used for end-to-end timing: per block, the step's inputs come from (pinned)
+ * HOST memory and its outputs return to HOST memory, all asynchronously on the pipeline's streams:
+ *   H2D  host_q_rep[l] -> layers[l].q_rep ; host_q_blk/k_blk/v_blk[l] -> layers[l].q_blk/k_blk/v_blk
+ *   herald_pipeline_step
+ *   D2H  layers[l].out -> host_out[l]
+ * Each host_* is a host array of n_layers host pointers with the same extents as the device tensors.
+ * The KV cache stays resident in HBM (it is the state, not a per-step input).  The caller
+ * synchronises main_stream before reading host_out. */
+typedef struct herald_host_io {
+    const void* const* host_q_rep;
+    const void* const* host_q_blk;
+    const void* const* host_k_blk;
+    const void* const* host_v_blk;
+    void* const* host_out;
+} herald_host_io_t;
+
+int herald_pipeline_step_host(herald_pipeline_t* pipe, const herald_host_io_t* io);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HERALD_H */

@@ -1,0 +1,436 @@
+// Host side of the C ABI declared in include/herald.h: argument checks, workspace carving,
+// launches, and the dual-stream block step.  No allocation, no host synchronisation.
+#include "../../include/herald.h"
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+
+#include "attn_mma.cuh"
+#include "common.cuh"
+#include "gather.cuh"
+#include "scan.cuh"
+#include "topk.cuh"
+
+namespace herald {
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+static int cuda_fail(cudaError_t e, const char* what) {
+    return fail(HERALD_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+static int env_int(const char* name, int dflt) {
+    const char* s = getenv(name);
+    return (s && *s) ? atoi(s) : dflt;
+}
+
+static int check_shape(const herald_shape_t* s) {
+    if (!s) return fail(HERALD_ERR_INVALID_ARG, "shape is NULL");
+    if (s->batch < 0 || s->n_q_heads <= 0 || s->n_kv_heads <= 0 || s->block_size <= 0 || s->max_seq_len < 0 ||
+        s->max_pages_per_seq < 0 || s->pool_capacity < 0)
+        return fail(HERALD_ERR_INVALID_ARG, "negative or zero extent in shape");
+    if (s->head_dim != kHeadDim) return fail(HERALD_ERR_UNSUPPORTED, "head_dim must be 128 (got %d)", s->head_dim);
+    if (s->page_size != kPageSize) return fail(HERALD_ERR_UNSUPPORTED, "page_size must be 16 (got %d)", s->page_size);
+    if (s->n_q_heads % s->n_kv_heads) return fail(HERALD_ERR_INVALID_ARG, "n_q_heads %% n_kv_heads != 0");
+    if (s->n_q_heads / s->n_kv_heads > 8) return fail(HERALD_ERR_UNSUPPORTED, "G = n_q_heads/n_kv_heads must be <= 8");
+    if (s->block_size > 64) return fail(HERALD_ERR_UNSUPPORTED, "block_size must be <= 64");
+    if (s->max_seq_len % kPageSize) return fail(HERALD_ERR_INVALID_ARG, "max_seq_len must be a multiple of 16");
+    if ((int64_t)s->max_pages_per_seq * kPageSize < s->max_seq_len)
+        return fail(HERALD_ERR_INVALID_ARG, "max_pages_per_seq * 16 < max_seq_len");
+    if (s->agg_mode != HERALD_AGG_MAX_LOGIT && s->agg_mode != HERALD_AGG_SOFTMAX_SUM)
+        return fail(HERALD_ERR_INVALID_ARG, "agg_mode must be 0 or 1");
+    if (!(s->sm_scale > 0.f)) return fail(HERALD_ERR_INVALID_ARG, "sm_scale must be > 0");
+    return HERALD_OK;
+}
+
+static int check_cache(const herald_cache_t* c, bool need_v) {
+    if (!c) return fail(HERALD_ERR_INVALID_ARG, "cache is NULL");
+    if (!c->k_pages || (need_v && !c->v_pages) || !c->page_table || !c->seq_lens)
+        return fail(HERALD_ERR_INVALID_ARG, "cache has a NULL pointer");
+    if (!aligned16(c->k_pages) || (need_v && !aligned16(c->v_pages)))
+        return fail(HERALD_ERR_INVALID_ARG, "cache pages must be 16-byte aligned");
+    if (c->page_stride % 8 || c->token_stride % 8 || c->head_stride % 8 || c->head_stride < kHeadDim)
+        return fail(HERALD_ERR_INVALID_ARG, "cache strides must be multiples of 8 elements, head_stride >= 128");
+    return HERALD_OK;
+}
+
+// ---- select workspace layout ------------------------------------------------------------------
+struct SelectWs {
+    size_t hist1, scores, raw, stats, total;
+    int scan_ctas;
+};
+
+static int scan_ctas_for(const herald_shape_t* s) {
+    const int units = s->batch * s->n_kv_heads;
+    const int max_pages = (s->max_seq_len + kPageSize - 1) / kPageSize;
+    int target = env_int("HERALD_SCAN_TOTAL_CTAS", 148 * 4);
+    int per_unit = units > 0 ? (target + units - 1) / units : 1;
+    const int cap = (max_pages + kScanWarps - 1) / kScanWarps;
+    if (per_unit > cap) per_unit = cap;
+    if (per_unit < 1) per_unit = 1;
+    return per_unit;
+}
+
+static SelectWs select_ws_layout(const herald_shape_t* s) {
+    SelectWs w{};
+    const size_t units = (size_t)s->batch * s->n_kv_heads;
+    const int G = s->n_q_heads / s->n_kv_heads;
+    w.scan_ctas = scan_ctas_for(s);
+    size_t off = 0;
+    w.hist1 = off;
+    off = align_up(off + units * kBins1 * sizeof(uint32_t), 256);
+    w.scores = off;
+    off = align_up(off + units * (size_t)s->max_seq_len * sizeof(float), 256);
+    w.raw = off;
+    w.stats = off;
+    if (s->agg_mode == HERALD_AGG_SOFTMAX_SUM) {
+        off = align_up(off + units * G * (size_t)s->max_seq_len * sizeof(float), 256);
+        w.stats = off;
+        off = align_up(off + units * G * (size_t)w.scan_ctas * sizeof(float2), 256);
+    }
+    w.total = off;
+    return w;
+}
+
+// ---- attention launch geometry ----------------------------------------------------------------
+struct AttnGeom {
+    int m_tiles, m_pad, n_splits;
+    size_t part_o, part_ml, total;
+};
+
+static AttnGeom attn_geom(const herald_shape_t* s) {
+    AttnGeom a{};
+    const int G = s->n_q_heads / s->n_kv_heads;
+    const int M = s->block_size * G;
+    const int units = s->batch * s->n_kv_heads;
+    a.m_tiles = (M + kAttnBM - 1) / kAttnBM;
+    a.m_pad = a.m_tiles * kAttnBM;
+    const int max_tiles = (s->pool_capacity + s->block_size + kAttnBN - 1) / kAttnBN;
+    const int target = env_int("HERALD_ATTN_TOTAL_CTAS", 148 * 3);
+    int splits = units > 0 ? (target + units * a.m_tiles - 1) / (units * a.m_tiles) : 1;
+    if (splits > max_tiles / 2) splits = max_tiles / 2;
+    if (splits > 32) splits = 32;
+    if (splits < 1) splits = 1;
+    const int forced = env_int("HERALD_ATTN_SPLITS", 0);
+    if (forced > 0) splits = forced < max_tiles ? forced : (max_tiles > 0 ? max_tiles : 1);
+    a.n_splits = splits;
+    size_t off = 0;
+    a.part_o = off;
+    if (splits > 1) off = align_up(off + (size_t)units * splits * a.m_pad * kHeadDim * sizeof(float), 256);
+    a.part_ml = off;
+    if (splits > 1) off = align_up(off + (size_t)units * splits * a.m_pad * sizeof(float2), 256);
+    a.total = off > 256 ? off : 256;
+    return a;
+}
+
+}  // namespace herald
+
+using namespace herald;
+
+extern "C" {
+
+const char* herald_last_error(void) { return g_err; }
+
+int32_t herald_budget_rows(int32_t seq_len, int32_t permille) {
+    if (seq_len < 0 || permille < 0 || permille > 1000) return -1;
+    const int64_t k = ((int64_t)seq_len * permille + 999) / 1000;
+    return (int32_t)(k < seq_len ? k : seq_len);
+}
+
+size_t herald_select_workspace_bytes(const herald_shape_t* shape) {
+    if (check_shape(shape) != HERALD_OK) return 0;
+    return select_ws_layout(shape).total;
+}
+
+size_t herald_attn_workspace_bytes(const herald_shape_t* shape) {
+    if (check_shape(shape) != HERALD_OK) return 0;
+    return attn_geom(shape).total;
+}
+
+int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep,
+                  const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, float* scores_out, void* ws,
+                  size_t ws_bytes, herald_stream_t stream_) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    rc = check_cache(cache, false);
+    if (rc) return rc;
+    if (!q_rep || !k_per_seq || !sel_idx || !sel_cnt || !ws) return fail(HERALD_ERR_INVALID_ARG, "herald_select: NULL pointer");
+    if (!aligned16(q_rep) || !aligned16(sel_idx) || !aligned16(scores_out) || (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return fail(HERALD_ERR_INVALID_ARG, "herald_select: misaligned pointer (16 B; workspace 256 B)");
+    const SelectWs w = select_ws_layout(shape);
+    if (ws_bytes < w.total) return fail(HERALD_ERR_WORKSPACE_TOO_SMALL, "herald_select: workspace %zu < %zu", ws_bytes, w.total);
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const int units = shape->batch * shape->n_kv_heads;
+    if (units == 0) return HERALD_OK;
+    g_err[0] = 0;
+
+    uint8_t* wsb = static_cast<uint8_t*>(ws);
+    uint32_t* hist1 = reinterpret_cast<uint32_t*>(wsb + w.hist1);
+    float* scores = scores_out ? scores_out : reinterpret_cast<float*>(wsb + w.scores);
+    cudaError_t e = cudaMemsetAsync(hist1, 0, (size_t)units * kBins1 * sizeof(uint32_t), stream);
+    if (e != cudaSuccess) return cuda_fail(e, "memset hist1");
+
+    if (shape->max_seq_len > 0) {
+        ScanParams sp{};
+        sp.k_pages = static_cast<const __nv_bfloat16*>(cache->k_pages);
+        sp.page_stride = cache->page_stride;
+        sp.token_stride = cache->token_stride;
+        sp.head_stride = cache->head_stride;
+        sp.page_table = cache->page_table;
+        sp.seq_lens = cache->seq_lens;
+        sp.q_rep = static_cast<const __nv_bfloat16*>(q_rep);
+        sp.scores = scores;
+        sp.raw = reinterpret_cast<float*>(wsb + w.raw);
+        sp.stats_part = reinterpret_cast<float2*>(wsb + w.stats);
+        sp.hist1 = hist1;
+        sp.n_q_heads = shape->n_q_heads;
+        sp.n_kv_heads = shape->n_kv_heads;
+        sp.max_seq_len = shape->max_seq_len;
+        sp.max_pages = shape->max_pages_per_seq;
+        sp.sm_scale = shape->sm_scale;
+        dim3 grid(w.scan_ctas, shape->n_kv_heads, shape->batch);
+        if (shape->agg_mode == HERALD_AGG_MAX_LOGIT) {
+            scan_kernel<0><<<grid, kScanThreads, 0, stream>>>(sp);
+        } else {
+            scan_kernel<1><<<grid, kScanThreads, 0, stream>>>(sp);
+            AggParams ap{};
+            ap.raw = sp.raw;
+            ap.stats_part = sp.stats_part;
+            ap.n_parts = w.scan_ctas;
+            ap.seq_lens = cache->seq_lens;
+            ap.scores = scores;
+            ap.hist1 = hist1;
+            ap.n_q_heads = shape->n_q_heads;
+            ap.n_kv_heads = shape->n_kv_heads;
+            ap.max_seq_len = shape->max_seq_len;
+            int chunks = (shape->max_seq_len + 256 * 8 - 1) / (256 * 8);
+            if (chunks < 1) chunks = 1;
+            dim3 agrid(chunks, shape->n_kv_heads, shape->batch);
+            aggregate_softmax_kernel<<<agrid, 256, 0, stream>>>(ap);
+        }
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e, "scan launch");
+    }
+
+    TopkParams tp{};
+    tp.scores = scores;
+    tp.hist1 = hist1;
+    tp.seq_lens = cache->seq_lens;
+    tp.k_per_seq = k_per_seq;
+    tp.sel_idx = sel_idx;
+    tp.sel_cnt = sel_cnt;
+    tp.n_kv_heads = shape->n_kv_heads;
+    tp.max_seq_len = shape->max_seq_len;
+    tp.cap = shape->pool_capacity;
+    topk_kernel<<<units, kTopkThreads, 0, stream>>>(tp);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "topk launch");
+    return HERALD_OK;
+}
+
+int herald_gather(const herald_shape_t* shape, const herald_cache_t* cache, const int32_t* sel_idx,
+                  const int32_t* sel_cnt, void* pool_k, void* pool_v, herald_stream_t stream_) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    rc = check_cache(cache, true);
+    if (rc) return rc;
+    if (!sel_idx || !sel_cnt || !pool_k || !pool_v) return fail(HERALD_ERR_INVALID_ARG, "herald_gather: NULL pointer");
+    if (!aligned16(pool_k) || !aligned16(pool_v) || !aligned16(sel_idx))
+        return fail(HERALD_ERR_INVALID_ARG, "herald_gather: misaligned pointer");
+    const int units = shape->batch * shape->n_kv_heads;
+    if (units == 0 || shape->pool_capacity == 0) return HERALD_OK;
+    g_err[0] = 0;
+    GatherParams gp{};
+    gp.k_pages = static_cast<const __nv_bfloat16*>(cache->k_pages);
+    gp.v_pages = static_cast<const __nv_bfloat16*>(cache->v_pages);
+    gp.page_stride = cache->page_stride;
+    gp.token_stride = cache->token_stride;
+    gp.head_stride = cache->head_stride;
+    gp.page_table = cache->page_table;
+    gp.sel_idx = sel_idx;
+    gp.sel_cnt = sel_cnt;
+    gp.pool_k = static_cast<__nv_bfloat16*>(pool_k);
+    gp.pool_v = static_cast<__nv_bfloat16*>(pool_v);
+    gp.n_kv_heads = shape->n_kv_heads;
+    gp.max_pages = shape->max_pages_per_seq;
+    gp.cap = shape->pool_capacity;
+    const int rows_per_cta = (kGatherThreads / 32) * kGatherRowsPerWarp;
+    int gx = (shape->pool_capacity + rows_per_cta - 1) / rows_per_cta;
+    if (gx > 4096) gx = 4096;
+    dim3 grid(gx, units);
+    gather_kernel<<<grid, kGatherThreads, 0, static_cast<cudaStream_t>(stream_)>>>(gp);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "gather launch");
+    return HERALD_OK;
+}
+
+int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const void* pool_v, const int32_t* pool_len,
+                       const void* q_blk, const void* k_blk, const void* v_blk, float* out, float* lse, void* ws,
+                       size_t ws_bytes, herald_stream_t stream_) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    if (!pool_k || !pool_v || !pool_len || !q_blk || !k_blk || !v_blk || !out || !ws)
+        return fail(HERALD_ERR_INVALID_ARG, "herald_sparse_attn: NULL pointer");
+    if (!aligned16(pool_k) || !aligned16(pool_v) || !aligned16(q_blk) || !aligned16(k_blk) || !aligned16(v_blk) ||
+        !aligned16(out) || (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return fail(HERALD_ERR_INVALID_ARG, "herald_sparse_attn: misaligned pointer (16 B; workspace 256 B)");
+    const AttnGeom a = attn_geom(shape);
+    if (ws_bytes < a.total) return fail(HERALD_ERR_WORKSPACE_TOO_SMALL, "herald_sparse_attn: workspace %zu < %zu", ws_bytes, a.total);
+    const int units = shape->batch * shape->n_kv_heads;
+    if (units == 0) return HERALD_OK;
+    g_err[0] = 0;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(attn_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kAttnSmemBytes);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(attn)");
+        attr_set = true;
+    }
+    AttnParams ap{};
+    ap.pool_k = static_cast<const __nv_bfloat16*>(pool_k);
+    ap.pool_v = static_cast<const __nv_bfloat16*>(pool_v);
+    ap.pool_len = pool_len;
+    ap.q_blk = static_cast<const __nv_bfloat16*>(q_blk);
+    ap.k_blk = static_cast<const __nv_bfloat16*>(k_blk);
+    ap.v_blk = static_cast<const __nv_bfloat16*>(v_blk);
+    ap.out = out;
+    ap.lse = lse;
+    ap.part_o = reinterpret_cast<float*>(static_cast<uint8_t*>(ws) + a.part_o);
+    ap.part_ml = reinterpret_cast<float2*>(static_cast<uint8_t*>(ws) + a.part_ml);
+    ap.n_q_heads = shape->n_q_heads;
+    ap.n_kv_heads = shape->n_kv_heads;
+    ap.block_size = shape->block_size;
+    ap.cap = shape->pool_capacity;
+    ap.n_splits = a.n_splits;
+    ap.m_pad = a.m_pad;
+    ap.scale_log2 = shape->sm_scale * 1.4426950408889634f;
+    dim3 grid(a.m_tiles, a.n_splits, units);
+    attn_mma_kernel<<<grid, kAttnThreads, kAttnSmemBytes, stream>>>(ap);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "attention launch");
+    if (a.n_splits > 1) {
+        const int M = shape->block_size * (shape->n_q_heads / shape->n_kv_heads);
+        attn_combine_kernel<<<dim3(M, units), 128, 0, stream>>>(ap);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e, "combine launch");
+    }
+    return HERALD_OK;
+}
+
+static int check_pipeline(const herald_pipeline_t* p) {
+    if (!p) return fail(HERALD_ERR_INVALID_ARG, "pipeline is NULL");
+    int rc = check_shape(&p->shape);
+    if (rc) return rc;
+    if (p->n_layers <= 0 || !p->layers) return fail(HERALD_ERR_INVALID_ARG, "pipeline: no layers");
+    if (p->n_steps < 0 || p->start_after_step < 0 || p->start_after_step > p->n_steps)
+        return fail(HERALD_ERR_INVALID_ARG, "pipeline: bad n_steps / start_after_step");
+    if (p->active != 0 && p->active != 1) return fail(HERALD_ERR_INVALID_ARG, "pipeline: active must be 0 or 1");
+    if (!p->sel_idx || !p->ws_select || !p->ws_attn || !p->ev_fork || !p->ev_join)
+        return fail(HERALD_ERR_INVALID_ARG, "pipeline: NULL scratch / workspace / event");
+    if (p->main_stream == p->retrieval_stream)
+        return fail(HERALD_ERR_INVALID_ARG, "pipeline: main and retrieval streams must differ");
+    return HERALD_OK;
+}
+
+int herald_pipeline_step(herald_pipeline_t* p) {
+    int rc = check_pipeline(p);
+    if (rc) return rc;
+    cudaStream_t s_main = static_cast<cudaStream_t>(p->main_stream);
+    cudaStream_t s_ret = static_cast<cudaStream_t>(p->retrieval_stream);
+    cudaEvent_t ev_fork = static_cast<cudaEvent_t>(p->ev_fork), ev_join = static_cast<cudaEvent_t>(p->ev_join);
+    const herald_shape_t* sh = &p->shape;
+    const int act = p->active, idle = 1 - act;
+    const size_t q_step = (size_t)sh->batch * sh->block_size * sh->n_q_heads * kHeadDim;
+    const size_t kv_step = (size_t)sh->batch * sh->block_size * sh->n_kv_heads * kHeadDim;
+    cudaError_t e;
+
+    auto retrieval = [&]() -> int {
+        e = cudaEventRecord(ev_fork, s_main);
+        if (e != cudaSuccess) return cuda_fail(e, "record fork");
+        e = cudaStreamWaitEvent(s_ret, ev_fork, 0);
+        if (e != cudaSuccess) return cuda_fail(e, "wait fork");
+        for (int l = 0; l < p->n_layers; ++l) {
+            herald_layer_t* ly = &p->layers[l];
+            int r = herald_select(sh, &ly->cache, ly->q_rep, ly->k_per_seq, p->sel_idx, ly->pool_len[idle], nullptr,
+                                  p->ws_select, p->ws_select_bytes, s_ret);
+            if (r) return r;
+            r = herald_gather(sh, &ly->cache, p->sel_idx, ly->pool_len[idle], ly->pool_k[idle], ly->pool_v[idle], s_ret);
+            if (r) return r;
+        }
+        e = cudaEventRecord(ev_join, s_ret);
+        if (e != cudaSuccess) return cuda_fail(e, "record join");
+        return HERALD_OK;
+    };
+
+    bool forked = false;
+    for (int s = 0; s <= p->n_steps; ++s) {
+        if (s == p->start_after_step && !forked) {
+            rc = retrieval();
+            if (rc) return rc;
+            forked = true;
+        }
+        if (s == p->n_steps) break;
+        for (int l = 0; l < p->n_layers; ++l) {
+            herald_layer_t* ly = &p->layers[l];
+            rc = herald_sparse_attn(sh, ly->pool_k[act], ly->pool_v[act], ly->pool_len[act],
+                                    static_cast<const __nv_bfloat16*>(ly->q_blk) + s * q_step,
+                                    static_cast<const __nv_bfloat16*>(ly->k_blk) + s * kv_step,
+                                    static_cast<const __nv_bfloat16*>(ly->v_blk) + s * kv_step,
+                                    ly->out + s * q_step, nullptr, p->ws_attn, p->ws_attn_bytes, s_main);
+            if (rc) return rc;
+        }
+    }
+    e = cudaStreamWaitEvent(s_main, ev_join, 0);
+    if (e != cudaSuccess) return cuda_fail(e, "wait join");
+    p->active = idle;
+    return HERALD_OK;
+}
+
+int herald_pipeline_step_host(herald_pipeline_t* p, const herald_host_io_t* io) {
+    int rc = check_pipeline(p);
+    if (rc) return rc;
+    if (!io || !io->host_q_rep || !io->host_q_blk || !io->host_k_blk || !io->host_v_blk || !io->host_out)
+        return fail(HERALD_ERR_INVALID_ARG, "pipeline_step_host: NULL host io");
+    cudaStream_t s_main = static_cast<cudaStream_t>(p->main_stream);
+    const herald_shape_t* sh = &p->shape;
+    const size_t q_step = (size_t)sh->batch * sh->block_size * sh->n_q_heads * kHeadDim;
+    const size_t kv_step = (size_t)sh->batch * sh->block_size * sh->n_kv_heads * kHeadDim;
+    const size_t q_rep_bytes = (size_t)sh->batch * sh->n_q_heads * kHeadDim * 2;
+    cudaError_t e;
+    for (int l = 0; l < p->n_layers; ++l) {
+        herald_layer_t* ly = &p->layers[l];
+        // inputs are enqueued on the main stream; the fork event orders the retrieval stream after them
+        e = cudaMemcpyAsync(const_cast<void*>(ly->q_rep), io->host_q_rep[l], q_rep_bytes, cudaMemcpyHostToDevice, s_main);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(const_cast<void*>(ly->q_blk), io->host_q_blk[l], q_step * p->n_steps * 2, cudaMemcpyHostToDevice, s_main);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(const_cast<void*>(ly->k_blk), io->host_k_blk[l], kv_step * p->n_steps * 2, cudaMemcpyHostToDevice, s_main);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(const_cast<void*>(ly->v_blk), io->host_v_blk[l], kv_step * p->n_steps * 2, cudaMemcpyHostToDevice, s_main);
+        if (e != cudaSuccess) return cuda_fail(e, "H2D copy");
+    }
+    rc = herald_pipeline_step(p);
+    if (rc) return rc;
+    for (int l = 0; l < p->n_layers; ++l) {
+        herald_layer_t* ly = &p->layers[l];
+        e = cudaMemcpyAsync(io->host_out[l], ly->out, q_step * p->n_steps * sizeof(float), cudaMemcpyDeviceToHost, s_main);
+        if (e != cudaSuccess) return cuda_fail(e, "D2H copy");
+    }
+    return HERALD_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,92 @@
+"""CPU-side checks of the C-ABI boundary: the library builds/loads, exports every symbol that
+include/herald.h declares, and its host-only logic (budget, workspace sizes, argument checks that
+fail before any CUDA call) behaves as documented.  No GPU compute here."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from oracle import herald_oracle as O
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def H():
+    from paper_2606_21633_b200 import build
+    build.build()
+    from paper_2606_21633_b200 import herald
+    return herald
+
+
+def declared_functions():
+    text = open(os.path.join(ROOT, "include", "herald.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(herald_[a-z_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol(H):
+    names = declared_functions()
+    assert len(names) >= 9
+    lib = C.CDLL(H.LIB_PATH)
+    for n in names:
+        assert hasattr(lib, n), f"{n} is declared in include/herald.h but not exported"
+    assert set(names) == set(H.EXPORTS)
+
+
+def test_budget_rows_matches_oracle_and_golden(H):
+    for L in list(range(0, 70)) + [4096, 32768, 65536, 131072, 99999]:
+        for pm in (0, 1, 25, 50, 100, 175, 500, 999, 1000):
+            assert H.herald_budget_rows(L, pm) == O.budget_rows(L, pm)
+    assert H.herald_budget_rows(4096, 50) == 205 and H.herald_budget_rows(32768, 50) == 1639
+    assert H.herald_budget_rows(-1, 50) == -1 and H.herald_budget_rows(10, 1001) == -1
+
+
+def test_workspace_sizes(H):
+    s = H.make_shape(8, 28, 4, 32, 32768, 2048, 1639 + 32)
+    sel, att = H.herald_select_workspace_bytes(s), H.herald_attn_workspace_bytes(s)
+    assert sel >= 32 * 4096 * 4 + 32 * 32768 * 4      # level-1 histograms + score plane
+    assert att >= 256
+    s1 = H.make_shape(8, 28, 4, 32, 32768, 2048, 1639 + 32, agg_mode=1)
+    assert H.herald_select_workspace_bytes(s1) >= sel + 32 * 7 * 32768 * 4   # raw per-head scores
+    bad = H.make_shape(8, 28, 4, 32, 32768, 2048, 100, head_dim=64)
+    assert H.herald_select_workspace_bytes(bad) == 0
+
+
+@pytest.mark.parametrize("kw,code", [
+    (dict(head_dim=64), -2), (dict(page_size=32), -2), (dict(n_q_heads=36), -2), (dict(n_q_heads=30), -1),
+    (dict(block_size=128), -2), (dict(max_seq_len=1000), -1), (dict(agg_mode=3), -1), (dict(sm_scale=0.0), -1),
+    (dict(max_pages_per_seq=1), -1),
+])
+def test_invalid_shapes_are_rejected_before_any_cuda_call(H, kw, code):
+    base = dict(batch=2, n_q_heads=8, n_kv_heads=4, block_size=16, max_seq_len=1024, max_pages_per_seq=64, pool_capacity=64)
+    base.update(kw)
+    shape = H.make_shape(**base)
+    cache = H.Cache(256, 256, 16 * 4 * 128, 4 * 128, 128, 256, 256)
+    with pytest.raises(H.HeraldError) as ei:
+        H.herald_select(shape, cache, 256, 256, 256, 256, None, (256, 1 << 30), stream=0)
+    assert ei.value.code == code and H.herald_last_error() != ""
+
+
+def test_null_and_misaligned_pointers_are_rejected(H):
+    shape = H.make_shape(2, 8, 4, 16, 1024, 64, 64)
+    cache = H.Cache(256, 256, 16 * 4 * 128, 4 * 128, 128, 256, 256)
+    with pytest.raises(H.HeraldError) as ei:
+        H.herald_select(shape, cache, None, 256, 256, 256, None, (256, 1 << 30), stream=0)
+    assert ei.value.code == H.ERR_INVALID_ARG
+    with pytest.raises(H.HeraldError) as ei:
+        H.herald_gather(shape, cache, 256, 256, 264, 256, stream=0)       # pool_k not 16-byte aligned
+    assert ei.value.code == H.ERR_INVALID_ARG
+    bad_cache = H.Cache(256, 256, 16 * 4 * 128, 4 * 128 + 4, 128, 256, 256)
+    with pytest.raises(H.HeraldError) as ei:
+        H.herald_gather(shape, bad_cache, 256, 256, 256, 256, stream=0)
+    assert ei.value.code == H.ERR_INVALID_ARG
+
+
+def test_workspace_too_small_is_reported(H):
+    shape = H.make_shape(2, 8, 4, 16, 1024, 64, 64)
+    cache = H.Cache(256, 256, 16 * 4 * 128, 4 * 128, 128, 256, 256)
+    with pytest.raises(H.HeraldError) as ei:       # the size check fails before any device access
+        H.herald_select(shape, cache, 256, 256, 256, 256, None, (4096, 256), stream=0)
+    assert ei.value.code == H.ERR_WORKSPACE_TOO_SMALL

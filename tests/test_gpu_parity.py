@@ -1,0 +1,319 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the fp64 oracle, element by element,
+on seeded inputs that span several tiles and ragged tails.  Run with -m gpu on a B200."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import herald_oracle as O
+from paper_2606_21633_b200 import synth
+from parity_util import ATTN_TOL, check_selection, oracle_inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def H():
+    from paper_2606_21633_b200 import herald
+    return herald
+
+
+def run_select(H, w, inp, ks, agg_mode=0, cap=None, want_scores=True):
+    dev = inp["k_pages"].device
+    cap = cap if cap is not None else max(max(ks), 1) + w.block_size
+    max_seq = (w.max_seq_len + 15) // 16 * 16
+    shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, max_seq, inp["page_table"].shape[1], cap, agg_mode)
+    cache = H.make_cache(inp["k_pages"], inp["v_pages"], inp["page_table"], inp["seq_lens"])
+    k_per_seq = torch.tensor(ks, dtype=torch.int32, device=dev)
+    sel_idx = torch.full((w.batch, w.n_kv_heads, cap), -7, dtype=torch.int32, device=dev)
+    sel_cnt = torch.full((w.batch, w.n_kv_heads), -7, dtype=torch.int32, device=dev)
+    scores = torch.full((w.batch, w.n_kv_heads, max(max_seq, 16)), float("nan"), dtype=torch.float32, device=dev) if want_scores else None
+    ws = H.alloc_workspace(H.herald_select_workspace_bytes(shape), dev)
+    H.herald_select(shape, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, scores, ws)
+    torch.cuda.synchronize()
+    return shape, cache, k_per_seq, sel_idx, sel_cnt, scores
+
+
+SELECT_CASES = {
+    "tiny_ragged": dict(w=synth.tiny(seq_lens=(300, 77), permille=100), spare=3, hostile=True),
+    "one_token": dict(w=synth.tiny(seq_lens=(1, 17), permille=500), spare=0, hostile=True),
+    "C1": dict(w=synth.config("C1"), spare=0, hostile=False),
+    "g7_ragged": dict(w=synth.Workload("g7", 3, (5000, 3333, 16), 28, 4, 32, 4, 50, "planted", 20), spare=2, hostile=True),
+    "g8_h8": dict(w=synth.Workload("g8", 2, (2049, 4096), 64, 8, 16, 3, 25, "zipf"), spare=0, hostile=False),
+    "g1": dict(w=synth.Workload("g1", 2, (1000, 999), 2, 2, 16, 3, 100, "plain"), spare=0, hostile=True),
+}
+
+
+@pytest.mark.parametrize("agg_mode", [0, 1])
+@pytest.mark.parametrize("case", list(SELECT_CASES))
+def test_select_matches_oracle(H, cuda, case, agg_mode):
+    c = SELECT_CASES[case]
+    w = c["w"]
+    inp = synth.make_inputs(w, seed=100 + len(case), device=cuda, spare_pages=c["spare"], hostile_tails=c["hostile"])
+    ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
+    assert ks == [H.herald_budget_rows(L, w.permille) for L in w.seq_lens]
+    shape, cache, k_per_seq, sel_idx, sel_cnt, scores = run_select(H, w, inp, ks, agg_mode)
+    oi = oracle_inputs(inp)
+    sel_o, sc_o = O.select(oi["q_rep"], oi["k_pages"], oi["page_table"], oi["seq_lens"], ks, w.n_kv_heads, 128 ** -0.5, agg_mode)
+    sel_g, cnt_g, sc_g = sel_idx.cpu().numpy(), sel_cnt.cpu().numpy(), scores.cpu().numpy()
+    differing = 0
+    for b, L in enumerate(w.seq_lens):
+        for h in range(w.n_kv_heads):
+            ref = sc_o[b][h]
+            got = sc_g[b, h, :L]
+            tol = 1e-4 if agg_mode == 0 else 2e-3 * max(ref.max(), 1e-30)
+            assert np.abs(got - ref).max() <= tol, (case, b, h, np.abs(got - ref).max())
+            differing += check_selection(sel_g[b, h], int(cnt_g[b, h]), ref, ks[b], L, f"{case} b{b} h{h}")
+            assert np.all(sel_g[b, h, int(cnt_g[b, h]):] == -7), "entries past sel_cnt must stay untouched"
+    units = w.batch * w.n_kv_heads
+    assert differing <= max(1, units // 4), f"{differing} in-band swaps over {units} units is more than rounding explains"
+    if w.structure == "planted" and agg_mode == 0:
+        for b in range(w.batch):
+            for h in range(w.n_kv_heads):
+                planted = set(inp["planted"][b][h].tolist())
+                assert len(planted - set(sel_o[b][h].tolist())) <= max(1, len(planted) // 8)
+
+
+def test_select_edge_cases(H, cuda):
+    # empty sequence, k = 0, k >= L (identity), k > pool capacity (clamped)
+    w = synth.Workload("edge", 4, (0, 40, 33, 64), 4, 2, 16, 3, 100, "plain")
+    inp = synth.make_inputs(w, seed=7, device=cuda, hostile_tails=True)
+    ks = [5, 0, 1000, 64]
+    shape, cache, k_per_seq, sel_idx, sel_cnt, scores = run_select(H, w, inp, ks, cap=48)
+    cnt = sel_cnt.cpu().numpy()
+    sel = sel_idx.cpu().numpy()
+    assert cnt.tolist() == [[0, 0], [0, 0], [33, 33], [48, 48]]
+    assert sel[2, 0, :33].tolist() == list(range(33)) and sel[2, 1, :33].tolist() == list(range(33))
+    oi = oracle_inputs(inp)
+    _, sc_o = O.select(oi["q_rep"], oi["k_pages"], oi["page_table"], oi["seq_lens"], [0, 0, 33, 48], 2, 128 ** -0.5)
+    for h in range(2):
+        assert check_selection(sel[3, h], 48, sc_o[3][h], 48, 64, "clamped") == 0
+
+
+def test_select_exact_ties_take_lowest_positions(H, cuda):
+    # all keys identical => every score equal => the k lowest positions; two-valued keys => ties at the boundary
+    w = synth.Workload("ties", 2, (1000, 515), 4, 1, 16, 3, 100, "plain")
+    inp = synth.make_inputs(w, seed=8, device=cuda)
+    inp["k_pages"][:] = inp["k_pages"][0, 0, 0]
+    ks = [100, 52]
+    _, _, _, sel_idx, sel_cnt, _ = run_select(H, w, inp, ks)
+    sel = sel_idx.cpu().numpy()
+    assert sel[0, 0, :100].tolist() == list(range(100)) and sel[1, 0, :52].tolist() == list(range(52))
+    # every 7th position gets a second key value; k cuts through one of the two tie classes
+    inp2 = synth.make_inputs(w, seed=8, device=cuda)
+    base = inp2["k_pages"][0, 0, 0].clone()
+    inp2["k_pages"][:] = base
+    pt = inp2["page_table"].cpu().numpy()
+    other = inp2["q_rep"][0, 0].clone()
+    for b, L in enumerate(w.seq_lens):
+        for t in range(0, L, 7):
+            inp2["k_pages"][int(pt[b, t // 16]), t % 16, 0] = other if b == 0 else base * 0
+    _, _, _, sel_idx, sel_cnt, _ = run_select(H, w, inp2, ks)
+    oi = oracle_inputs(inp2)
+    sel_o, _ = O.select(oi["q_rep"], oi["k_pages"], oi["page_table"], oi["seq_lens"], ks, 1, 128 ** -0.5)
+    sel = sel_idx.cpu().numpy()
+    for b in range(2):
+        assert sel[b, 0, :ks[b]].tolist() == sel_o[b][0].tolist()
+
+
+@pytest.mark.parametrize("case", ["tiny_ragged", "g7_ragged", "C1"])
+def test_gather_is_bit_exact(H, cuda, case):
+    c = SELECT_CASES[case]
+    w = c["w"]
+    inp = synth.make_inputs(w, seed=200, device=cuda, spare_pages=c["spare"], hostile_tails=c["hostile"])
+    ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
+    shape, cache, k_per_seq, sel_idx, sel_cnt, _ = run_select(H, w, inp, ks, want_scores=False)
+    cap = shape.pool_capacity
+    canary = 0x7FC1
+    pool_k = torch.full((w.batch, w.n_kv_heads, cap, 128), canary, dtype=torch.int16, device=cuda).view(torch.bfloat16)
+    pool_v = torch.full((w.batch, w.n_kv_heads, cap, 128), canary, dtype=torch.int16, device=cuda).view(torch.bfloat16)
+    H.herald_gather(shape, cache, sel_idx, sel_cnt, pool_k, pool_v)
+    torch.cuda.synchronize()
+    oi = oracle_inputs(inp)
+    cnt = sel_cnt.cpu().numpy()
+    sel_g = sel_idx.cpu().numpy()
+    sel = [[sel_g[b, h, :cnt[b, h]] for h in range(w.n_kv_heads)] for b in range(w.batch)]
+    pk_o, pv_o, pl_o = O.gather(oi["k_pages"], oi["v_pages"], oi["page_table"], sel, cap, fill=canary)
+    assert np.array_equal(synth.to_u16(pool_k), pk_o)      # includes the untouched canary rows past sel_cnt
+    assert np.array_equal(synth.to_u16(pool_v), pv_o)
+    assert np.array_equal(cnt, pl_o)
+
+
+def _attn_case(cuda, batch, B, Hq, Hkv, cap, pool_len, seed, q_scale=1.0):
+    g = torch.Generator(device=cuda)
+    g.manual_seed(seed)
+    rn = lambda *s: torch.randn(*s, generator=g, device=cuda, dtype=torch.float32)
+    q = (q_scale * rn(batch, B, Hq, 128)).to(torch.bfloat16)
+    kb, vb = rn(batch, B, Hkv, 128).to(torch.bfloat16), rn(batch, B, Hkv, 128).to(torch.bfloat16)
+    pk, pv = rn(batch, Hkv, cap, 128).to(torch.bfloat16), rn(batch, Hkv, cap, 128).to(torch.bfloat16)
+    pl = torch.tensor(pool_len, dtype=torch.int32, device=cuda).reshape(batch, Hkv)
+    # rows past pool_len must be ignored: poison them
+    for b in range(batch):
+        for h in range(Hkv):
+            pk[b, h, int(pl[b, h]):] = 300.0
+            pv[b, h, int(pl[b, h]):] = float("nan")
+    return q, kb, vb, pk, pv, pl
+
+
+ATTN_CASES = {
+    # name: (batch, B, Hq, Hkv, cap, pool_len per (b,h), q_scale)
+    "tiny": (1, 16, 4, 2, 40, [[40, 7]], 1.0),
+    "empty_pool": (2, 16, 4, 1, 16, [[0], [1]], 1.0),
+    "c1_shape": (1, 16, 4, 1, 221, [[205]], 1.0),
+    "m224_ragged": (2, 32, 28, 4, 700, [[700, 1, 333, 64], [63, 65, 0, 512]], 1.0),
+    "m64_g8": (2, 8, 64, 8, 130, [[130, 129, 128, 127, 2, 3, 64, 100]] * 2, 1.0),
+    "peaked": (1, 16, 8, 2, 300, [[300, 150]], 4.0),
+    "b64": (1, 64, 8, 2, 90, [[90, 33]], 1.0),
+}
+
+
+@pytest.mark.parametrize("case", list(ATTN_CASES))
+def test_sparse_attn_matches_oracle(H, cuda, case):
+    batch, B, Hq, Hkv, cap, pool_len, q_scale = ATTN_CASES[case]
+    q, kb, vb, pk, pv, pl = _attn_case(cuda, batch, B, Hq, Hkv, cap, pool_len, seed=300 + len(case), q_scale=q_scale)
+    shape = H.make_shape(batch, Hq, Hkv, B, 16, 1, cap)
+    out = torch.full((batch, B, Hq, 128), float("nan"), dtype=torch.float32, device=cuda)
+    lse = torch.full((batch, B, Hq), float("nan"), dtype=torch.float32, device=cuda)
+    ws = H.alloc_workspace(H.herald_attn_workspace_bytes(shape), cuda)
+    H.herald_sparse_attn(shape, pk, pv, pl, q, kb, vb, out, lse, ws)
+    torch.cuda.synchronize()
+    pv_clean = pv.clone()
+    pv_clean[torch.isnan(pv_clean)] = 0
+    ref, lse_ref = O.sparse_attn(synth.to_u16(q), synth.to_u16(kb), synth.to_u16(vb), synth.to_u16(pk),
+                                 synth.to_u16(pv_clean), pl.cpu().numpy(), 128 ** -0.5)
+    err = np.abs(out.cpu().numpy().astype(np.float64) - ref).max()
+    assert np.isfinite(err) and err <= ATTN_TOL, (case, err)
+    assert np.abs(lse.cpu().numpy() - lse_ref).max() <= 2e-3
+
+
+@pytest.mark.parametrize("splits", [1, 2, 5])
+def test_sparse_attn_split_kv_is_consistent(H, cuda, splits, monkeypatch):
+    monkeypatch.setenv("HERALD_ATTN_SPLITS", str(splits))
+    batch, B, Hq, Hkv, cap = 1, 32, 14, 2, 600
+    q, kb, vb, pk, pv, pl = _attn_case(cuda, batch, B, Hq, Hkv, cap, [[600, 100]], seed=77)
+    shape = H.make_shape(batch, Hq, Hkv, B, 16, 1, cap)
+    out = torch.empty((batch, B, Hq, 128), dtype=torch.float32, device=cuda)
+    ws = H.alloc_workspace(H.herald_attn_workspace_bytes(shape), cuda)
+    H.herald_sparse_attn(shape, pk, pv, pl, q, kb, vb, out, None, ws)
+    torch.cuda.synchronize()
+    pv_clean = pv.clone()
+    pv_clean[torch.isnan(pv_clean)] = 0
+    ref, _ = O.sparse_attn(synth.to_u16(q), synth.to_u16(kb), synth.to_u16(vb), synth.to_u16(pk),
+                           synth.to_u16(pv_clean), pl.cpu().numpy(), 128 ** -0.5)
+    assert np.abs(out.cpu().numpy() - ref).max() <= ATTN_TOL
+
+
+def _layer_inputs(w, inp, ks, cuda):
+    return dict(k_pages=inp["k_pages"], v_pages=inp["v_pages"], page_table=inp["page_table"], seq_lens=inp["seq_lens"],
+                q_rep=inp["q_rep"], k_per_seq=torch.tensor(ks, dtype=torch.int32, device=cuda),
+                q_blk=inp["q_blk"], k_blk=inp["k_blk"], v_blk=inp["v_blk"])
+
+
+@pytest.mark.parametrize("start_after", [0, 2])
+def test_pipeline_step_matches_sequential_oracle(H, cuda, start_after):
+    w = synth.Workload("pipe", 2, (3000, 1111), 28, 4, 32, 5, 50, "planted", 10)
+    n_layers = 2
+    inps = [synth.make_inputs(w, seed=400 + l, device=cuda, spare_pages=1, hostile_tails=True) for l in range(n_layers)]
+    ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
+    cap = max(ks) + w.block_size
+    max_seq = (w.max_seq_len + 15) // 16 * 16
+    shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, max_seq, inps[0]["page_table"].shape[1], cap)
+    pipe = H.BlockPipeline(shape, [_layer_inputs(w, inp, ks, cuda) for inp in inps], w.n_attn_steps, start_after, cuda)
+    # active pool: random rows; idle pool: poison (must be fully overwritten up to sel_cnt and never read by attention)
+    g = torch.Generator(device=cuda)
+    g.manual_seed(5)
+    act_len = torch.tensor([[cap, 10, 0, 77], [1, cap - 1, 64, 65]], dtype=torch.int32, device=cuda)
+    for l in range(n_layers):
+        pipe.pools_k[l][0].copy_(torch.randn(pipe.pools_k[l][0].shape, generator=g, device=cuda).to(torch.bfloat16))
+        pipe.pools_v[l][0].copy_(torch.randn(pipe.pools_v[l][0].shape, generator=g, device=cuda).to(torch.bfloat16))
+        pipe.pool_lens[l][0].copy_(act_len)
+        pipe.pools_k[l][1].fill_(float("nan"))
+        pipe.pools_v[l][1].fill_(float("nan"))
+        pipe.pool_lens[l][1].fill_(-1)
+    act_k = [synth.to_u16(pipe.pools_k[l][0]) for l in range(n_layers)]
+    act_v = [synth.to_u16(pipe.pools_v[l][0]) for l in range(n_layers)]
+    assert pipe.active == 0
+    pipe.step()
+    torch.cuda.synchronize()
+    assert pipe.active == 1
+    layers_o = []
+    for l, inp in enumerate(inps):
+        oi = oracle_inputs(inp)
+        layers_o.append(dict(k_pages=oi["k_pages"], v_pages=oi["v_pages"], page_table=oi["page_table"], seq_lens=oi["seq_lens"],
+                             k_per_seq=ks, q_rep_next=oi["q_rep"], q_blk=synth.to_u16(inp["q_blk"]), k_blk=synth.to_u16(inp["k_blk"]),
+                             v_blk=synth.to_u16(inp["v_blk"]), pool_k=act_k[l], pool_v=act_v[l], pool_len=act_len.cpu().numpy(),
+                             pool_capacity=cap))
+    res = O.pipeline_step(layers_o, w.n_attn_steps, 128 ** -0.5)
+    for l in range(n_layers):
+        outs = pipe.outs[l].cpu().numpy()
+        for s in range(w.n_attn_steps):
+            assert np.abs(outs[s] - res[l]["outs"][s]).max() <= ATTN_TOL
+        pl = pipe.pool_lens[l][1].cpu().numpy()
+        assert np.array_equal(pl, res[l]["next_pool_len"])
+        pk, pv = synth.to_u16(pipe.pools_k[l][1]), synth.to_u16(pipe.pools_v[l][1])
+        sel_equal = True
+        for b in range(w.batch):
+            for h in range(w.n_kv_heads):
+                n = pl[b, h]
+                same = np.array_equal(pk[b, h, :n], res[l]["next_pool_k"][b, h, :n]) and np.array_equal(pv[b, h, :n], res[l]["next_pool_v"][b, h, :n])
+                sel_equal &= same
+                assert torch.isnan(pipe.pools_k[l][1][b, h, n:].float()).all(), "rows past sel_cnt must stay untouched"
+        assert sel_equal, "pool after the swap differs from the oracle's pool (index sets were expected to be equal here)"
+    # second block: the new active pool (buffer 1) must now be the one attention reads
+    pipe.step()
+    torch.cuda.synchronize()
+    assert pipe.active == 0
+    for l in range(n_layers):
+        ref, _ = O.sparse_attn(layers_o[l]["q_blk"][0], layers_o[l]["k_blk"][0], layers_o[l]["v_blk"][0],
+                               res[l]["next_pool_k"], res[l]["next_pool_v"], res[l]["next_pool_len"], 128 ** -0.5)
+        assert np.abs(pipe.outs[l][0].cpu().numpy() - ref).max() <= ATTN_TOL
+
+
+def test_pipeline_host_io_roundtrip(H, cuda):
+    w = synth.Workload("pipeh", 1, (1024,), 8, 2, 16, 3, 100, "plain")
+    inp = synth.make_inputs(w, seed=9, device=cuda)
+    ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
+    cap = max(ks) + w.block_size
+    shape = H.make_shape(1, 8, 2, 16, 1024, 64, cap)
+    dev_layer = _layer_inputs(w, inp, ks, cuda)
+    host = {n: inp[n].cpu().pin_memory() for n in ("q_rep", "q_blk", "k_blk", "v_blk")}
+    for n in ("q_rep", "q_blk", "k_blk", "v_blk"):       # device staging buffers start out as garbage
+        dev_layer[n] = torch.zeros_like(inp[n])
+    pipe = H.BlockPipeline(shape, [dev_layer], w.n_attn_steps, 0, cuda)
+    host["out"] = torch.zeros(pipe.outs[0].shape, dtype=torch.float32).pin_memory()
+    io = pipe.make_host_io([host])
+    pipe.step_host(io)
+    pipe.step_host(io)       # second block attends over the pool selected by the first
+    torch.cuda.synchronize()
+    oi = oracle_inputs(inp)
+    sel, _ = O.select(oi["q_rep"], oi["k_pages"], oi["page_table"], oi["seq_lens"], ks, 2, 128 ** -0.5)
+    pk, pv, pl = O.gather(oi["k_pages"], oi["v_pages"], oi["page_table"], sel, cap)
+    for s in range(w.n_attn_steps):
+        ref, _ = O.sparse_attn(synth.to_u16(inp["q_blk"][s]), synth.to_u16(inp["k_blk"][s]), synth.to_u16(inp["v_blk"][s]), pk, pv, pl, 128 ** -0.5)
+        assert np.abs(host["out"][s].numpy() - ref).max() <= ATTN_TOL
+
+
+def test_full_budget_equals_dense_attention(H, cuda):
+    """north_star invariant on the GPU path: budget 100 % => select->gather->attention == dense attention."""
+    w = synth.Workload("dense", 2, (777, 130), 8, 2, 16, 2, 1000, "plain")
+    inp = synth.make_inputs(w, seed=10, device=cuda, hostile_tails=True)
+    ks = list(w.seq_lens)
+    shape, cache, k_per_seq, sel_idx, sel_cnt, _ = run_select(H, w, inp, ks, cap=777, want_scores=False)
+    pool_k = torch.zeros((2, 2, 777, 128), dtype=torch.bfloat16, device=cuda)
+    pool_v = torch.zeros_like(pool_k)
+    H.herald_gather(shape, cache, sel_idx, sel_cnt, pool_k, pool_v)
+    out = torch.empty((2, 16, 8, 128), dtype=torch.float32, device=cuda)
+    ws = H.alloc_workspace(H.herald_attn_workspace_bytes(shape), cuda)
+    H.herald_sparse_attn(shape, pool_k, pool_v, sel_cnt, inp["q_blk"][0], inp["k_blk"][0], inp["v_blk"][0], out, None, ws)
+    torch.cuda.synchronize()
+    # dense reference with torch fp64 on the un-paged cache
+    pt = inp["page_table"].cpu()
+    for b, L in enumerate(w.seq_lens):
+        phys = pt[b, :(L + 15) // 16].long().to(cuda)
+        K = inp["k_pages"][phys].reshape(-1, 2, 128)[:L].double()
+        V = inp["v_pages"][phys].reshape(-1, 2, 128)[:L].double()
+        K = torch.cat([K, inp["k_blk"][0, b].double()], 0)
+        V = torch.cat([V, inp["v_blk"][0, b].double()], 0)
+        for hq in range(8):
+            logits = inp["q_blk"][0, b, :, hq].double() @ K[:, hq // 4].T * 128 ** -0.5
+            ref = torch.softmax(logits, -1) @ V[:, hq // 4]
+            assert (out[b, :, hq].double() - ref).abs().max().item() <= ATTN_TOL
