@@ -170,6 +170,17 @@ typedef struct herald_pipeline {
 
 int herald_pipeline_step(herald_pipeline_t* pipe);
 
+/* Optional timing hooks for the retrieval stream (measurement only, no effect on results): caller-created
+ * events recorded on the retrieval stream around the stages of the LAST layer's selection inside
+ * herald_pipeline_step.  Any member may be NULL.  scan = score scan (+ aggregation in mode 1),
+ * topk = radix select, gather = pool fill.  Pass NULL to herald_pipeline_set_profile to switch off. */
+typedef struct herald_profile {
+    herald_event_t scan_begin, scan_end, topk_end, gather_end;
+} herald_profile_t;
+
+/* Stores `prof` (host pointer, must outlive the following pipeline steps) for this thread.  Host only. */
+int herald_pipeline_set_profile(const herald_profile_t* prof);
+
 /* Host-buffer variant used for end-to-end timing: per block, the step's inputs come from (pinned)
  * HOST memory and its outputs return to HOST memory, all asynchronously on the pipeline's streams:
  *   H2D  host_q_rep[l] -> layers[l].q_rep ; host_q_blk/k_blk/v_blk[l] -> layers[l].q_blk/k_blk/v_blk

@@ -16,6 +16,8 @@
 namespace herald {
 
 static thread_local char g_err[512] = "";
+static thread_local const herald_profile_t* g_prof = nullptr;   // timing hooks (herald_pipeline_set_profile)
+static thread_local bool g_prof_armed = false;                   // true only inside the last layer's retrieval
 
 static int fail(int code, const char* fmt, ...) {
     va_list ap;
@@ -182,6 +184,8 @@ int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, cons
     float* scores = scores_out ? scores_out : reinterpret_cast<float*>(wsb + w.scores);
     cudaError_t e = cudaMemsetAsync(hist1, 0, (size_t)units * kBins1 * sizeof(uint32_t), stream);
     if (e != cudaSuccess) return cuda_fail(e, "memset hist1");
+    const herald_profile_t* prof = g_prof_armed ? g_prof : nullptr;
+    if (prof && prof->scan_begin) cudaEventRecord(static_cast<cudaEvent_t>(prof->scan_begin), stream);
 
     if (shape->max_seq_len > 0) {
         ScanParams sp{};
@@ -225,6 +229,7 @@ int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, cons
         if (e != cudaSuccess) return cuda_fail(e, "scan launch");
     }
 
+    if (prof && prof->scan_end) cudaEventRecord(static_cast<cudaEvent_t>(prof->scan_end), stream);
     TopkParams tp{};
     tp.scores = scores;
     tp.hist1 = hist1;
@@ -238,6 +243,7 @@ int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, cons
     topk_kernel<<<units, kTopkThreads, 0, stream>>>(tp);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "topk launch");
+    if (prof && prof->topk_end) cudaEventRecord(static_cast<cudaEvent_t>(prof->topk_end), stream);
     return HERALD_OK;
 }
 
@@ -365,11 +371,15 @@ int herald_pipeline_step(herald_pipeline_t* p) {
         if (e != cudaSuccess) return cuda_fail(e, "wait fork");
         for (int l = 0; l < p->n_layers; ++l) {
             herald_layer_t* ly = &p->layers[l];
+            g_prof_armed = (l == p->n_layers - 1);
             int r = herald_select(sh, &ly->cache, ly->q_rep, ly->k_per_seq, p->sel_idx, ly->pool_len[idle], nullptr,
                                   p->ws_select, p->ws_select_bytes, s_ret);
+            g_prof_armed = false;
             if (r) return r;
             r = herald_gather(sh, &ly->cache, p->sel_idx, ly->pool_len[idle], ly->pool_k[idle], ly->pool_v[idle], s_ret);
             if (r) return r;
+            if (l == p->n_layers - 1 && g_prof && g_prof->gather_end)
+                cudaEventRecord(static_cast<cudaEvent_t>(g_prof->gather_end), s_ret);
         }
         e = cudaEventRecord(ev_join, s_ret);
         if (e != cudaSuccess) return cuda_fail(e, "record join");
@@ -397,6 +407,11 @@ int herald_pipeline_step(herald_pipeline_t* p) {
     e = cudaStreamWaitEvent(s_main, ev_join, 0);
     if (e != cudaSuccess) return cuda_fail(e, "wait join");
     p->active = idle;
+    return HERALD_OK;
+}
+
+int herald_pipeline_set_profile(const herald_profile_t* prof) {
+    g_prof = prof;
     return HERALD_OK;
 }
 

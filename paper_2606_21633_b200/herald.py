@@ -25,7 +25,7 @@ AGG_MAX_LOGIT, AGG_SOFTMAX_SUM = 0, 1
 
 EXPORTS = ("herald_last_error", "herald_budget_rows", "herald_select_workspace_bytes",
            "herald_attn_workspace_bytes", "herald_select", "herald_gather", "herald_sparse_attn",
-           "herald_pipeline_step", "herald_pipeline_step_host")
+           "herald_pipeline_step", "herald_pipeline_step_host", "herald_pipeline_set_profile")
 
 
 class HeraldError(RuntimeError):
@@ -66,6 +66,11 @@ class HostIO(C.Structure):
     _fields_ = [("host_q_rep", C.POINTER(C.c_void_p)), ("host_q_blk", C.POINTER(C.c_void_p)),
                 ("host_k_blk", C.POINTER(C.c_void_p)), ("host_v_blk", C.POINTER(C.c_void_p)),
                 ("host_out", C.POINTER(C.c_void_p))]
+
+
+class Profile(C.Structure):
+    _fields_ = [("scan_begin", C.c_void_p), ("scan_end", C.c_void_p), ("topk_end", C.c_void_p),
+                ("gather_end", C.c_void_p)]
 
 
 _lib.herald_last_error.restype = C.c_char_p
@@ -175,6 +180,15 @@ def herald_pipeline_step(pipe: Pipeline):
 
 def herald_pipeline_step_host(pipe: Pipeline, io: HostIO):
     _check(_lib.herald_pipeline_step_host(C.byref(pipe), C.byref(io)))
+
+
+_lib.herald_pipeline_set_profile.restype = C.c_int
+_lib.herald_pipeline_set_profile.argtypes = [C.POINTER(Profile)]
+
+
+def herald_pipeline_set_profile(prof):
+    """prof: a Profile struct (kept alive by the caller) or None."""
+    _check(_lib.herald_pipeline_set_profile(C.byref(prof) if prof is not None else None))
 
 
 def alloc_workspace(nbytes: int, device) -> torch.Tensor:

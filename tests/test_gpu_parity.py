@@ -70,7 +70,8 @@ def test_select_matches_oracle(H, cuda, case, agg_mode):
         for b in range(w.batch):
             for h in range(w.n_kv_heads):
                 planted = set(inp["planted"][b][h].tolist())
-                assert len(planted - set(sel_o[b][h].tolist())) <= max(1, len(planted) // 8)
+                if 2 * len(planted) <= ks[b]:     # the budget has room: keys shifted +4 sigma toward q_rep must be recalled
+                    assert len(planted - set(sel_g[b, h, :ks[b]].tolist())) <= max(1, len(planted) // 8)
 
 
 def test_select_edge_cases(H, cuda):
