@@ -45,6 +45,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cmd = [nvcc_path(), "-shared", "-Xcompiler", "-fPIC", "-std=c++17", "-O3", "-lineinfo",
            "-gencode", "arch=compute_100a,code=sm_100a", "-I", os.path.join(ROOT, "include"),
            "-o", LIB] + SOURCES
+    cmd[1:1] = os.environ.get("HERALD_NVCC_FLAGS", "").split()
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     res = subprocess.run(cmd, capture_output=True, text=True)

@@ -7,7 +7,7 @@
 #include <cstdlib>
 #include <cstring>
 
-#include "attn_mma.cuh"
+#include "attn_tc.cuh"
 #include "common.cuh"
 #include "gather.cuh"
 #include "scan.cuh"
@@ -118,13 +118,14 @@ static AttnGeom attn_geom(const herald_shape_t* s) {
     const int G = s->n_q_heads / s->n_kv_heads;
     const int M = s->block_size * G;
     const int units = s->batch * s->n_kv_heads;
-    a.m_tiles = (M + kAttnBM - 1) / kAttnBM;
-    a.m_pad = a.m_tiles * kAttnBM;
-    const int max_tiles = (s->pool_capacity + s->block_size + kAttnBN - 1) / kAttnBN;
-    const int target = env_int("HERALD_ATTN_TOTAL_CTAS", 148 * 3);
-    int splits = units > 0 ? (target + units * a.m_tiles - 1) / (units * a.m_tiles) : 1;
-    if (splits > max_tiles / 2) splits = max_tiles / 2;
-    if (splits > 32) splits = 32;
+    a.m_tiles = (M + kTcBM - 1) / kTcBM;
+    a.m_pad = a.m_tiles * kTcBM;
+    // one CTA per SM: split the keys of a unit until the grid covers the 148 SMs once
+    const int max_tiles = (s->pool_capacity + s->block_size + kTcBN - 1) / kTcBN;
+    const int target = env_int("HERALD_ATTN_TOTAL_CTAS", 148);
+    int splits = units > 0 ? target / (units * a.m_tiles) : 1;
+    if (splits > max_tiles) splits = max_tiles;
+    if (splits > 16) splits = 16;
     if (splits < 1) splits = 1;
     const int forced = env_int("HERALD_ATTN_SPLITS", 0);
     if (forced > 0) splits = forced < max_tiles ? forced : (max_tiles > 0 ? max_tiles : 1);
@@ -136,6 +137,42 @@ static AttnGeom attn_geom(const herald_shape_t* s) {
     if (splits > 1) off = align_up(off + (size_t)units * splits * a.m_pad * sizeof(float2), 256);
     a.total = off > 256 ? off : 256;
     return a;
+}
+
+// ---- TMA tensor maps (driver entry point resolved at run time; libcuda is not linked) -------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* ptr = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(ptr);
+    }
+    return fn;
+}
+
+// bf16 pool [units][cap][128] as a 3-D tensor (d, row, unit); box = 64 channels x 128 rows, 128-byte swizzle:
+// the box lands in shared memory exactly in the UMMA canonical layout (K-major for K, MN-major for V).
+static int make_pool_map(CUtensorMap* map, const void* pool, int units, int cap) {
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
+    const cuuint64_t rows = cap > 0 ? cap : 1;
+    const cuuint64_t dims[3] = {(cuuint64_t)kHeadDim, rows, (cuuint64_t)units};
+    const cuuint64_t strides[2] = {(cuuint64_t)kRowBytes, (cuuint64_t)cap * kRowBytes > 0 ? (cuuint64_t)cap * kRowBytes : kRowBytes};
+    const cuuint32_t box[3] = {64u, (cuuint32_t)(rows < (cuuint64_t)kTcBN ? rows : kTcBN), 1u};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(pool), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+    return HERALD_OK;
 }
 
 }  // namespace herald
@@ -302,10 +339,15 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
 
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(attn_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kAttnSmemBytes);
+        cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes);
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(attn)");
         attr_set = true;
     }
+    CUtensorMap tm_k, tm_v;
+    rc = make_pool_map(&tm_k, pool_k, units, shape->pool_capacity);
+    if (rc) return rc;
+    rc = make_pool_map(&tm_v, pool_v, units, shape->pool_capacity);
+    if (rc) return rc;
     AttnParams ap{};
     ap.pool_k = static_cast<const __nv_bfloat16*>(pool_k);
     ap.pool_v = static_cast<const __nv_bfloat16*>(pool_v);
@@ -324,8 +366,8 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
     ap.n_splits = a.n_splits;
     ap.m_pad = a.m_pad;
     ap.scale_log2 = shape->sm_scale * 1.4426950408889634f;
-    dim3 grid(a.m_tiles, a.n_splits, units);
-    attn_mma_kernel<<<grid, kAttnThreads, kAttnSmemBytes, stream>>>(ap);
+    dim3 grid(a.n_splits, a.m_tiles, units);
+    attn_tc_kernel<<<grid, kTcThreads, kTcSmemBytes, stream>>>(tm_k, tm_v, ap);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "attention launch");
     if (a.n_splits > 1) {
