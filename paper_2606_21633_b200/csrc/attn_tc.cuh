@@ -8,17 +8,18 @@
 // tcgen05.mma (UMMA M=128, bf16 x bf16 -> fp32; P enters the PV product as a bf16 hi+lo pair) with the
 // accumulators in TMEM:
 //
-//   grid  = (KV splits, M tiles of 128 rows, units), 320 threads, 1 CTA / SM
-//   warp 8      producer: full 128-key pool tiles arrive by TMA (cp.async.bulk.tensor, 128B swizzle,
-//               2-stage K/V ring); the ragged tail of the pool and the in-block rows are written with
-//               zero-filling cp.async so that rows past the end are exact zeros
-//   warp 9      issues the MMAs (one elected lane): S[j&1] = Q K_j^T into a double-buffered TMEM tile,
-//               then O += P_{j-1} V_{j-1}; completion is signalled with tcgen05.commit -> mbarrier
+//   grid  = (KV splits, M tiles of 128 rows, units), 352 threads, 1 CTA / SM
+//   warps 8, 9  producers, one for K and one for V: whole 128-key pool tiles arrive by TMA (cp.async.bulk.tensor,
+//               128B swizzle) into 3-stage rings; a K stage is released as soon as QK^T has read it, a V stage
+//               after PV.  The ragged tail of the pool and the in-block rows are written with zero-filling
+//               cp.async, so rows past the end are exact zeros.
+//   warp 10     issues the MMAs (one lane): S[j&1] = Q K_j^T (operands in shared memory) into a double-buffered
+//               TMEM tile, then O += P_{j-1} V_{j-1} with P read from TMEM; tcgen05.commit -> mbarrier
 //   warps 0..7  softmax: thread (row, column half) reads 64 logits of its row from TMEM (tcgen05.ld),
-//               exchanges the row maximum with its partner warp, exponentiates (ex2), accumulates the
-//               row sum, splits P into a bf16 hi+lo pair and stores both to shared memory in the UMMA K-major layout.
+//               exchanges the row maximum with its partner warp, exponentiates (ex2), accumulates the row sum,
+//               splits P into a bf16 hi+lo pair and writes both back over S_j in TMEM (tcgen05.st).
 //               The running maximum is only raised when it grows by more than 2^8 ("lazy rescale"):
-//               O in TMEM is then rescaled in place (tcgen05.ld / tcgen05.st), which is rare.
+//               O in TMEM is then rescaled in place, which is rare.
 //   split-KV partials (unnormalised O, running max, row sum) go to the workspace and are merged by
 //   attn_combine_kernel; with one split the epilogue normalises and writes `out` directly.
 #pragma once
@@ -30,26 +31,27 @@ namespace herald {
 
 constexpr int kTcBM = 128;                       // query rows per CTA (UMMA M)
 constexpr int kTcBN = 128;                       // keys per tile (UMMA N of QK^T, K of PV)
-constexpr int kTcStages = 2;                     // K/V ring depth
-constexpr int kTcThreads = 320;                  // 8 softmax warps + producer + MMA issuer
-constexpr int kTcProducerWarp = 8, kTcMmaWarp = 9;
+constexpr int kTcStages = 3;                     // depth of the K ring and of the V ring
+constexpr int kTcThreads = 352;                  // 8 softmax warps + K producer + V producer + MMA issuer
+constexpr int kTcKWarp = 8, kTcVWarp = 9, kTcMmaWarp = 10;
 constexpr int kTcHalfBytes = kTcBN * 128;        // one [128 rows x 64 el] swizzled half tile (16 KB)
-constexpr int kTcTileBytes = 2 * kTcHalfBytes;   // a [128 x 128] 16-bit tile = two halves (32 KB)
+constexpr int kTcTileBytes = 2 * kTcHalfBytes;   // a [128 x 128] bf16 tile = two halves (32 KB)
 constexpr int kTcSmemQ = 0;
-constexpr int kTcSmemP = kTcSmemQ + kTcTileBytes;                        // P_hi, then P_lo (bf16 pair, see below)
-constexpr int kTcSmemKV = kTcSmemP + 2 * kTcTileBytes;                   // stage s: K at +2s tiles, V at +(2s+1)
-constexpr int kTcSmemMisc = kTcSmemKV + kTcStages * 2 * kTcTileBytes;    // barriers, TMEM pointer, exchange buffers
+constexpr int kTcSmemK = kTcSmemQ + kTcTileBytes;                        // K ring
+constexpr int kTcSmemV = kTcSmemK + kTcStages * kTcTileBytes;            // V ring
+constexpr int kTcSmemMisc = kTcSmemV + kTcStages * kTcTileBytes;         // barriers, TMEM pointer, exchange buffers
 constexpr int kTcMiscBytes = 2304;
 constexpr int kTcSmemBytes = kTcSmemMisc + kTcMiscBytes;                 // 231,680 B of the 232,448 B a CTA may own
-constexpr int kTcTmemCols = 512;                 // S0 [0,128) S1 [128,256) O [256,384)
+constexpr int kTcTmemCols = 512;                 // S0/P0 [0,128) S1/P1 [128,256) O [256,384)
 constexpr float kTcRescaleThreshold = 8.f;       // log2 units
 
 // barrier slots (8 bytes each) inside the misc area
-enum { kBarKvFull = 0, kBarKvEmpty = kBarKvFull + kTcStages, kBarSFull = kBarKvEmpty + kTcStages, kBarSFree = kBarSFull + 2,
-       kBarPFull = kBarSFree + 2, kBarPvDone, kBarCount };
-constexpr int kTcMiscTmemPtr = 128;              // uint32
+enum { kBarKFull = 0, kBarKEmpty = kBarKFull + kTcStages, kBarVFull = kBarKEmpty + kTcStages, kBarVEmpty = kBarVFull + kTcStages,
+       kBarSFull = kBarVEmpty + kTcStages, kBarPFull = kBarSFull + 2, kBarPvDone, kBarCount = kBarPvDone + 2 };
+constexpr int kTcMiscTmemPtr = 192;              // uint32
 constexpr int kTcMiscMax = 256;                  // float [2 buffers][2 halves][128 rows]
 constexpr int kTcMiscSum = kTcMiscMax;           // float [2 halves][128 rows]; reuses the max buffer after the last tile
+static_assert(kBarCount * 8 <= kTcMiscTmemPtr, "barriers overlap the TMEM pointer slot");
 
 struct AttnParams {
     const __nv_bfloat16* pool_k;
@@ -116,6 +118,15 @@ __device__ __forceinline__ void umma_ss(uint32_t d_tmem, uint64_t a_desc, uint64
         "setp.ne.b32 p, %4, 0;\n\t"
         "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
         "}" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// D[tmem] (+)= A[tmem] * B[smem desc]; A: row = TMEM lane, two 16-bit K elements per 32-bit column
+__device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
+        "}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
@@ -192,7 +203,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     const int n_full = n_pool / kTcBN;                       // tiles [0, n_full) are whole pool tiles -> TMA
     const int per = (n_tiles + p.n_splits - 1) / p.n_splits;
     const int t0 = split * per, t1 = min(n_tiles, t0 + per);
-    const int nt = t1 - t0;                                  // tile j of this CTA is key tile t1-1-j (ragged tiles first)
+    const int nt = t1 - t0;                                  // tile j of this CTA is key tile t0 + j (ragged tiles last)
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int64_t part_base = ((int64_t)unit * p.n_splits + split) * p.m_pad + mtile * kTcBM;
 
@@ -212,17 +223,16 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(misc + kTcMiscTmemPtr), "n"(kTcTmemCols));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
-    if (warp == kTcProducerWarp && lane == 0) {
+    if (warp == kTcKWarp && lane == 0) {
         for (int s = 0; s < kTcStages; ++s) {
-            mbar_init(bar(kBarKvFull + s), 1);
-            mbar_init(bar(kBarKvEmpty + s), 1);
+            mbar_init(bar(kBarKFull + s), 1);
+            mbar_init(bar(kBarKEmpty + s), 1);
+            mbar_init(bar(kBarVFull + s), 1);
+            mbar_init(bar(kBarVEmpty + s), 1);
         }
-        for (int s = 0; s < 2; ++s) {
-            mbar_init(bar(kBarSFull + s), 1);
-            mbar_init(bar(kBarSFree + s), 8);
-        }
+        for (int s = 0; s < 2; ++s) mbar_init(bar(kBarSFull + s), 1);
         mbar_init(bar(kBarPFull), 8);
-        mbar_init(bar(kBarPvDone), 1);
+        for (int s = 0; s < 2; ++s) mbar_init(bar(kBarPvDone + s), 1);   // PV_j commits to slot j&1 (see the epilogue wait)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_k) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_v) : "memory");
@@ -242,93 +252,80 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     const uint32_t tmem = *tmem_ptr_gen;
 
     auto tile_cols = [&](int j) {   // key columns of this CTA's j-th tile that the MMAs touch (multiple of 16)
-        const int t = t1 - 1 - j;
-        const int valid = min(kTcBN, N - t * kTcBN);
+        const int valid = min(kTcBN, N - (t0 + j) * kTcBN);
         return (valid + 15) & ~15;
     };
 
-    if (warp == kTcProducerWarp) {
-        // =========================== producer ===========================
-        auto issue_tma = [&](int j) {
-            const int t = t1 - 1 - j, stage = j % kTcStages;
-            if (lane == 0) {
-                const uint32_t kdst = sbase + kTcSmemKV + stage * 2 * kTcTileBytes, vdst = kdst + kTcTileBytes;
-                const uint32_t full = bar(kBarKvFull + stage);
-                mbar_arrive_expect_tx(full, 2 * kTcTileBytes);
-                tma_load_3d(kdst, &tm_k, 0, t * kTcBN, unit, full);
-                tma_load_3d(kdst + kTcHalfBytes, &tm_k, 64, t * kTcBN, unit, full);
-                tma_load_3d(vdst, &tm_v, 0, t * kTcBN, unit, full);
-                tma_load_3d(vdst + kTcHalfBytes, &tm_v, 64, t * kTcBN, unit, full);
-            }
-        };
-        auto fill_manual = [&](int j) {
-            const int t = t1 - 1 - j, stage = j % kTcStages;
-            const uint32_t kdst = sbase + kTcSmemKV + stage * 2 * kTcTileBytes, vdst = kdst + kTcTileBytes;
-            const int rows = tile_cols(j);
-            for (int c = lane; c < rows * 16; c += 32) {
-                const int r = c >> 4, ch = c & 15;
-                const int kj = t * kTcBN + r;
-                const __nv_bfloat16 *ksrc = p.pool_k, *vsrc = p.pool_v;
-                int bytes = 0;
-                if (kj < n_pool) {
-                    const int64_t off = ((int64_t)unit * p.cap + kj) * kHeadDim + ch * 8;
-                    ksrc = p.pool_k + off;
-                    vsrc = p.pool_v + off;
-                    bytes = 16;
-                } else if (kj < N) {
-                    const int64_t off = (((int64_t)b * B + (kj - n_pool)) * p.n_kv_heads + h) * kHeadDim + ch * 8;
-                    ksrc = p.k_blk + off;
-                    vsrc = p.v_blk + off;
-                    bytes = 16;
+    if (warp == kTcKWarp || warp == kTcVWarp) {
+        // =========================== producers: one warp streams K tiles, one streams V tiles ===========================
+        const bool is_k = warp == kTcKWarp;
+        const CUtensorMap* map = is_k ? &tm_k : &tm_v;
+        const __nv_bfloat16* pool = is_k ? p.pool_k : p.pool_v;
+        const __nv_bfloat16* blk = is_k ? p.k_blk : p.v_blk;
+        const int bar_full = is_k ? kBarKFull : kBarVFull, bar_empty = is_k ? kBarKEmpty : kBarVEmpty;
+        const uint32_t ring = sbase + (is_k ? kTcSmemK : kTcSmemV);
+        for (int j = 0; j < nt; ++j) {
+            const int stage = j % kTcStages, t = t0 + j;
+            if (j >= kTcStages) mbar_wait(bar(bar_empty + stage), ((j / kTcStages) - 1) & 1);
+            const uint32_t dst = ring + stage * kTcTileBytes, full = bar(bar_full + stage);
+            if (t < n_full) {
+                if (lane == 0) {
+                    mbar_arrive_expect_tx(full, kTcTileBytes);
+                    tma_load_3d(dst, map, 0, t * kTcBN, unit, full);
+                    tma_load_3d(dst + kTcHalfBytes, map, 64, t * kTcBN, unit, full);
                 }
-                const uint32_t dst = (ch >> 3) * kTcHalfBytes + r * 128 + (((ch & 7) ^ (r & 7)) << 4);
-                cp_async_16_zfill(kdst + dst, ksrc, bytes);
-                cp_async_16_zfill(vdst + dst, vsrc, bytes);
+            } else {
+                // ragged tile (pool tail and/or in-block rows): zero-filling 16-byte cp.async, rows past N are zeros
+                const int rows = tile_cols(j);
+                for (int c = lane; c < rows * 16; c += 32) {
+                    const int r = c >> 4, ch = c & 15;
+                    const int kj = t * kTcBN + r;
+                    const __nv_bfloat16* src = pool;
+                    int bytes = 0;
+                    if (kj < n_pool) {
+                        src = pool + ((int64_t)unit * p.cap + kj) * kHeadDim + ch * 8;
+                        bytes = 16;
+                    } else if (kj < N) {
+                        src = blk + (((int64_t)b * B + (kj - n_pool)) * p.n_kv_heads + h) * kHeadDim + ch * 8;
+                        bytes = 16;
+                    }
+                    cp_async_16_zfill(dst + (ch >> 3) * kTcHalfBytes + r * 128 + (((ch & 7) ^ (r & 7)) << 4), src, bytes);
+                }
+                cp_async_wait_all();
+                fence_proxy_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(full);
             }
-            cp_async_wait_all();
-            fence_proxy_async_smem();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar(kBarKvFull + stage));
-        };
-        const int first = min(nt, kTcStages);
-        for (int j = 0; j < first; ++j)
-            if (t1 - 1 - j < n_full) issue_tma(j);          // asynchronous tiles first, so they fly during the manual fills
-        for (int j = 0; j < first; ++j)
-            if (t1 - 1 - j >= n_full) fill_manual(j);
-        for (int j = kTcStages; j < nt; ++j) {
-            mbar_wait(bar(kBarKvEmpty + j % kTcStages), ((j / kTcStages) - 1) & 1);
-            if (t1 - 1 - j < n_full) issue_tma(j);
-            else fill_manual(j);
         }
     } else if (warp == kTcMmaWarp) {
         // =========================== MMA issuer ===========================
         constexpr uint32_t idesc_pv = umma_idesc(/*A bf16*/ 1, /*B bf16*/ 1, /*A K-major*/ 0, /*B MN-major*/ 1, kTcBM, kHeadDim);
-        const uint32_t q_base = sbase + kTcSmemQ, p_base = sbase + kTcSmemP;
-        auto issue_pv = [&](int j) {   // O (+)= P_j V_j
-            const int stage = j % kTcStages;
+        const uint32_t q_base = sbase + kTcSmemQ;
+        auto issue_pv = [&](int j) {   // O (+)= (P_hi + P_lo)_j V_j, P read from TMEM (it overlays S_j)
+            const int stage = j % kTcStages, sb = j & 1;
+            mbar_wait(bar(kBarVFull + stage), (j / kTcStages) & 1);
             mbar_wait(bar(kBarPFull), j & 1);
             tc_fence_after();
             if (lane == 0) {
-                const uint32_t v_base = sbase + kTcSmemKV + stage * 2 * kTcTileBytes + kTcTileBytes;
+                const uint32_t v_base = sbase + kTcSmemV + stage * kTcTileBytes;
                 const int ksteps = tile_cols(j) >> 4;
                 for (int kk = 0; kk < ksteps; ++kk) {
-                    const uint32_t a_off = (kk >> 2) * kTcHalfBytes + (kk & 3) * 32;
                     const uint64_t bd = umma_desc_sw128(v_base + kk * 2048, kTcHalfBytes, 1024);
-                    umma_ss(tmem + 256, umma_desc_sw128(p_base + a_off, 16, 1024), bd, idesc_pv, (j > 0 || kk > 0) ? 1u : 0u);
-                    umma_ss(tmem + 256, umma_desc_sw128(p_base + kTcTileBytes + a_off, 16, 1024), bd, idesc_pv, 1u);
+                    umma_ts(tmem + 256, tmem + sb * 128 + kk * 8, bd, idesc_pv, (j > 0 || kk > 0) ? 1u : 0u);
+                    umma_ts(tmem + 256, tmem + sb * 128 + 64 + kk * 8, bd, idesc_pv, 1u);
                 }
-                umma_commit(bar(kBarPvDone));
-                umma_commit(bar(kBarKvEmpty + stage));
+                umma_commit(bar(kBarPvDone + sb));
+                umma_commit(bar(kBarVEmpty + stage));
             }
             __syncwarp();
         };
         for (int j = 0; j < nt; ++j) {
             const int stage = j % kTcStages, sb = j & 1;
-            mbar_wait(bar(kBarKvFull + stage), (j / kTcStages) & 1);
-            if (j >= 2) mbar_wait(bar(kBarSFree + sb), ((j >> 1) - 1) & 1);
+            mbar_wait(bar(kBarKFull + stage), (j / kTcStages) & 1);
             tc_fence_after();
             if (lane == 0) {
-                const uint32_t k_base = sbase + kTcSmemKV + stage * 2 * kTcTileBytes;
+                // S_j overwrites the TMEM columns of P_{j-2}: PV_{j-2} was issued earlier and the tensor pipe runs in order
+                const uint32_t k_base = sbase + kTcSmemK + stage * kTcTileBytes;
                 const uint32_t idesc_s = umma_idesc(1, 1, 0, 0, kTcBM, tile_cols(j));
 #pragma unroll
                 for (int ks = 0; ks < 8; ++ks) {
@@ -337,6 +334,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                             idesc_s, ks > 0 ? 1u : 0u);
                 }
                 umma_commit(bar(kBarSFull + sb));
+                umma_commit(bar(kBarKEmpty + stage));
             }
             __syncwarp();
             if (j > 0) issue_pv(j - 1);
@@ -350,6 +348,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
         float m_used = -INFINITY, l = 0.f;
         for (int j = 0; j < nt; ++j) {
             const int sb = j & 1;
+            // S_j complete; the commit also covers PV_{j-2}, so the P columns overlaying this S buffer are free
             mbar_wait(bar(kBarSFull + sb), (j >> 1) & 1);
             tc_fence_after();
             float s[64];
@@ -360,11 +359,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
 #pragma unroll
                 for (int i = 0; i < 32; ++i) { s[i] = a[i]; s[32 + i] = c[i]; }
             }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar(kBarSFree + sb));
-            const int t = t1 - 1 - j;
-            const int valid = N - t * kTcBN;                  // >= 1
+            const int valid = N - (t0 + j) * kTcBN;           // >= 1
             if (valid < kTcBN) {
 #pragma unroll
                 for (int i = 0; i < 64; ++i)
@@ -374,7 +369,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
 #pragma unroll
             for (int i = 1; i < 64; ++i) mx = fmaxf(mx, s[i]);
             ex_max[(sb * 2 + hf) * 128 + row] = mx;
-            named_bar_sync(1 + quarter, 64);
+            named_bar_sync(1 + quarter, 64);                  // both column halves of these 32 rows have read S_j
             const float mrow = fmaxf(mx, ex_max[(sb * 2 + (hf ^ 1)) * 128 + row]) * p.scale_log2;
             float alpha = 1.f;
             bool need = false;
@@ -393,41 +388,42 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 sum += s[i];
             }
             l = l * alpha + sum;
-            if (j > 0) {
-                mbar_wait(bar(kBarPvDone), (j - 1) & 1);       // PV_{j-1} finished: P buffer free, O up to date
+            if (any) {   // rare: the running maximum of some row grew by more than 2^8 -> rescale O in place
+                mbar_wait(bar(kBarPvDone + ((j - 1) & 1)), ((j - 1) >> 1) & 1);   // PV_{j-1} finished; PV_j waits for our arrive
                 tc_fence_after();
-                if (any) {
 #pragma unroll
-                    for (int q = 0; q < 2; ++q) {
-                        float o[32];
-                        tmem_ld32(lane_base + 256 + hf * 64 + q * 32, o);
+                for (int q = 0; q < 2; ++q) {
+                    float o[32];
+                    tmem_ld32(lane_base + 256 + hf * 64 + q * 32, o);
 #pragma unroll
-                        for (int i = 0; i < 32; ++i) o[i] *= alpha;
-                        tmem_st32(lane_base + 256 + hf * 64 + q * 32, o);
-                    }
-                    tmem_wait_st();
+                    for (int i = 0; i < 32; ++i) o[i] *= alpha;
+                    tmem_st32(lane_base + 256 + hf * 64 + q * 32, o);
                 }
             }
-            // P row (64 weights of this column half) -> shared memory, UMMA K-major 128B-swizzled, as the bf16 pair
-            // P = P_hi + P_lo: the pair carries 16 significand bits, so the PV product keeps the weights to ~2^-17
-            // relative and peaked rows stay inside the 2e-3 output tolerance.
-            uint8_t* prow = sgen + kTcSmemP + hf * kTcHalfBytes + row * 128;
+            // P = P_hi + P_lo (bf16 pair, 16 significand bits: the PV product keeps the weights to ~2^-17 relative, so
+            // peaked rows stay inside the 2e-3 output tolerance).  Both go to TMEM as the A operand of the PV MMA:
+            // row = lane, two keys per 32-bit column; P_hi in columns [0,64) of the S buffer, P_lo in [64,128).
+            {
+                float hi[32], lo[32];
 #pragma unroll
-            for (int c8 = 0; c8 < 8; ++c8) {
-                uint32_t hi[4], lo[4];
-#pragma unroll
-                for (int e = 0; e < 4; ++e) split_bf16(s[8 * c8 + 2 * e], s[8 * c8 + 2 * e + 1], hi[e], lo[e]);
-                const int off = (c8 ^ (row & 7)) << 4;
-                *reinterpret_cast<uint4*>(prow + off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-                *reinterpret_cast<uint4*>(prow + kTcTileBytes + off) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+                for (int i = 0; i < 32; ++i) {
+                    uint32_t h2, l2;
+                    split_bf16(s[2 * i], s[2 * i + 1], h2, l2);
+                    hi[i] = __uint_as_float(h2);
+                    lo[i] = __uint_as_float(l2);
+                }
+                tmem_st32(lane_base + sb * 128 + hf * 32, hi);
+                tmem_st32(lane_base + sb * 128 + 64 + hf * 32, lo);
             }
-            fence_proxy_async_smem();
+            tmem_wait_st();
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(kBarPFull));
         }
         // ---- epilogue: O / l -> out (one split) or partials (split-KV) ----
-        mbar_wait(bar(kBarPvDone), (nt - 1) & 1);
+        // A parity wait is only sound when the waiter is at most one phase behind.  The softmax warps do not wait for
+        // every PV, but S_j's commit covers PV_{j-2}, so with one barrier per tile parity the lag is at most one phase.
+        mbar_wait(bar(kBarPvDone + ((nt - 1) & 1)), ((nt - 1) >> 1) & 1);
         tc_fence_after();
         ex_sum[hf * 128 + row] = l;
         named_bar_sync(1 + quarter, 64);
