@@ -17,7 +17,10 @@ namespace herald {
 
 static thread_local char g_err[512] = "";
 static thread_local const herald_profile_t* g_prof = nullptr;   // timing hooks (herald_pipeline_set_profile)
-static thread_local bool g_prof_armed = false;                   // true only inside the last layer's retrieval
+static thread_local bool g_prof_armed = false;
+#ifdef HERALD_ATTN_TRACE
+static unsigned long long* g_attn_trace = nullptr;               // debug builds only: device buffer [CTAs][64]
+#endif                   // true only inside the last layer's retrieval
 
 static int fail(int code, const char* fmt, ...) {
     va_list ap;
@@ -109,33 +112,29 @@ static SelectWs select_ws_layout(const herald_shape_t* s) {
 
 // ---- attention launch geometry ----------------------------------------------------------------
 struct AttnGeom {
-    int m_tiles, m_pad, n_splits;
-    size_t part_o, part_ml, total;
+    int m_tiles, ipt, n_splits;
+    size_t total;
 };
 
 static AttnGeom attn_geom(const herald_shape_t* s) {
     AttnGeom a{};
     const int G = s->n_q_heads / s->n_kv_heads;
-    const int M = s->block_size * G;
     const int units = s->batch * s->n_kv_heads;
-    a.m_tiles = (M + kTcBM - 1) / kTcBM;
-    a.m_pad = a.m_tiles * kTcBM;
-    // one CTA per SM: split the keys of a unit until the grid covers the 148 SMs once
+    // an M tile is `ipt` whole block rows x G heads (<= 128 rows), balanced over the tiles
+    const int rows_cap = kTcBM / G;
+    a.m_tiles = (s->block_size + rows_cap - 1) / rows_cap;
+    a.ipt = (s->block_size + a.m_tiles - 1) / a.m_tiles;
+    // one CTA per SM: split the keys of a unit over a cluster until the grid covers the 148 SMs once
     const int max_tiles = (s->pool_capacity + s->block_size + kTcBN - 1) / kTcBN;
     const int target = env_int("HERALD_ATTN_TOTAL_CTAS", 148);
     int splits = units > 0 ? target / (units * a.m_tiles) : 1;
-    if (splits > max_tiles) splits = max_tiles;
-    if (splits > 16) splits = 16;
-    if (splits < 1) splits = 1;
     const int forced = env_int("HERALD_ATTN_SPLITS", 0);
-    if (forced > 0) splits = forced < max_tiles ? forced : (max_tiles > 0 ? max_tiles : 1);
+    if (forced > 0) splits = forced;
+    if (splits > max_tiles) splits = max_tiles;
+    if (splits > kTcMaxSplits) splits = kTcMaxSplits;
+    if (splits < 1) splits = 1;
     a.n_splits = splits;
-    size_t off = 0;
-    a.part_o = off;
-    if (splits > 1) off = align_up(off + (size_t)units * splits * a.m_pad * kHeadDim * sizeof(float), 256);
-    a.part_ml = off;
-    if (splits > 1) off = align_up(off + (size_t)units * splits * a.m_pad * sizeof(float2), 256);
-    a.total = off > 256 ? off : 256;
+    a.total = 256;   // split-KV partials are merged on chip (DSMEM): the workspace is reserved, not used
     return a;
 }
 
@@ -158,20 +157,81 @@ static EncodeTiledFn encode_tiled_fn() {
     return fn;
 }
 
+// Encoding a tensor map costs about a microsecond of host time and the same few maps come back every denoising
+// step, so the last encodings are kept per thread, keyed by (base pointer, extents).
+struct MapKey {
+    const void* ptr;
+    int32_t d[4];
+    bool operator==(const MapKey& o) const { return ptr == o.ptr && d[0] == o.d[0] && d[1] == o.d[1] && d[2] == o.d[2] && d[3] == o.d[3]; }
+};
+struct MapSlot {
+    MapKey key;
+    CUtensorMap map;
+    bool used;
+};
+constexpr int kMapSlots = 64;
+static thread_local MapSlot g_maps[kMapSlots];
+static thread_local int g_map_next = 0;
+
+static const CUtensorMap* cached_map(const MapKey& key) {
+    for (int i = 0; i < kMapSlots; ++i)
+        if (g_maps[i].used && g_maps[i].key == key) return &g_maps[i].map;
+    return nullptr;
+}
+static CUtensorMap* new_map_slot(const MapKey& key) {
+    MapSlot* s = &g_maps[g_map_next];
+    g_map_next = (g_map_next + 1) % kMapSlots;
+    s->key = key;
+    s->used = false;   // set by the caller once the encode succeeded
+    return &s->map;
+}
+static void commit_map_slot(const CUtensorMap* m) {
+    for (int i = 0; i < kMapSlots; ++i)
+        if (&g_maps[i].map == m) g_maps[i].used = true;
+}
+
 // bf16 pool [units][cap][128] as a 3-D tensor (d, row, unit); box = 64 channels x 128 rows, 128-byte swizzle:
 // the box lands in shared memory exactly in the UMMA canonical layout (K-major for K, MN-major for V).
-static int make_pool_map(CUtensorMap* map, const void* pool, int units, int cap) {
+static int make_pool_map(const CUtensorMap** out, const void* pool, int units, int cap) {
+    const MapKey key{pool, {units, cap, 0, 3}};
+    if ((*out = cached_map(key)) != nullptr) return HERALD_OK;
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
+    CUtensorMap* map = new_map_slot(key);
     const cuuint64_t rows = cap > 0 ? cap : 1;
     const cuuint64_t dims[3] = {(cuuint64_t)kHeadDim, rows, (cuuint64_t)units};
-    const cuuint64_t strides[2] = {(cuuint64_t)kRowBytes, (cuuint64_t)cap * kRowBytes > 0 ? (cuuint64_t)cap * kRowBytes : kRowBytes};
+    const cuuint64_t strides[2] = {(cuuint64_t)kRowBytes, rows * kRowBytes};
     const cuuint32_t box[3] = {64u, (cuuint32_t)(rows < (cuuint64_t)kTcBN ? rows : kTcBN), 1u};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
     const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(pool), dims, strides, box, estr,
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+    if (r != CUDA_SUCCESS) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled(pool) failed with CUresult %d", (int)r);
+    commit_map_slot(map);
+    *out = map;
+    return HERALD_OK;
+}
+
+// bf16 q_blk [batch][B][H_q][128] as a 4-D tensor (d, head, block row, sequence); box = 64 channels x G heads x ipt
+// block rows: one box is one half of the Q tile of an (unit, M tile), rows ordered (block row, head), zero-filled past B.
+static int make_q_map(const CUtensorMap** out, const void* q_blk, const herald_shape_t* s, int ipt) {
+    const MapKey key{q_blk, {s->batch, s->block_size, s->n_q_heads, 4 | (ipt << 8) | (s->n_kv_heads << 16)}};
+    if ((*out = cached_map(key)) != nullptr) return HERALD_OK;
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
+    CUtensorMap* map = new_map_slot(key);
+    const int G = s->n_q_heads / s->n_kv_heads;
+    const cuuint64_t dims[4] = {(cuuint64_t)kHeadDim, (cuuint64_t)s->n_q_heads, (cuuint64_t)s->block_size, (cuuint64_t)s->batch};
+    const cuuint64_t strides[3] = {(cuuint64_t)kRowBytes, (cuuint64_t)s->n_q_heads * kRowBytes,
+                                   (cuuint64_t)s->block_size * s->n_q_heads * kRowBytes};
+    const cuuint32_t box[4] = {64u, (cuuint32_t)G, (cuuint32_t)ipt, 1u};
+    const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(q_blk), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled(q_blk) failed with CUresult %d", (int)r);
+    commit_map_slot(map);
+    *out = map;
     return HERALD_OK;
 }
 
@@ -343,39 +403,46 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(attn)");
         attr_set = true;
     }
-    CUtensorMap tm_k, tm_v;
+    const CUtensorMap *tm_k, *tm_v, *tm_q;
     rc = make_pool_map(&tm_k, pool_k, units, shape->pool_capacity);
     if (rc) return rc;
     rc = make_pool_map(&tm_v, pool_v, units, shape->pool_capacity);
+    if (rc) return rc;
+    rc = make_q_map(&tm_q, q_blk, shape, a.ipt);
     if (rc) return rc;
     AttnParams ap{};
     ap.pool_k = static_cast<const __nv_bfloat16*>(pool_k);
     ap.pool_v = static_cast<const __nv_bfloat16*>(pool_v);
     ap.pool_len = pool_len;
-    ap.q_blk = static_cast<const __nv_bfloat16*>(q_blk);
     ap.k_blk = static_cast<const __nv_bfloat16*>(k_blk);
     ap.v_blk = static_cast<const __nv_bfloat16*>(v_blk);
     ap.out = out;
     ap.lse = lse;
-    ap.part_o = reinterpret_cast<float*>(static_cast<uint8_t*>(ws) + a.part_o);
-    ap.part_ml = reinterpret_cast<float2*>(static_cast<uint8_t*>(ws) + a.part_ml);
     ap.n_q_heads = shape->n_q_heads;
     ap.n_kv_heads = shape->n_kv_heads;
     ap.block_size = shape->block_size;
     ap.cap = shape->pool_capacity;
     ap.n_splits = a.n_splits;
-    ap.m_pad = a.m_pad;
+    ap.ipt = a.ipt;
     ap.scale_log2 = shape->sm_scale * 1.4426950408889634f;
-    dim3 grid(a.n_splits, a.m_tiles, units);
-    attn_tc_kernel<<<grid, kTcThreads, kTcSmemBytes, stream>>>(tm_k, tm_v, ap);
-    cudaError_t e = cudaGetLastError();
+#ifdef HERALD_ATTN_TRACE
+    ap.trace = g_attn_trace;
+#endif
+    // the n_splits CTAs of one (unit, M tile) are one thread-block cluster: the split-KV merge runs over DSMEM
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(a.n_splits, a.m_tiles, units);
+    cfg.blockDim = dim3(kTcThreads);
+    cfg.dynamicSmemBytes = kTcSmemBytes;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = a.n_splits;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = a.n_splits > 1 ? 1 : 0;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, attn_tc_kernel, *tm_k, *tm_v, *tm_q, ap);
     if (e != cudaSuccess) return cuda_fail(e, "attention launch");
-    if (a.n_splits > 1) {
-        const int M = shape->block_size * (shape->n_q_heads / shape->n_kv_heads);
-        attn_combine_kernel<<<dim3(M, units), 128, 0, stream>>>(ap);
-        e = cudaGetLastError();
-        if (e != cudaSuccess) return cuda_fail(e, "combine launch");
-    }
     return HERALD_OK;
 }
 
@@ -451,6 +518,13 @@ int herald_pipeline_step(herald_pipeline_t* p) {
     p->active = idle;
     return HERALD_OK;
 }
+
+#ifdef HERALD_ATTN_TRACE
+int herald_debug_set_attn_trace(void* dev_buf) {
+    g_attn_trace = static_cast<unsigned long long*>(dev_buf);
+    return HERALD_OK;
+}
+#endif
 
 int herald_pipeline_set_profile(const herald_profile_t* prof) {
     g_prof = prof;

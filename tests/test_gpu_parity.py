@@ -186,7 +186,7 @@ def test_sparse_attn_matches_oracle(H, cuda, case):
     assert np.abs(lse.cpu().numpy() - lse_ref).max() <= 2e-3
 
 
-@pytest.mark.parametrize("splits", [1, 2, 5])
+@pytest.mark.parametrize("splits", [1, 2, 3, 5, 8])
 def test_sparse_attn_split_kv_is_consistent(H, cuda, splits, monkeypatch):
     monkeypatch.setenv("HERALD_ATTN_SPLITS", str(splits))
     batch, B, Hq, Hkv, cap = 1, 32, 14, 2, 600
