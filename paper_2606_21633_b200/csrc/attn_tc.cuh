@@ -12,20 +12,28 @@
 //   grid    = (KV splits S, M tiles, units); the S CTAs of one (unit, M tile) form a thread-block cluster
 //   M tile  = `ipt` block rows x G heads (row r = block row r/G, head r%G; at most 128 rows), so the Q tile
 //             is one TMA box of q_blk; rows past ipt*G are zeros
-//   warp  8   K producer (+ Q): whole 128-key pool tiles arrive by TMA (cp.async.bulk.tensor, 128B swizzle)
-//             into a 3-stage ring; a stage is released as soon as QK^T has read it
-//   warp  9   V producer, same, released after PV.  The ragged tail of the pool and the in-block rows
-//             are written with zero-filling cp.async, so rows past the end are exact zeros.
-//   warp 10   issues the MMAs (one elected lane, descriptors precomputed so the issue keeps up with the
-//             tensor pipe): S[j&1] = Q K_j^T into a double-buffered TMEM tile, then O += P_{j-1} V_{j-1}
-//             with P read from TMEM; tcgen05.commit -> mbarrier
-//   warps 0-7 softmax: thread (row, column half) reads 64 logits of its row from TMEM (tcgen05.ld),
-//             exchanges the row maximum with its partner warp, exponentiates (ex2), accumulates the row
-//             sum, and writes P back over S_j in TMEM (tcgen05.st).  The running maximum is only raised
-//             when it grows by more than 2^8 ("lazy rescale"): O in TMEM is then rescaled in place.
-//   merge     split-KV partials never leave the chip: every CTA pushes its unnormalised O rows and
-//             (max, sum) into the shared memory of the row's owner CTA of the cluster (DSMEM), the owner
-//             merges, normalises and writes `out` with fully coalesced 512-byte rows.
+//   TMEM    = three S/P tiles of 128 columns + O (128 columns): QK^T runs two tiles ahead of PV, so the softmax
+//             warps never wait for the tensor pipe and the pipe never waits for one softmax
+//   keys    = key tile 0 holds the B in-block rows (one TMA box of k_blk / v_blk), key tile t >= 1 holds pool rows
+//             [128(t-1), 128t) (one TMA box of the pool; softmax is invariant to the key order)
+//   warp 16   K producer (+ Q): tiles arrive by TMA (cp.async.bulk.tensor, 128B swizzle) into a 3-stage ring; a
+//             stage is released as soon as QK^T has read it.  Rows past the valid keys of a tile (stale pool rows,
+//             zero fill) give logits that the softmax masks.
+//   warp 17   V producer, same, released after PV.  Where the valid keys of a tile are not a multiple of the MMA
+//             k-step (16), it zeroes the few V rows up to the next multiple after the box has landed (P is 0 there,
+//             but 0 x NaN would poison O).
+//   warp 18   issues the MMAs (one elected lane, descriptors precomputed so the issue keeps up with the
+//             tensor pipe): S[j%3] = Q K_j^T, then O += P_{j-2} V_{j-2} with P read from TMEM; tcgen05.commit -> mbarrier
+//   warps 0-15 softmax: thread (row, column quarter) reads 32 logits of its row from TMEM (tcgen05.ld),
+//             exchanges the row maximum with the three warps that hold the rest of the row, exponentiates (ex2),
+//             accumulates the row sum, and writes P back over S_j in TMEM (tcgen05.st).  The running maximum
+//             is only raised when it grows by more than 2^kTcRescaleThreshold ("lazy rescale"; P, l and O are
+//             fp32/bf16-ranged, so the threshold only guards overflow): O in TMEM is then rescaled in place.
+//   merge     split-KV partials never leave the chip: tile row r is owned by CTA r / rows_own of the cluster; the
+//             other CTAs stage their unnormalised O rows and (max, sum) and send them to the owner's shared memory
+//             with one bulk DSMEM copy each (cp.async.bulk shared::cta -> shared::cluster, mbarrier-tracked); the
+//             owner merges with its own registers, normalises, stages the rows in shared memory and writes `out`
+//             with fully coalesced 512-byte rows.
 #pragma once
 #include <cuda.h>
 
@@ -36,8 +44,10 @@ namespace herald {
 constexpr int kTcBM = 128;                       // query rows per CTA (UMMA M)
 constexpr int kTcBN = 128;                       // keys per tile (UMMA N of QK^T, K of PV)
 constexpr int kTcStages = 3;                     // depth of the K ring and of the V ring
-constexpr int kTcThreads = 352;                  // 8 softmax warps + K producer + V producer + MMA issuer
-constexpr int kTcKWarp = 8, kTcVWarp = 9, kTcMmaWarp = 10;
+constexpr int kTcSBufs = 3;                      // S/P tiles in TMEM
+constexpr int kTcSoftmaxWarps = 16;              // 4 row quarters (TMEM lane quarters) x 4 column quarters
+constexpr int kTcKWarp = 16, kTcVWarp = 17, kTcMmaWarp = 18;
+constexpr int kTcThreads = 19 * 32;
 constexpr int kTcMaxSplits = 8;                  // portable cluster size
 constexpr int kTcHalfBytes = kTcBN * 128;        // one [128 rows x 64 el] swizzled half tile (16 KB)
 constexpr int kTcTileBytes = 2 * kTcHalfBytes;   // a [128 x 128] bf16 tile = two halves (32 KB)
@@ -47,31 +57,44 @@ constexpr int kTcSmemV = kTcSmemK + kTcStages * kTcTileBytes;            // V ri
 constexpr int kTcSmemMisc = kTcSmemV + kTcStages * kTcTileBytes;         // barriers, TMEM pointer, exchange buffers
 constexpr int kTcMiscBytes = 2304;
 constexpr int kTcSmemBytes = kTcSmemMisc + kTcMiscBytes;                 // 231,680 B of the 232,448 B a CTA may own
-constexpr int kTcTmemCols = 512;                 // S0/P0 [0,128) S1/P1 [128,256) O [256,384)
-constexpr float kTcRescaleThreshold = 8.f;       // log2 units
-// merge buffers (alias the K ring once every CTA of the cluster has left its main loop)
-constexpr int kTcRecvRowFloats = kHeadDim + 4;   // 528-byte rows: 16-byte stores of 8 consecutive rows hit 8 bank groups
-constexpr int kTcRecvO = kTcSmemK;                                                    // float [<= 128 + S rows][132]
-constexpr int kTcRecvML = kTcRecvO + (kTcBM + kTcMaxSplits) * kTcRecvRowFloats * 4;   // float2 [<= 128 + S rows]
-static_assert(kTcRecvML + (kTcBM + kTcMaxSplits) * 8 <= kTcSmemV, "merge buffers must fit in the K ring");
+constexpr int kTcTmemCols = 512;                 // S0/P0 [0,128) S1/P1 [128,256) S2/P2 [256,384) O [384,512)
+constexpr int kTcTmemO = kTcSBufs * 128;
+constexpr float kTcRescaleThreshold = 40.f;      // log2 units
+// merge buffers: received partial rows alias the K ring, the output staging rows alias the V ring (both dead once
+// every CTA of the cluster has left its main loop)
+constexpr int kTcRowFloats = kHeadDim + 4;       // 528-byte rows: 16-byte accesses of 8 consecutive rows hit 8 bank groups
+constexpr int kTcRecvO = kTcSmemK;                                               // float [S-1 sources][rows_own][132]
+constexpr int kTcRecvML = kTcRecvO + kTcBM * kTcRowFloats * 4;                   // float2 [S-1 sources][ml_stride]
+constexpr int kTcPushO = kTcSmemV;                                               // float [S-1 owners][rows_own][132], then
+                                                                                 // float2 [S-1][ml_stride], then the output rows
+static_assert(kTcRecvML + (kTcBM + 2 * kTcMaxSplits) * 8 <= kTcSmemV, "receive buffers must fit in the K ring");
+constexpr int tc_merge_stage_bytes(int S) {      // bytes of the V ring used by the merge for a cluster of S CTAs
+    const int rows_own = (kTcBM + S - 1) / S, ml_stride = (rows_own + 1) & ~1;
+    return (S - 1) * (rows_own * kTcRowFloats * 4 + ml_stride * 8) + rows_own * kTcRowFloats * 4;
+}
+constexpr bool tc_merge_fits() {
+    for (int S = 1; S <= kTcMaxSplits; ++S)
+        if (tc_merge_stage_bytes(S) > kTcStages * kTcTileBytes) return false;
+    return true;
+}
+static_assert(tc_merge_fits(), "push + output staging must fit in the V ring");
 
 // barrier slots (8 bytes each) inside the misc area
 enum { kBarKFull = 0, kBarKEmpty = kBarKFull + kTcStages, kBarVFull = kBarKEmpty + kTcStages, kBarVEmpty = kBarVFull + kTcStages,
-       kBarSFull = kBarVEmpty + kTcStages, kBarPFull = kBarSFull + 2, kBarPvDone, kBarQFull = kBarPvDone + 2, kBarCount };
-constexpr int kTcMiscTmemPtr = 192;              // uint32
-constexpr int kTcMiscMax = 256;                  // float [2 buffers][2 halves][128 rows]
+       kBarSFull = kBarVEmpty + kTcStages, kBarPFull = kBarSFull + kTcSBufs, kBarPvDone = kBarPFull + kTcSBufs,
+       kBarQFull = kBarPvDone + kTcSBufs, kBarVTail, kBarMerge, kBarAck, kBarCount };
+constexpr int kTcMiscTmemPtr = 200;              // uint32
+constexpr int kTcMiscMax = 256;                  // bf16 [2 buffers][4 column quarters][128 rows]; float [4][128] for the row sums
 static_assert(kBarCount * 8 <= kTcMiscTmemPtr, "barriers overlap the TMEM pointer slot");
+static_assert(kTcMiscMax + 2 * 4 * 128 * 2 <= kTcMiscBytes, "exchange buffer overflows the misc area");
 
 struct AttnParams {
-    const __nv_bfloat16* pool_k;
-    const __nv_bfloat16* pool_v;
     const int32_t* pool_len;
-    const __nv_bfloat16* k_blk;
-    const __nv_bfloat16* v_blk;
     float* out;
     float* lse;
     int32_t n_q_heads, n_kv_heads, block_size, cap, n_splits;
     int32_t ipt;        // block rows per M tile (ipt * G <= 128)
+    int32_t pool_box;   // rows of the pool tensor-map box: min(cap, 128)
     float scale_log2;   // sm_scale * log2(e)
 #ifdef HERALD_ATTN_TRACE
     unsigned long long* trace;   // [CTAs][64] clock64 stamps (debug builds only)
@@ -139,6 +162,14 @@ __device__ __forceinline__ void st_cluster_f2(uint32_t addr, float a, float b) {
     asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(a), "f"(b) : "memory");
 }
 
+// local shared memory -> shared memory of another CTA of the cluster; completion counts bytes on the destination's mbarrier
+__device__ __forceinline__ void dsmem_bulk_copy(uint32_t dst_cluster, uint32_t src_cta, uint32_t bytes, uint32_t bar_cluster) {
+    asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst_cluster), "r"(src_cta), "r"(bytes), "r"(bar_cluster) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t bar_cluster) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster) : "memory");
+}
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint32_t bar) {
     asm volatile(
         "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
@@ -242,9 +273,18 @@ __device__ __forceinline__ float fmax3(float a, float b, float c) {
     return r;
 }
 
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* v) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%16], "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15};"
+        ::"r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]),
+          "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]), "r"(taddr) : "memory");
+}
+
 __global__ void __launch_bounds__(kTcThreads, 1)
 attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
-               const __grid_constant__ CUtensorMap tm_q, const AttnParams p) {
+               const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_kb,
+               const __grid_constant__ CUtensorMap tm_vb, const AttnParams p) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const uint32_t sbase = smem_u32(smem_raw);
     uint8_t* sgen = smem_raw;
@@ -258,19 +298,21 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     const int rows_valid = min(p.ipt, B - i0) * G;           // tile rows that are real queries
     const int rows_box = p.ipt * G;                          // tile rows the Q box writes (zeros past the block)
     const int n_pool = max(0, min(p.pool_len[unit], p.cap));
-    const int N = n_pool + B;
-    const int n_tiles = (N + kTcBN - 1) / kTcBN;
-    const int n_full = n_pool / kTcBN;                       // tiles [0, n_full) are whole pool tiles -> TMA
+    const int n_tiles = 1 + (n_pool + kTcBN - 1) / kTcBN;    // key tile 0 = the in-block rows, tile t >= 1 = pool rows [128(t-1), 128t)
     const int per = (n_tiles + S - 1) / S;
     const int t0 = split * per, t1 = min(n_tiles, t0 + per);
-    const int nt = max(t1 - t0, 0);                          // tile j of this CTA is key tile t0 + j (ragged tiles last)
+    const int nt = max(t1 - t0, 0);                          // tile j of this CTA is key tile t0 + j
+    const int rows_own = (kTcBM + S - 1) / S;                // tile rows merged and written by each CTA of the cluster
+    const int ml_stride = (rows_own + 1) & ~1;               // float2 per source, padded to 16 bytes
+    const int g_inv = (65536 + G - 1) / G;                   // (r * g_inv) >> 16 == r / G for r < 128, G <= 8
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) HERALD_STAMP(0);
 
     const uint32_t misc = sbase + kTcSmemMisc;
     auto bar = [&](int i) { return misc + 8u * i; };
     volatile uint32_t* tmem_ptr_gen = reinterpret_cast<volatile uint32_t*>(sgen + kTcSmemMisc + kTcMiscTmemPtr);
-    float* ex_max = reinterpret_cast<float*>(sgen + kTcSmemMisc + kTcMiscMax);
+    __nv_bfloat16* ex_max = reinterpret_cast<__nv_bfloat16*>(sgen + kTcSmemMisc + kTcMiscMax);
+    float* ex_sum = reinterpret_cast<float*>(sgen + kTcSmemMisc + kTcMiscMax);   // after the last tile
 
     // ---- one-time setup: nothing here waits on global memory ------------------------------------------
     if (warp == kTcMmaWarp) {
@@ -284,18 +326,27 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 mbar_init(bar(kBarVFull + s), 1);
                 mbar_init(bar(kBarVEmpty + s), 1);
             }
-            for (int s = 0; s < 2; ++s) mbar_init(bar(kBarSFull + s), 1);
-            mbar_init(bar(kBarPFull), 8);
-            for (int s = 0; s < 2; ++s) mbar_init(bar(kBarPvDone + s), 1);   // PV_j commits to slot j&1 (see the epilogue wait)
+            for (int s = 0; s < kTcSBufs; ++s) {
+                mbar_init(bar(kBarSFull + s), 1);
+                mbar_init(bar(kBarPFull + s), kTcSoftmaxWarps);
+                mbar_init(bar(kBarPvDone + s), 1);   // PV_j commits to slot j % 3
+            }
             mbar_init(bar(kBarQFull), 1);
+            mbar_init(bar(kBarVTail), 1);
+            mbar_init(bar(kBarMerge), 1);
+            mbar_init(bar(kBarAck), S > 1 ? S - 1 : 1);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            // the partial rows the other CTAs of the cluster will send (nothing can arrive before the first cluster barrier)
+            mbar_arrive_expect_tx(bar(kBarMerge), (uint32_t)((S - 1) * (rows_own * kTcRowFloats * 4 + ml_stride * 8)));
             asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_q) : "memory");
             asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_k) : "memory");
             asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_v) : "memory");
+            asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_kb) : "memory");
+            asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_vb) : "memory");
         }
-    } else if (warp < 8) {
+    } else if (warp < kTcSoftmaxWarps) {
         // Q rows the TMA box does not write are zeros (all 16 chunks of a row, so the swizzle does not matter)
-        for (int c = tid; c < (kTcBM - rows_box) * 16; c += 256) {
+        for (int c = tid; c < (kTcBM - rows_box) * 16; c += kTcSoftmaxWarps * 32) {
             const int r = rows_box + (c >> 4), ch = c & 15;
             *reinterpret_cast<uint4*>(sgen + kTcSmemQ + (ch >> 3) * kTcHalfBytes + r * 128 + ((ch & 7) << 4)) = make_uint4(0, 0, 0, 0);
         }
@@ -307,22 +358,30 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     const uint32_t tmem = *tmem_ptr_gen;
     if (tid == 0) HERALD_STAMP(1);
 
-    auto tile_cols = [&](int j) {   // key columns of this CTA's j-th tile that the MMAs touch (multiple of 16)
-        const int valid = min(kTcBN, N - (t0 + j) * kTcBN);
-        return (valid + 15) & ~15;
+    auto tile_valid = [&](int j) {  // valid keys of this CTA's j-th tile (>= 1)
+        const int t = t0 + j;
+        return t == 0 ? B : min(kTcBN, n_pool - (t - 1) * kTcBN);
+    };
+    auto tile_cols = [&](int j) {   // key columns of the tile that the MMAs touch (multiple of 16)
+        return (tile_valid(j) + 15) & ~15;
     };
 
-    float m_used = -INFINITY, l_run = 0.f;   // softmax warps: running max (log2 units) and row sum of this thread's half row
+    // softmax threads: row of the M tile == TMEM lane, column quarter cq of every key tile
+    const int quarter = warp & 3, cq = (warp >> 2) & 3;
+    const int row = quarter * 32 + lane;
+    const uint32_t lane_base = tmem + ((uint32_t)(quarter * 32) << 16);
+    float m_used = -INFINITY, l_run = 0.f;   // running max (log2 units) and the sum of this thread's quarter row
 
     if (nt > 0) {
         if (warp == kTcKWarp || warp == kTcVWarp) {
             // =========================== producers: one warp streams K tiles (and Q), one streams V tiles ===========================
             const bool is_k = warp == kTcKWarp;
             const CUtensorMap* map = is_k ? &tm_k : &tm_v;
-            const __nv_bfloat16* pool = is_k ? p.pool_k : p.pool_v;
-            const __nv_bfloat16* blk = is_k ? p.k_blk : p.v_blk;
+            const CUtensorMap* map_blk = is_k ? &tm_kb : &tm_vb;
             const int bar_full = is_k ? kBarKFull : kBarVFull, bar_empty = is_k ? kBarKEmpty : kBarVEmpty;
             const uint32_t ring = sbase + (is_k ? kTcSmemK : kTcSmemV);
+            uint8_t* ring_gen = sgen + (is_k ? kTcSmemK : kTcSmemV);
+            int n_fixed = 0;                                  // V tiles whose tail rows were zeroed so far (phase of kBarVTail)
             if (is_k) {
                 if (elect_one()) {
                     // Q tile: one box of q_blk [batch][B][H_q][128] = (64 channels, G heads, ipt block rows) per half
@@ -335,32 +394,31 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
             for (int j = 0; j < nt; ++j) {
                 const int stage = j % kTcStages, t = t0 + j;
                 if (j >= kTcStages) mbar_wait(bar(bar_empty + stage), ((j / kTcStages) - 1) & 1);
+                if (!is_k && j == 0) named_bar_sync(9, 64);   // Q and K_0 are requested before any V tile
                 const uint32_t dst = ring + stage * kTcTileBytes, full = bar(bar_full + stage);
-                if (t < n_full) {
-                    if (elect_one()) {
-                        mbar_arrive_expect_tx(full, kTcTileBytes);
-                        tma_load_3d(dst, map, 0, t * kTcBN, unit, full);
-                        tma_load_3d(dst + kTcHalfBytes, map, 64, t * kTcBN, unit, full);
+                const int valid = tile_valid(j), cols = (valid + 15) & ~15;
+                const bool fix = !is_k && cols != valid;      // V rows [valid, cols) must be zeros: land on kBarVTail first
+                const uint32_t land = fix ? bar(kBarVTail) : full;
+                if (elect_one()) {
+                    if (t == 0) {   // in-block rows: box = (64 channels, 1 head, B rows, 1 sequence) per half
+                        mbar_arrive_expect_tx(land, (uint32_t)B * 256u);
+                        tma_load_4d(dst, map_blk, 0, h, 0, b, land);
+                        tma_load_4d(dst + kTcHalfBytes, map_blk, 64, h, 0, b, land);
+                    } else {        // pool rows: box = (64 channels, pool_box rows, 1 unit) per half; rows past cap are zero-filled
+                        mbar_arrive_expect_tx(land, (uint32_t)p.pool_box * 256u);
+                        tma_load_3d(dst, map, 0, (t - 1) * kTcBN, unit, land);
+                        tma_load_3d(dst + kTcHalfBytes, map, 64, (t - 1) * kTcBN, unit, land);
                     }
-                    __syncwarp();
-                } else {
-                    // ragged tile (pool tail and/or in-block rows): zero-filling 16-byte cp.async, rows past N are zeros
-                    const int rows = tile_cols(j);
-                    for (int c = lane; c < rows * 16; c += 32) {
-                        const int r = c >> 4, ch = c & 15;
-                        const int kj = t * kTcBN + r;
-                        const __nv_bfloat16* src = pool;
-                        int bytes = 0;
-                        if (kj < n_pool) {
-                            src = pool + ((int64_t)unit * p.cap + kj) * kHeadDim + ch * 8;
-                            bytes = 16;
-                        } else if (kj < N) {
-                            src = blk + (((int64_t)b * B + (kj - n_pool)) * p.n_kv_heads + h) * kHeadDim + ch * 8;
-                            bytes = 16;
-                        }
-                        cp_async_16_zfill(dst + (ch >> 3) * kTcHalfBytes + r * 128 + (((ch & 7) ^ (r & 7)) << 4), src, bytes);
+                }
+                __syncwarp();
+                if (is_k && j == 0) named_bar_sync(9, 64);
+                if (fix) {
+                    mbar_wait(bar(kBarVTail), n_fixed & 1);
+                    ++n_fixed;
+                    for (int c = lane; c < (cols - valid) * 16; c += 32) {   // all 16 chunks of a row: the swizzle does not matter
+                        const int r = valid + (c >> 4), ch = c & 15;
+                        *reinterpret_cast<uint4*>(ring_gen + stage * kTcTileBytes + (ch >> 3) * kTcHalfBytes + r * 128 + ((ch & 7) << 4)) = make_uint4(0, 0, 0, 0);
                     }
-                    cp_async_wait_all();
                     fence_proxy_async_smem();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(full);
@@ -371,15 +429,35 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
             constexpr uint32_t idesc_pv = umma_idesc(/*A bf16*/ 1, /*B bf16*/ 1, /*A K-major*/ 0, /*B MN-major*/ 1, kTcBM, kHeadDim);
             constexpr uint32_t hi_k = umma_desc_hi(1024);
             const uint32_t q_lo = umma_desc_lo(sbase + kTcSmemQ, 16);
+            auto issue_qk = [&](int j) {   // S_j = Q K_j^T into S buffer j % 3 (it held P_{j-3}: PV_{j-3} was issued before, the pipe runs in order)
+                const int stage = j % kTcStages, sb = j % kTcSBufs;
+                mbar_wait(bar(kBarKFull + stage), (j / kTcStages) & 1);
+                tc_fence_after();
+                if (lane == 0) HERALD_STAMP(8 + 4 * j);
+                if (elect_one()) {
+                    const uint32_t k_lo = umma_desc_lo(sbase + kTcSmemK + stage * kTcTileBytes, 16);
+                    const uint32_t idesc_s = umma_idesc(1, 1, 0, 0, kTcBM, tile_cols(j));
+                    const uint32_t s_base = tmem + sb * 128;
+#pragma unroll
+                    for (int ks = 0; ks < 8; ++ks) {
+                        const uint32_t off = ((ks >> 2) * kTcHalfBytes + (ks & 3) * 32) >> 4;
+                        if (ks == 0) umma_ss<false>(s_base, q_lo + off, hi_k, k_lo + off, hi_k, idesc_s);
+                        else umma_ss<true>(s_base, q_lo + off, hi_k, k_lo + off, hi_k, idesc_s);
+                    }
+                    umma_commit(bar(kBarSFull + sb));
+                    umma_commit(bar(kBarKEmpty + stage));
+                }
+                __syncwarp();
+            };
             auto issue_pv = [&](int j) {   // O (+)= (P_hi + P_lo)_j V_j, P read from TMEM (it overlays S_j)
-                const int stage = j % kTcStages, sb = j & 1;
+                const int stage = j % kTcStages, sb = j % kTcSBufs;
                 mbar_wait(bar(kBarVFull + stage), (j / kTcStages) & 1);
-                mbar_wait(bar(kBarPFull), j & 1);
+                mbar_wait(bar(kBarPFull + sb), (j / kTcSBufs) & 1);
                 tc_fence_after();
                 if (lane == 0) HERALD_STAMP(8 + 4 * j + 3);
                 if (elect_one()) {
                     const uint32_t v_lo = umma_desc_lo(sbase + kTcSmemV + stage * kTcTileBytes, kTcHalfBytes);
-                    const uint32_t p_base = tmem + sb * 128, o_base = tmem + 256;
+                    const uint32_t p_base = tmem + sb * 128, o_base = tmem + kTcTmemO;
                     const int ksteps = tile_cols(j) >> 4;
                     if (ksteps == 8) {
 #pragma unroll
@@ -399,57 +477,40 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 __syncwarp();
             };
             mbar_wait(bar(kBarQFull), 0);
+            issue_qk(0);
+            if (nt > 1) issue_qk(1);
             for (int j = 0; j < nt; ++j) {
-                const int stage = j % kTcStages, sb = j & 1;
-                mbar_wait(bar(kBarKFull + stage), (j / kTcStages) & 1);
-                tc_fence_after();
-                if (lane == 0) HERALD_STAMP(8 + 4 * j);
-                if (elect_one()) {
-                    // S_j overwrites the TMEM columns of P_{j-2}: PV_{j-2} was issued earlier and the tensor pipe runs in order
-                    const uint32_t k_lo = umma_desc_lo(sbase + kTcSmemK + stage * kTcTileBytes, 16);
-                    const uint32_t idesc_s = umma_idesc(1, 1, 0, 0, kTcBM, tile_cols(j));
-                    const uint32_t s_base = tmem + sb * 128;
-#pragma unroll
-                    for (int ks = 0; ks < 8; ++ks) {
-                        const uint32_t off = ((ks >> 2) * kTcHalfBytes + (ks & 3) * 32) >> 4;
-                        if (ks == 0) umma_ss<false>(s_base, q_lo + off, hi_k, k_lo + off, hi_k, idesc_s);
-                        else umma_ss<true>(s_base, q_lo + off, hi_k, k_lo + off, hi_k, idesc_s);
-                    }
-                    umma_commit(bar(kBarSFull + sb));
-                    umma_commit(bar(kBarKEmpty + stage));
-                }
-                __syncwarp();
-                if (j > 0) issue_pv(j - 1);
+                if (j + 2 < nt) issue_qk(j + 2);
+                issue_pv(j);
             }
-            issue_pv(nt - 1);
         } else {
             // =========================== softmax warps ===========================
-            const int quarter = warp & 3, hf = warp >> 2;
-            const int row = quarter * 32 + lane;                 // row of the M tile == TMEM lane
-            const uint32_t lane_base = tmem + ((uint32_t)(quarter * 32) << 16);
             for (int j = 0; j < nt; ++j) {
-                const int sb = j & 1;
-                // S_j complete; the commit also covers PV_{j-2}, so the P columns overlaying this S buffer are free
-                mbar_wait(bar(kBarSFull + sb), (j >> 1) & 1);
+                const int sb = j % kTcSBufs, eb = j & 1;
+                mbar_wait(bar(kBarSFull + sb), (j / kTcSBufs) & 1);
                 tc_fence_after();
                 if (tid == 0) HERALD_STAMP(8 + 4 * j + 1);
-                float s[64];
-                tmem_ld32_async(lane_base + sb * 128 + hf * 64, s);
-                tmem_ld32_async(lane_base + sb * 128 + hf * 64 + 32, s + 32);
+                float s[32];
+                tmem_ld32_async(lane_base + sb * 128 + cq * 32, s);
                 tmem_wait_ld();
-                const int valid = N - (t0 + j) * kTcBN;           // >= 1
+                const int valid = tile_valid(j);
                 if (valid < kTcBN) {
 #pragma unroll
-                    for (int i = 0; i < 64; ++i)
-                        if (hf * 64 + i >= valid) s[i] = -INFINITY;
+                    for (int i = 0; i < 32; ++i)
+                        if (cq * 32 + i >= valid) s[i] = -INFINITY;
                 }
                 float mx = fmax3(s[0], s[1], s[2]);
 #pragma unroll
-                for (int i = 3; i + 1 < 64; i += 2) mx = fmax3(mx, s[i], s[i + 1]);
-                mx = fmaxf(mx, s[63]);
-                ex_max[(sb * 2 + hf) * 128 + row] = mx;
-                named_bar_sync(1 + quarter, 64);                  // both column halves of these 32 rows have read S_j
-                const float mrow = fmaxf(mx, ex_max[(sb * 2 + (hf ^ 1)) * 128 + row]) * p.scale_log2;
+                for (int i = 3; i + 1 < 32; i += 2) mx = fmax3(mx, s[i], s[i + 1]);
+                mx = fmaxf(mx, s[31]);
+                // the row maximum only has to be common to the four column quarters and not below the true maximum:
+                // it is exchanged rounded up to bf16
+                ex_max[(eb * 4 + cq) * 128 + row] = __float2bfloat16_ru(mx);
+                named_bar_sync(1 + quarter, 128);                 // the four warps that hold these 32 rows
+                float mrow = __bfloat162float(ex_max[(eb * 4 + 0) * 128 + row]);
+#pragma unroll
+                for (int c = 1; c < 4; ++c) mrow = fmaxf(mrow, __bfloat162float(ex_max[(eb * 4 + c) * 128 + row]));
+                mrow *= p.scale_log2;
                 float alpha = 1.f;
                 bool need = false;
                 if (j == 0) {
@@ -460,117 +521,146 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                     m_used = mrow;
                 }
                 const bool any = __any_sync(0xffffffffu, need);
+                // P = P_hi + P_lo (bf16 pair: the PV product keeps the weights to ~2^-17 relative).  The exponentials (MUFU,
+                // 16 per clock and SM: the scarce unit) and the splitting arithmetic of earlier pairs share one unrolled loop
+                // so that the scheduler interleaves them.
                 float sum0 = 0.f, sum1 = 0.f;
+                uint32_t hi[16], lo[16];
 #pragma unroll
-                for (int i = 0; i < 64; i += 2) {
-                    s[i] = fast_exp2(fmaf(s[i], p.scale_log2, -m_used));
-                    s[i + 1] = fast_exp2(fmaf(s[i + 1], p.scale_log2, -m_used));
-                    sum0 += s[i];
-                    sum1 += s[i + 1];
+                for (int i = 0; i < 16; ++i) {
+                    const float e0 = fast_exp2(fmaf(s[2 * i], p.scale_log2, -m_used));
+                    const float e1 = fast_exp2(fmaf(s[2 * i + 1], p.scale_log2, -m_used));
+                    sum0 += e0;
+                    sum1 += e1;
+                    split_bf16(e0, e1, hi[i], lo[i]);
                 }
                 l_run = l_run * alpha + (sum0 + sum1);
-                if (any) {   // rare: the running maximum of some row grew by more than 2^8 -> rescale O in place
-                    mbar_wait(bar(kBarPvDone + ((j - 1) & 1)), ((j - 1) >> 1) & 1);   // PV_{j-1} finished; PV_j waits for our arrive
+                if (any) {   // rare: the running maximum of some row grew past the threshold -> rescale O in place
+                    mbar_wait(bar(kBarPvDone + ((j - 1) % kTcSBufs)), ((j - 1) / kTcSBufs) & 1);   // PV_{j-1} finished; PV_j waits for our arrive
                     tc_fence_after();
+                    float o[32];
+                    tmem_ld32_async(lane_base + kTcTmemO + cq * 32, o);
+                    tmem_wait_ld();
 #pragma unroll
-                    for (int q = 0; q < 2; ++q) {
-                        float o[32];
-                        tmem_ld32_async(lane_base + 256 + hf * 64 + q * 32, o);
-                        tmem_wait_ld();
-#pragma unroll
-                        for (int i = 0; i < 32; ++i) o[i] *= alpha;
-                        tmem_st32(lane_base + 256 + hf * 64 + q * 32, reinterpret_cast<const uint32_t*>(o));
-                    }
+                    for (int i = 0; i < 32; ++i) o[i] *= alpha;
+                    tmem_st32(lane_base + kTcTmemO + cq * 32, reinterpret_cast<const uint32_t*>(o));
                 }
-                // P = P_hi + P_lo (bf16 pair: the PV product keeps the weights to ~2^-17 relative).  Both go to TMEM as
-                // the A operand of the PV MMA: row = lane, two keys per 32-bit column; P_hi in columns [0,64) of the
-                // S buffer, P_lo in [64,128), this thread's half row at [hf*32, hf*32+32) of each.
-                {
-                    uint32_t hi[32], lo[32];
-#pragma unroll
-                    for (int i = 0; i < 32; ++i) split_bf16(s[2 * i], s[2 * i + 1], hi[i], lo[i]);
-                    tmem_st32(lane_base + sb * 128 + hf * 32, hi);
-                    tmem_st32(lane_base + sb * 128 + 64 + hf * 32, lo);
-                }
+                // Both halves go to TMEM as the A operand of the PV MMA: row = lane, two keys per 32-bit column; P_hi in
+                // columns [0,64) of the S buffer, P_lo in [64,128), this thread's quarter row at [cq*16, cq*16+16) of each.
+                tmem_st16(lane_base + sb * 128 + cq * 16, hi);
+                tmem_st16(lane_base + sb * 128 + 64 + cq * 16, lo);
                 tmem_wait_st();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar(kBarPFull));
+                if (lane == 0) mbar_arrive(bar(kBarPFull + sb));
                 if (tid == 0) HERALD_STAMP(8 + 4 * j + 2);
             }
-            // A parity wait is only sound when the waiter is at most one phase behind.  The softmax warps do not wait for
-            // every PV, but S_j's commit covers PV_{j-2}, so with one barrier per tile parity the lag is at most one phase.
-            mbar_wait(bar(kBarPvDone + ((nt - 1) & 1)), ((nt - 1) >> 1) & 1);
+            // A parity wait is only sound when the waiter is at most one phase behind: slot (nt-1) % 3 completes next for
+            // PV_{nt+2}, which does not exist.
+            mbar_wait(bar(kBarPvDone + ((nt - 1) % kTcSBufs)), ((nt - 1) / kTcSBufs) & 1);
             tc_fence_after();
             if (tid == 0) HERALD_STAMP(2);
         }
     }
 
     // ---- merge of the split-KV partials inside the cluster, normalisation, output -----------------------
-    // Owner of tile row r is CTA r / rows_own of the cluster.  Every CTA has left its main loop after the first
-    // cluster barrier (the softmax warps arrive only once their last PV has completed, i.e. after every MMA and
-    // every TMA write of the CTA), so the K ring can be reused as the receive buffer.
-    const int rows_own = (kTcBM + S - 1) / S;
-    __syncwarp();
-    if (S > 1) cluster_sync_all(); else __syncthreads();
-    if (warp < 8) {
-        const int quarter = warp & 3, hf = warp >> 2;
-        const int row = quarter * 32 + lane;
-        const uint32_t lane_base = tmem + ((uint32_t)(quarter * 32) << 16);
-        const int owner = row / rows_own, row_l = row - owner * rows_own;
-        const int slot = split * rows_own + row_l;            // [source CTA][row within the owner's slice]
-        uint32_t dst_o = sbase + kTcRecvO + (uint32_t)(slot * kTcRecvRowFloats + hf * 64) * 4u;
-        uint32_t dst_ml = sbase + kTcRecvML + (uint32_t)slot * 8u;
-        if (S > 1) {
-            dst_o = map_to_cta(dst_o, owner);
-            dst_ml = map_to_cta(dst_ml, owner);
-        }
+    // The V ring of this CTA is dead once its softmax warps have seen the last PV complete (every MMA and every TMA
+    // write of the CTA is then done): it stages what this CTA sends and the rows it writes out.  The K ring receives
+    // the other CTAs' partial rows, so nothing is sent before the cluster barrier that every CTA passes after its main loop.
+    const int owner = row / rows_own, row_l = row - owner * rows_own;
+    const int push_ml_off = kTcPushO + (S - 1) * rows_own * kTcRowFloats * 4;
+    const int stage_off = push_ml_off + (S - 1) * ml_stride * 8;
+    float o[32];
+    float l_tot = 0.f;
+    if (warp < kTcSoftmaxWarps) {
         if (nt > 0) {
-            ex_max[hf * 128 + row] = l_run;
-            named_bar_sync(1 + quarter, 64);
-            const float l_tot = l_run + ex_max[(hf ^ 1) * 128 + row];
+            ex_sum[cq * 128 + row] = l_run;
+            tmem_ld32_async(lane_base + kTcTmemO + cq * 32, o);
+            tmem_wait_ld();
+            named_bar_sync(1 + quarter, 128);
+            l_tot = (ex_sum[row] + ex_sum[128 + row]) + (ex_sum[256 + row] + ex_sum[384 + row]);
+        } else {
 #pragma unroll
-            for (int q = 0; q < 2; ++q) {
-                float o[32];
-                tmem_ld32_async(lane_base + 256 + hf * 64 + q * 32, o);
-                tmem_wait_ld();
-#pragma unroll
-                for (int i = 0; i < 32; i += 4) st_cluster_f4(dst_o + (q * 32 + i) * 4, o[i], o[i + 1], o[i + 2], o[i + 3]);
-            }
-            if (hf == 0) st_cluster_f2(dst_ml, m_used, l_tot);
-        } else if (hf == 0) {
-            st_cluster_f2(dst_ml, -INFINITY, 0.f);            // empty split: the owner skips this source
+            for (int i = 0; i < 32; ++i) o[i] = 0.f;
         }
+        if (owner != split) {
+            // stage this quarter row (unnormalised) and (m, l) for its owner; slots skip the sender / the owner itself
+            const int d = owner < split ? owner : owner - 1;
+            float4* dst = reinterpret_cast<float4*>(sgen + kTcPushO + ((d * rows_own + row_l) * kTcRowFloats + cq * 32) * 4);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) dst[i] = make_float4(o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
+            if (cq == 0)
+                *reinterpret_cast<float2*>(sgen + push_ml_off + (d * ml_stride + row_l) * 8) = make_float2(nt > 0 ? m_used : -INFINITY, l_tot);
+        }
+        fence_proxy_async_smem();
     }
     tc_fence_before();
     __syncwarp();
-    if (S > 1) cluster_sync_all(); else __syncthreads();
-    if (tid == 0) HERALD_STAMP(3);
-    {
-        const float* recv_o = reinterpret_cast<const float*>(sgen + kTcRecvO);
-        const float2* recv_ml = reinterpret_cast<const float2*>(sgen + kTcRecvML);
-        const int r_begin = split * rows_own, r_end = min(min(kTcBM, r_begin + rows_own), rows_valid);
-        for (int idx = tid; idx < (r_end - r_begin) * 32; idx += kTcThreads) {
-            const int row_l = idx >> 5, c4 = idx & 31;
-            float mstar = -INFINITY;
-            for (int s = 0; s < S; ++s) mstar = fmaxf(mstar, recv_ml[s * rows_own + row_l].x);
-            float den = 0.f;
-            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-            for (int s = 0; s < S; ++s) {
-                const float2 ml = recv_ml[s * rows_own + row_l];
-                if (ml.x == -INFINITY) continue;
+    if (S > 1) cluster_sync_all(); else __syncthreads();   // staging complete here, main loops complete everywhere
+    if (tid == 0) HERALD_STAMP(5);
+    if (tid < (S - 1) * 8) {
+        // bulk copies to each owner: this CTA's rows of that owner's slice in 8 chunks (8 threads), then their (m, l)
+        const int d = tid >> 3, chunk = tid & 7, dst_cta = d < split ? d : d + 1;
+        const int src_slot = split < dst_cta ? split : split - 1;
+        const uint32_t bar_remote = map_to_cta(bar(kBarMerge), dst_cta);
+        const int rows_chunk = (rows_own + 7) >> 3, r0 = chunk * rows_chunk, nr = min(rows_chunk, rows_own - r0);
+        if (nr > 0)
+            dsmem_bulk_copy(map_to_cta(sbase + kTcRecvO + (src_slot * rows_own + r0) * kTcRowFloats * 4, dst_cta),
+                            sbase + kTcPushO + (d * rows_own + r0) * kTcRowFloats * 4, nr * kTcRowFloats * 4, bar_remote);
+        if (chunk == 0)
+            dsmem_bulk_copy(map_to_cta(sbase + kTcRecvML + src_slot * ml_stride * 8, dst_cta),
+                            sbase + push_ml_off + d * ml_stride * 8, ml_stride * 8, bar_remote);
+    }
+    if (warp < kTcSoftmaxWarps && owner == split) {
+        if (S > 1) mbar_wait(bar(kBarMerge), 0);
+        if (tid == 0) HERALD_STAMP(3);
+        // every partial row addressed to this CTA has landed: release the senders (they may not exit before)
+        if (S > 1 && cq == 0 && row_l < S - 1) mbar_arrive_remote(map_to_cta(bar(kBarAck), row_l < split ? row_l : row_l + 1));
+        if (row < rows_valid) {
+            const float* recv_o = reinterpret_cast<const float*>(sgen + kTcRecvO);
+            const float2* recv_ml = reinterpret_cast<const float2*>(sgen + kTcRecvML);
+            float mstar = nt > 0 ? m_used : -INFINITY;
+            for (int s = 0; s < S - 1; ++s) mstar = fmaxf(mstar, recv_ml[s * ml_stride + row_l].x);
+            const float w_self = nt > 0 ? fast_exp2(m_used - mstar) : 0.f;
+            float den = w_self * l_tot;
+#pragma unroll
+            for (int i = 0; i < 32; ++i) o[i] *= w_self;
+            for (int s = 0; s < S - 1; ++s) {
+                const float2 ml = recv_ml[s * ml_stride + row_l];
+                if (ml.x == -INFINITY) continue;                  // empty split: its rows carry nothing
                 const float w = fast_exp2(ml.x - mstar);
-                const float4 o = *reinterpret_cast<const float4*>(recv_o + (s * rows_own + row_l) * kTcRecvRowFloats + c4 * 4);
                 den += w * ml.y;
-                acc.x += w * o.x; acc.y += w * o.y; acc.z += w * o.z; acc.w += w * o.w;
+                const float4* src = reinterpret_cast<const float4*>(recv_o + (s * rows_own + row_l) * kTcRowFloats + cq * 32);
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const float4 v = src[i];
+                    o[4 * i] += w * v.x; o[4 * i + 1] += w * v.y; o[4 * i + 2] += w * v.z; o[4 * i + 3] += w * v.w;
+                }
             }
             const float inv = 1.f / den;
-            const int r = r_begin + row_l;
-            const int64_t orow = ((int64_t)b * B + i0 + r / G) * p.n_q_heads + h * G + r % G;
-            *reinterpret_cast<float4*>(p.out + orow * kHeadDim + c4 * 4) = make_float4(acc.x * inv, acc.y * inv, acc.z * inv, acc.w * inv);
-            if (p.lse && c4 == 0) p.lse[orow] = (mstar + log2f(den)) * 0.6931471805599453f;
+            float4* dst = reinterpret_cast<float4*>(sgen + stage_off + (row_l * kTcRowFloats + cq * 32) * 4);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) dst[i] = make_float4(o[4 * i] * inv, o[4 * i + 1] * inv, o[4 * i + 2] * inv, o[4 * i + 3] * inv);
+            if (p.lse && cq == 0) {
+                const int bi = (row * g_inv) >> 16;           // row / G
+                const int64_t orow = ((int64_t)b * B + i0 + bi) * p.n_q_heads + h * G + (row - bi * G);
+                p.lse[orow] = (mstar + log2f(den)) * 0.6931471805599453f;
+            }
         }
     }
+    __syncthreads();
+    {
+        // coalesced copy of this CTA's finished rows: one warp writes one 512-byte row per instruction
+        const float* stage = reinterpret_cast<const float*>(sgen + stage_off);
+        const int r_begin = split * rows_own, r_end = min(min(kTcBM, r_begin + rows_own), rows_valid);
+        for (int rl = warp; rl < r_end - r_begin; rl += kTcThreads / 32) {
+            const int r = r_begin + rl, bi = (r * g_inv) >> 16;   // r / G
+            const int64_t orow = ((int64_t)b * B + i0 + bi) * p.n_q_heads + h * G + (r - bi * G);
+            *reinterpret_cast<float4*>(p.out + orow * kHeadDim + lane * 4) = *reinterpret_cast<const float4*>(stage + rl * kTcRowFloats + lane * 4);
+        }
+    }
+    // a CTA may not exit while a bulk copy out of its shared memory is in flight: every owner it sent rows to has acknowledged
+    if (S > 1) mbar_wait(bar(kBarAck), 0);
     if (tid == 0) HERALD_STAMP(4);
 
     // ---- teardown ----

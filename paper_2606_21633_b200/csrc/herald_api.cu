@@ -125,7 +125,7 @@ static AttnGeom attn_geom(const herald_shape_t* s) {
     a.m_tiles = (s->block_size + rows_cap - 1) / rows_cap;
     a.ipt = (s->block_size + a.m_tiles - 1) / a.m_tiles;
     // one CTA per SM: split the keys of a unit over a cluster until the grid covers the 148 SMs once
-    const int max_tiles = (s->pool_capacity + s->block_size + kTcBN - 1) / kTcBN;
+    const int max_tiles = 1 + (s->pool_capacity + kTcBN - 1) / kTcBN;   // the in-block rows are a key tile of their own
     const int target = env_int("HERALD_ATTN_TOTAL_CTAS", 148);
     int splits = units > 0 ? target / (units * a.m_tiles) : 1;
     const int forced = env_int("HERALD_ATTN_SPLITS", 0);
@@ -214,6 +214,28 @@ static int make_pool_map(const CUtensorMap** out, const void* pool, int units, i
 
 // bf16 q_blk [batch][B][H_q][128] as a 4-D tensor (d, head, block row, sequence); box = 64 channels x G heads x ipt
 // block rows: one box is one half of the Q tile of an (unit, M tile), rows ordered (block row, head), zero-filled past B.
+// bf16 k_blk / v_blk [batch][B][H_kv][128] as a 4-D tensor (d, head, block row, sequence); box = 64 channels x 1 head x
+// B block rows: one half of the in-block key tile of a unit.
+static int make_blk_map(const CUtensorMap** out, const void* blk, const herald_shape_t* s) {
+    const MapKey key{blk, {s->batch, s->block_size, s->n_kv_heads, 5}};
+    if ((*out = cached_map(key)) != nullptr) return HERALD_OK;
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
+    CUtensorMap* map = new_map_slot(key);
+    const cuuint64_t dims[4] = {(cuuint64_t)kHeadDim, (cuuint64_t)s->n_kv_heads, (cuuint64_t)s->block_size, (cuuint64_t)s->batch};
+    const cuuint64_t strides[3] = {(cuuint64_t)kRowBytes, (cuuint64_t)s->n_kv_heads * kRowBytes,
+                                   (cuuint64_t)s->block_size * s->n_kv_heads * kRowBytes};
+    const cuuint32_t box[4] = {64u, 1u, (cuuint32_t)s->block_size, 1u};
+    const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(blk), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled(k_blk/v_blk) failed with CUresult %d", (int)r);
+    commit_map_slot(map);
+    *out = map;
+    return HERALD_OK;
+}
+
 static int make_q_map(const CUtensorMap** out, const void* q_blk, const herald_shape_t* s, int ipt) {
     const MapKey key{q_blk, {s->batch, s->block_size, s->n_q_heads, 4 | (ipt << 8) | (s->n_kv_heads << 16)}};
     if ((*out = cached_map(key)) != nullptr) return HERALD_OK;
@@ -403,19 +425,19 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(attn)");
         attr_set = true;
     }
-    const CUtensorMap *tm_k, *tm_v, *tm_q;
+    const CUtensorMap *tm_k, *tm_v, *tm_q, *tm_kb, *tm_vb;
     rc = make_pool_map(&tm_k, pool_k, units, shape->pool_capacity);
     if (rc) return rc;
     rc = make_pool_map(&tm_v, pool_v, units, shape->pool_capacity);
     if (rc) return rc;
     rc = make_q_map(&tm_q, q_blk, shape, a.ipt);
     if (rc) return rc;
+    rc = make_blk_map(&tm_kb, k_blk, shape);
+    if (rc) return rc;
+    rc = make_blk_map(&tm_vb, v_blk, shape);
+    if (rc) return rc;
     AttnParams ap{};
-    ap.pool_k = static_cast<const __nv_bfloat16*>(pool_k);
-    ap.pool_v = static_cast<const __nv_bfloat16*>(pool_v);
     ap.pool_len = pool_len;
-    ap.k_blk = static_cast<const __nv_bfloat16*>(k_blk);
-    ap.v_blk = static_cast<const __nv_bfloat16*>(v_blk);
     ap.out = out;
     ap.lse = lse;
     ap.n_q_heads = shape->n_q_heads;
@@ -424,6 +446,7 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
     ap.cap = shape->pool_capacity;
     ap.n_splits = a.n_splits;
     ap.ipt = a.ipt;
+    ap.pool_box = shape->pool_capacity < kTcBN ? (shape->pool_capacity > 0 ? shape->pool_capacity : 1) : kTcBN;
     ap.scale_log2 = shape->sm_scale * 1.4426950408889634f;
 #ifdef HERALD_ATTN_TRACE
     ap.trace = g_attn_trace;
@@ -441,7 +464,7 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = a.n_splits > 1 ? 1 : 0;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, attn_tc_kernel, *tm_k, *tm_v, *tm_q, ap);
+    cudaError_t e = cudaLaunchKernelEx(&cfg, attn_tc_kernel, *tm_k, *tm_v, *tm_q, *tm_kb, *tm_vb, ap);
     if (e != cudaSuccess) return cuda_fail(e, "attention launch");
     return HERALD_OK;
 }
