@@ -78,15 +78,26 @@ struct SelectWs {
     int scan_ctas;
 };
 
+static int sm_count() {
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
+            n = 148;   // B200
+    }
+    return n;
+}
+
+// SMs the retrieval-stream kernels may occupy (0 = all); set by herald_pipeline_step around its select/gather calls
+static thread_local int g_retrieval_sms = 0;
+
+// Grid of the scan = number of SMs it may occupy (one 1024-thread CTA per SM).
 static int scan_ctas_for(const herald_shape_t* s) {
-    const int units = s->batch * s->n_kv_heads;
-    const int max_pages = (s->max_seq_len + kPageSize - 1) / kPageSize;
-    int target = env_int("HERALD_SCAN_TOTAL_CTAS", 148 * 4);
-    int per_unit = units > 0 ? (target + units - 1) / units : 1;
-    const int cap = (max_pages + kScanWarps - 1) / kScanWarps;
-    if (per_unit > cap) per_unit = cap;
-    if (per_unit < 1) per_unit = 1;
-    return per_unit;
+    (void)s;
+    int n = env_int("HERALD_SCAN_CTAS", 0);
+    if (n <= 0) n = g_retrieval_sms > 0 ? g_retrieval_sms : sm_count();
+    if (n > kScanMaxCtas) n = kScanMaxCtas;
+    return n;
 }
 
 static SelectWs select_ws_layout(const herald_shape_t* s) {
@@ -104,7 +115,7 @@ static SelectWs select_ws_layout(const herald_shape_t* s) {
     if (s->agg_mode == HERALD_AGG_SOFTMAX_SUM) {
         off = align_up(off + units * G * (size_t)s->max_seq_len * sizeof(float), 256);
         w.stats = off;
-        off = align_up(off + units * G * (size_t)w.scan_ctas * sizeof(float2), 256);
+        off = align_up(off + units * G * (size_t)kScanMaxCtas * sizeof(float2), 256);   // any grid size fits
     }
     w.total = off;
     return w;
@@ -281,6 +292,12 @@ size_t herald_attn_workspace_bytes(const herald_shape_t* shape) {
     return attn_geom(shape).total;
 }
 
+int32_t herald_attn_grid_ctas(const herald_shape_t* shape) {
+    if (check_shape(shape) != HERALD_OK) return 0;
+    const AttnGeom a = attn_geom(shape);
+    return a.n_splits * a.m_tiles * shape->batch * shape->n_kv_heads;
+}
+
 int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep,
                   const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, float* scores_out, void* ws,
                   size_t ws_bytes, herald_stream_t stream_) {
@@ -319,12 +336,14 @@ int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, cons
         sp.raw = reinterpret_cast<float*>(wsb + w.raw);
         sp.stats_part = reinterpret_cast<float2*>(wsb + w.stats);
         sp.hist1 = hist1;
+        sp.batch = shape->batch;
         sp.n_q_heads = shape->n_q_heads;
         sp.n_kv_heads = shape->n_kv_heads;
         sp.max_seq_len = shape->max_seq_len;
         sp.max_pages = shape->max_pages_per_seq;
         sp.sm_scale = shape->sm_scale;
-        dim3 grid(w.scan_ctas, shape->n_kv_heads, shape->batch);
+        const int scan_ctas = scan_ctas_for(shape);
+        dim3 grid(scan_ctas);
         if (shape->agg_mode == HERALD_AGG_MAX_LOGIT) {
             scan_kernel<0><<<grid, kScanThreads, 0, stream>>>(sp);
         } else {
@@ -332,7 +351,8 @@ int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, cons
             AggParams ap{};
             ap.raw = sp.raw;
             ap.stats_part = sp.stats_part;
-            ap.n_parts = w.scan_ctas;
+            ap.n_parts = scan_ctas;
+            ap.batch = shape->batch;
             ap.seq_lens = cache->seq_lens;
             ap.scores = scores;
             ap.hist1 = hist1;
@@ -477,6 +497,7 @@ static int check_pipeline(const herald_pipeline_t* p) {
     if (p->n_steps < 0 || p->start_after_step < 0 || p->start_after_step > p->n_steps)
         return fail(HERALD_ERR_INVALID_ARG, "pipeline: bad n_steps / start_after_step");
     if (p->active != 0 && p->active != 1) return fail(HERALD_ERR_INVALID_ARG, "pipeline: active must be 0 or 1");
+    if (p->retrieval_sms < 0) return fail(HERALD_ERR_INVALID_ARG, "pipeline: retrieval_sms must be >= 0");
     if (!p->sel_idx || !p->ws_select || !p->ws_attn || !p->ev_fork || !p->ev_join)
         return fail(HERALD_ERR_INVALID_ARG, "pipeline: NULL scratch / workspace / event");
     if (p->main_stream == p->retrieval_stream)
@@ -504,9 +525,11 @@ int herald_pipeline_step(herald_pipeline_t* p) {
         for (int l = 0; l < p->n_layers; ++l) {
             herald_layer_t* ly = &p->layers[l];
             g_prof_armed = (l == p->n_layers - 1);
+            g_retrieval_sms = p->retrieval_sms;
             int r = herald_select(sh, &ly->cache, ly->q_rep, ly->k_per_seq, p->sel_idx, ly->pool_len[idle], nullptr,
                                   p->ws_select, p->ws_select_bytes, s_ret);
             g_prof_armed = false;
+            g_retrieval_sms = 0;
             if (r) return r;
             r = herald_gather(sh, &ly->cache, p->sel_idx, ly->pool_len[idle], ly->pool_k[idle], ly->pool_v[idle], s_ret);
             if (r) return r;

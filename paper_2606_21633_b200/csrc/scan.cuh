@@ -15,8 +15,9 @@
 
 namespace herald {
 
-constexpr int kScanThreads = 256;
+constexpr int kScanThreads = 1024;             // one CTA per SM: 32 warps x 8 x 16-byte loads in flight per lane
 constexpr int kScanWarps = kScanThreads / 32;
+constexpr int kScanMaxCtas = 512;              // bound on the grid (sizes the mode-1 partial statistics)
 
 struct ScanParams {
     const __nv_bfloat16* k_pages;
@@ -28,132 +29,164 @@ struct ScanParams {
     float* raw;           // [batch][H_kv][G][max_seq_len]           (mode 1)
     float2* stats_part;   // [batch*H_kv][G][gridDim.x] (m, l)       (mode 1)
     uint32_t* hist1;      // [batch*H_kv][kBins1]                    (mode 0)
-    int32_t n_q_heads, n_kv_heads, max_seq_len, max_pages;
+    int32_t batch, n_q_heads, n_kv_heads, max_seq_len, max_pages;
     float sm_scale;
 };
 
+// The grid is flat and persistent: the (unit, page) tiles of the whole batch, in unit-major order, are cut into
+// gridDim.x equal contiguous ranges, one per CTA (units are ragged: sequence b has ceil(L_b / 16) pages per KV head).
+// A CTA therefore touches one or two units and keeps one shared-memory histogram at a time.  The grid size is the
+// number of SMs the scan may occupy: all of them when it runs alone, the SMs the attention kernel leaves free when
+// it runs beside the denoising steps.
+struct ScanRange {
+    int64_t g0, g1;   // this CTA's range of global tile indices
+};
+__device__ __forceinline__ int seq_pages(const ScanParams& p, int b) {
+    return (min(p.seq_lens[b], p.max_seq_len) + kPageSize - 1) / kPageSize;
+}
+__device__ __forceinline__ int64_t cta_range_begin(int64_t total, int cta, int n_ctas) { return total * cta / n_ctas; }
+
 template <int kMode>
-__global__ void __launch_bounds__(kScanThreads, 2) scan_kernel(const ScanParams p) {
+__global__ void __launch_bounds__(kScanThreads, 1) scan_kernel(const ScanParams p) {
     __shared__ uint32_t s_hist[kMode == 0 ? kBins1 : 1];
     __shared__ float2 s_stats[kMode == 1 ? kScanWarps * 8 : 1];
+    __shared__ int64_t s_total;
 
-    const int b = blockIdx.z, h = blockIdx.y;
-    const int unit = b * p.n_kv_heads + h;
-    const int L = min(p.seq_lens[b], p.max_seq_len);
-    const int n_pages = (L + kPageSize - 1) / kPageSize;
     const int G = p.n_q_heads / p.n_kv_heads;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = lane >> 2, tig = lane & 3;
 
-    if (kMode == 0) {
+    if (threadIdx.x == 0) {
+        int64_t total = 0;
+        for (int b = 0; b < p.batch; ++b) total += (int64_t)seq_pages(p, b) * p.n_kv_heads;
+        s_total = total;
+    }
+    if (kMode == 0)
         for (int i = threadIdx.x; i < kBins1; i += kScanThreads) s_hist[i] = 0;
-        __syncthreads();
-    }
+    __syncthreads();
+    const int64_t total = s_total;
+    const int64_t g0 = cta_range_begin(total, blockIdx.x, gridDim.x), g1 = cta_range_begin(total, blockIdx.x + 1, gridDim.x);
 
-    // B operand: query head g of this KV head's group (zeros for g >= G), channel-permuted like A.
-    uint4 qf[4];
-    {
-        const __nv_bfloat16* qrow = p.q_rep + ((int64_t)b * p.n_q_heads + h * G + g) * kHeadDim + 8 * tig;
+    // walk the units that intersect [g0, g1)
+    int64_t unit_begin = 0;   // global tile index of the current unit's page 0
+    for (int b = 0; b < p.batch && unit_begin < g1; ++b) {
+        const int L = min(p.seq_lens[b], p.max_seq_len);
+        const int n_pages = (L + kPageSize - 1) / kPageSize;
+        const int32_t* pt = p.page_table + (int64_t)b * p.max_pages;
+        for (int h = 0; h < p.n_kv_heads; ++h, unit_begin += n_pages) {
+            const int64_t lo = max(g0, unit_begin), hi = min(g1, unit_begin + n_pages);
+            if (lo >= hi) continue;                       // block-uniform
+            const int unit = b * p.n_kv_heads + h;
+            const int page_lo = (int)(lo - unit_begin), page_hi = (int)(hi - unit_begin);
+
+            // B operand: query head g of this KV head's group (zeros for g >= G), channel-permuted like A.
+            uint4 qf[4];
+            {
+                const __nv_bfloat16* qrow = p.q_rep + ((int64_t)b * p.n_q_heads + h * G + g) * kHeadDim + 8 * tig;
 #pragma unroll
-        for (int i = 0; i < 4; ++i) qf[i] = (g < G) ? ldg_u4(qrow + 32 * i) : make_uint4(0, 0, 0, 0);
-    }
-
-    // running softmax statistics of columns 2*tig, 2*tig+1 over this thread's rows (mode 1)
-    float run_m[2] = {-INFINITY, -INFINITY}, run_l[2] = {0.f, 0.f};
-
-    const int32_t* pt = p.page_table + (int64_t)b * p.max_pages;
-    const int stride = gridDim.x * kScanWarps;
-    int page = blockIdx.x * kScanWarps + warp;
-    int phys = page < n_pages ? __ldg(pt + page) : 0;
-    float* score_row = p.scores + (int64_t)unit * p.max_seq_len;
-
-    while (page < n_pages) {
-        const int next = page + stride;
-        const int phys_next = next < n_pages ? __ldg(pt + next) : 0;
-
-        const __nv_bfloat16* base = p.k_pages + (int64_t)phys * p.page_stride + (int64_t)h * p.head_stride + 8 * tig;
-        const __nv_bfloat16* r0 = base + (int64_t)g * p.token_stride;
-        const __nv_bfloat16* r1 = base + (int64_t)(g + 8) * p.token_stride;
-        uint4 a[4], c[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            a[i] = ldg_stream_u4(r0 + 32 * i);
-            c[i] = ldg_stream_u4(r1 + 32 * i);
-        }
-        float acc[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            mma_bf16_16816(acc, a[i].x, c[i].x, a[i].y, c[i].y, qf[i].x, qf[i].y);
-            mma_bf16_16816(acc, a[i].z, c[i].z, a[i].w, c[i].w, qf[i].z, qf[i].w);
-        }
-        // acc[0],acc[1]: token row g, heads 2*tig, 2*tig+1 ; acc[2],acc[3]: token row g+8
-        const int t0 = page * kPageSize;
-        if (kMode == 0) {
-            const bool v0 = 2 * tig < G, v1 = 2 * tig + 1 < G;
-            float m0 = fmaxf(v0 ? acc[0] : -INFINITY, v1 ? acc[1] : -INFINITY);
-            float m1 = fmaxf(v0 ? acc[2] : -INFINITY, v1 ? acc[3] : -INFINITY);
-            m0 = fmaxf(m0, __shfl_xor_sync(0xffffffffu, m0, 1));
-            m1 = fmaxf(m1, __shfl_xor_sync(0xffffffffu, m1, 1));
-            m0 = fmaxf(m0, __shfl_xor_sync(0xffffffffu, m0, 2));
-            m1 = fmaxf(m1, __shfl_xor_sync(0xffffffffu, m1, 2));
-            // lanes with tig 0 publish row g, lanes with tig 1 publish row g+8: 16 lanes -> 64 contiguous bytes
-            const int t = t0 + (tig == 0 ? g : g + 8);
-            if (tig < 2 && t < L) {
-                const float v = (tig == 0 ? m0 : m1) * p.sm_scale;
-                score_row[t] = v;
-                atomicAdd(&s_hist[score_key(v) >> (32 - kBits1)], 1u);
+                for (int i = 0; i < 4; ++i) qf[i] = (g < G) ? ldg_u4(qrow + 32 * i) : make_uint4(0, 0, 0, 0);
             }
-        } else {
-            float* raw_unit = p.raw + (int64_t)unit * G * p.max_seq_len;
+            // running softmax statistics of columns 2*tig, 2*tig+1 over this thread's rows (mode 1)
+            float run_m[2] = {-INFINITY, -INFINITY}, run_l[2] = {0.f, 0.f};
+            float* score_row = p.scores + (int64_t)unit * p.max_seq_len;
+
+            int page = page_lo + warp;
+            int phys = page < page_hi ? __ldg(pt + page) : 0;
+            while (page < page_hi) {
+                const int next = page + kScanWarps;
+                const int phys_next = next < page_hi ? __ldg(pt + next) : 0;
+
+                const __nv_bfloat16* base = p.k_pages + (int64_t)phys * p.page_stride + (int64_t)h * p.head_stride + 8 * tig;
+                const __nv_bfloat16* r0 = base + (int64_t)g * p.token_stride;
+                const __nv_bfloat16* r1 = base + (int64_t)(g + 8) * p.token_stride;
+                uint4 a[4], c[4];
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const int col = 2 * tig + (e & 1);
-                const int t = t0 + g + ((e >> 1) ? 8 : 0);
-                if (col < G && t < L) {
-                    const float v = acc[e] * p.sm_scale;
-                    raw_unit[(int64_t)col * p.max_seq_len + t] = v;
-                    const int c2 = e & 1;
-                    const float mn = fmaxf(run_m[c2], v);
-                    run_l[c2] = run_l[c2] * __expf(run_m[c2] - mn) + __expf(v - mn);
-                    run_m[c2] = mn;
+                for (int i = 0; i < 4; ++i) {
+                    a[i] = ldg_stream_u4(r0 + 32 * i);
+                    c[i] = ldg_stream_u4(r1 + 32 * i);
                 }
+                float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    mma_bf16_16816(acc, a[i].x, c[i].x, a[i].y, c[i].y, qf[i].x, qf[i].y);
+                    mma_bf16_16816(acc, a[i].z, c[i].z, a[i].w, c[i].w, qf[i].z, qf[i].w);
+                }
+                // acc[0],acc[1]: token row g, heads 2*tig, 2*tig+1 ; acc[2],acc[3]: token row g+8
+                const int t0 = page * kPageSize;
+                if (kMode == 0) {
+                    const bool v0 = 2 * tig < G, v1 = 2 * tig + 1 < G;
+                    float m0 = fmaxf(v0 ? acc[0] : -INFINITY, v1 ? acc[1] : -INFINITY);
+                    float m1 = fmaxf(v0 ? acc[2] : -INFINITY, v1 ? acc[3] : -INFINITY);
+                    m0 = fmaxf(m0, __shfl_xor_sync(0xffffffffu, m0, 1));
+                    m1 = fmaxf(m1, __shfl_xor_sync(0xffffffffu, m1, 1));
+                    m0 = fmaxf(m0, __shfl_xor_sync(0xffffffffu, m0, 2));
+                    m1 = fmaxf(m1, __shfl_xor_sync(0xffffffffu, m1, 2));
+                    // lanes with tig 0 publish row g, lanes with tig 1 publish row g+8: 16 lanes -> 64 contiguous bytes
+                    const int t = t0 + (tig == 0 ? g : g + 8);
+                    if (tig < 2 && t < L) {
+                        const float v = (tig == 0 ? m0 : m1) * p.sm_scale;
+                        score_row[t] = v;
+                        atomicAdd(&s_hist[score_key(v) >> (32 - kBits1)], 1u);
+                    }
+                } else {
+                    float* raw_unit = p.raw + (int64_t)unit * G * p.max_seq_len;
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const int col = 2 * tig + (e & 1);
+                        const int t = t0 + g + ((e >> 1) ? 8 : 0);
+                        if (col < G && t < L) {
+                            const float v = acc[e] * p.sm_scale;
+                            raw_unit[(int64_t)col * p.max_seq_len + t] = v;
+                            const int c2 = e & 1;
+                            const float mn = fmaxf(run_m[c2], v);
+                            run_l[c2] = run_l[c2] * __expf(run_m[c2] - mn) + __expf(v - mn);
+                            run_m[c2] = mn;
+                        }
+                    }
+                }
+                page = next;
+                phys = phys_next;
             }
-        }
-        page = next;
-        phys = phys_next;
-    }
 
-    if (kMode == 0) {
-        __syncthreads();
-        uint32_t* gh = p.hist1 + (int64_t)unit * kBins1;
-        for (int i = threadIdx.x; i < kBins1; i += kScanThreads) {
-            const uint32_t v = s_hist[i];
-            if (v) atomicAdd(gh + i, v);
-        }
-    } else {
-        // merge (m, l) over the 8 token-row groups of the warp (lanes with equal tig), then over warps
+            // ---- end of this CTA's share of the unit: flush ----
+            if (kMode == 0) {
+                __syncthreads();
+                uint32_t* gh = p.hist1 + (int64_t)unit * kBins1;
+                for (int i = threadIdx.x; i < kBins1; i += kScanThreads) {
+                    const uint32_t v = s_hist[i];
+                    if (v) {
+                        atomicAdd(gh + i, v);
+                        s_hist[i] = 0;
+                    }
+                }
+                __syncthreads();
+            } else {
+                // merge (m, l) over the 8 token-row groups of the warp (lanes with equal tig), then over warps
 #pragma unroll
-        for (int c2 = 0; c2 < 2; ++c2) {
-            float m = run_m[c2], l = run_l[c2];
+                for (int c2 = 0; c2 < 2; ++c2) {
+                    float m = run_m[c2], l = run_l[c2];
 #pragma unroll
-            for (int o = 4; o < 32; o <<= 1) {
-                const float mo = __shfl_xor_sync(0xffffffffu, m, o), lo = __shfl_xor_sync(0xffffffffu, l, o);
-                const float mn = fmaxf(m, mo);
-                l = (m == -INFINITY ? 0.f : l * __expf(m - mn)) + (mo == -INFINITY ? 0.f : lo * __expf(mo - mn));
-                m = mn;
+                    for (int o = 4; o < 32; o <<= 1) {
+                        const float mo = __shfl_xor_sync(0xffffffffu, m, o), lo2 = __shfl_xor_sync(0xffffffffu, l, o);
+                        const float mn = fmaxf(m, mo);
+                        l = (m == -INFINITY ? 0.f : l * __expf(m - mn)) + (mo == -INFINITY ? 0.f : lo2 * __expf(mo - mn));
+                        m = mn;
+                    }
+                    if (g == 0) s_stats[warp * 8 + 2 * tig + c2] = make_float2(m, l);
+                }
+                __syncthreads();
+                if (threadIdx.x < G) {
+                    float m = -INFINITY, l = 0.f;
+                    for (int w = 0; w < kScanWarps; ++w) {
+                        const float2 st = s_stats[w * 8 + threadIdx.x];
+                        const float mn = fmaxf(m, st.x);
+                        l = (m == -INFINITY ? 0.f : l * __expf(m - mn)) + (st.x == -INFINITY ? 0.f : st.y * __expf(st.x - mn));
+                        m = mn;
+                    }
+                    p.stats_part[((int64_t)unit * G + threadIdx.x) * gridDim.x + blockIdx.x] = make_float2(m, l);
+                }
+                __syncthreads();
             }
-            if (g == 0) s_stats[warp * 8 + 2 * tig + c2] = make_float2(m, l);
-        }
-        __syncthreads();
-        if (threadIdx.x < G) {
-            float m = -INFINITY, l = 0.f;
-            for (int w = 0; w < kScanWarps; ++w) {
-                const float2 s = s_stats[w * 8 + threadIdx.x];
-                const float mn = fmaxf(m, s.x);
-                l = (m == -INFINITY ? 0.f : l * __expf(m - mn)) + (s.x == -INFINITY ? 0.f : s.y * __expf(s.x - mn));
-                m = mn;
-            }
-            p.stats_part[((int64_t)unit * G + threadIdx.x) * gridDim.x + blockIdx.x] = make_float2(m, l);
         }
     }
 }
@@ -162,11 +195,11 @@ __global__ void __launch_bounds__(kScanThreads, 2) scan_kernel(const ScanParams 
 struct AggParams {
     const float* raw;
     const float2* stats_part;
-    int32_t n_parts;
+    int32_t n_parts;      // grid size of the scan that wrote stats_part
     const int32_t* seq_lens;
     float* scores;
     uint32_t* hist1;
-    int32_t n_q_heads, n_kv_heads, max_seq_len;
+    int32_t batch, n_q_heads, n_kv_heads, max_seq_len;
 };
 
 __global__ void __launch_bounds__(256) aggregate_softmax_kernel(const AggParams p) {
@@ -178,9 +211,21 @@ __global__ void __launch_bounds__(256) aggregate_softmax_kernel(const AggParams 
     const int L = min(p.seq_lens[b], p.max_seq_len);
     for (int i = threadIdx.x; i < kBins1; i += blockDim.x) s_hist[i] = 0;
     if (threadIdx.x < G) {
+        // the scan CTAs whose tile range intersects this unit wrote a partial (same range arithmetic as scan_kernel)
+        int64_t total = 0, unit_begin = 0;
+        for (int bb = 0; bb < p.batch; ++bb) {
+            const int np = (min(p.seq_lens[bb], p.max_seq_len) + kPageSize - 1) / kPageSize;
+            if (bb < b) unit_begin += (int64_t)np * p.n_kv_heads;
+            total += (int64_t)np * p.n_kv_heads;
+        }
+        const int n_pages = (L + kPageSize - 1) / kPageSize;
+        unit_begin += (int64_t)h * n_pages;
         float m = -INFINITY, l = 0.f;
         const float2* sp = p.stats_part + ((int64_t)unit * G + threadIdx.x) * p.n_parts;
         for (int i = 0; i < p.n_parts; ++i) {
+            const int64_t lo = max(cta_range_begin(total, i, p.n_parts), unit_begin);
+            const int64_t hi = min(cta_range_begin(total, i + 1, p.n_parts), unit_begin + n_pages);
+            if (lo >= hi) continue;
             const float2 s = sp[i];
             const float mn = fmaxf(m, s.x);
             l = (m == -INFINITY ? 0.f : l * __expf(m - mn)) + (s.x == -INFINITY ? 0.f : s.y * __expf(s.x - mn));

@@ -24,7 +24,7 @@ OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE_TOO_SMALL, ERR_CUDA = 0, -1,
 AGG_MAX_LOGIT, AGG_SOFTMAX_SUM = 0, 1
 
 EXPORTS = ("herald_last_error", "herald_budget_rows", "herald_select_workspace_bytes",
-           "herald_attn_workspace_bytes", "herald_select", "herald_gather", "herald_sparse_attn",
+           "herald_attn_workspace_bytes", "herald_attn_grid_ctas", "herald_select", "herald_gather", "herald_sparse_attn",
            "herald_pipeline_step", "herald_pipeline_step_host", "herald_pipeline_set_profile")
 
 
@@ -55,7 +55,8 @@ class Layer(C.Structure):
 
 class Pipeline(C.Structure):
     _fields_ = [("shape", Shape), ("n_layers", C.c_int32), ("n_steps", C.c_int32),
-                ("start_after_step", C.c_int32), ("active", C.c_int32), ("layers", C.POINTER(Layer)),
+                ("start_after_step", C.c_int32), ("active", C.c_int32), ("retrieval_sms", C.c_int32),
+                ("layers", C.POINTER(Layer)),
                 ("sel_idx", C.c_void_p), ("ws_select", C.c_void_p), ("ws_select_bytes", C.c_size_t),
                 ("ws_attn", C.c_void_p), ("ws_attn_bytes", C.c_size_t),
                 ("main_stream", C.c_void_p), ("retrieval_stream", C.c_void_p),
@@ -81,6 +82,8 @@ _lib.herald_select_workspace_bytes.restype = C.c_size_t
 _lib.herald_select_workspace_bytes.argtypes = [C.POINTER(Shape)]
 _lib.herald_attn_workspace_bytes.restype = C.c_size_t
 _lib.herald_attn_workspace_bytes.argtypes = [C.POINTER(Shape)]
+_lib.herald_attn_grid_ctas.restype = C.c_int32
+_lib.herald_attn_grid_ctas.argtypes = [C.POINTER(Shape)]
 _lib.herald_select.restype = C.c_int
 _lib.herald_select.argtypes = [C.POINTER(Shape), C.POINTER(Cache), C.c_void_p, C.c_void_p, C.c_void_p,
                                C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
@@ -156,6 +159,10 @@ def herald_attn_workspace_bytes(shape: Shape) -> int:
     return int(_lib.herald_attn_workspace_bytes(C.byref(shape)))
 
 
+def herald_attn_grid_ctas(shape: Shape) -> int:
+    return int(_lib.herald_attn_grid_ctas(C.byref(shape)))
+
+
 def herald_select(shape, cache, q_rep, k_per_seq, sel_idx, sel_cnt, scores_out, ws, stream=None):
     ws_ptr, ws_bytes = _ws(ws)
     _check(_lib.herald_select(C.byref(shape), C.byref(cache), _ptr(q_rep), _ptr(k_per_seq), _ptr(sel_idx),
@@ -200,7 +207,7 @@ class BlockPipeline:
     """Owns the device buffers of a dual-stream block pipeline (pools, workspaces, streams, events)
     and the ctypes structs that describe them.  Marshalling and memory ownership only."""
 
-    def __init__(self, shape: Shape, layers, n_steps: int, start_after_step: int = 0, device="cuda"):
+    def __init__(self, shape: Shape, layers, n_steps: int, start_after_step: int = 0, device="cuda", retrieval_sms=None):
         """layers: list of dicts with torch tensors k_pages, v_pages, page_table, seq_lens, q_rep, k_per_seq,
         q_blk, k_blk, v_blk ([n_steps, ...])."""
         dev = torch.device(device)
@@ -236,6 +243,11 @@ class BlockPipeline:
             self.ev_join.record(self.retrieval_stream)
         p = Pipeline()
         p.shape, p.n_layers, p.n_steps, p.start_after_step, p.active = shape, len(layers), n_steps, start_after_step, 0
+        if retrieval_sms is None:
+            # the score scan takes the SMs the attention grid leaves free (at least 1/8 of the device)
+            n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+            retrieval_sms = max(n_sm - herald_attn_grid_ctas(shape), n_sm // 8)
+        p.retrieval_sms = int(retrieval_sms)
         p.layers = C.cast(self.layer_arr, C.POINTER(Layer))
         p.sel_idx = _ptr(self.sel_idx)
         p.ws_select, p.ws_select_bytes = _ptr(self.ws_select), self.ws_select.numel()
@@ -265,3 +277,28 @@ class BlockPipeline:
 
     def step_host(self, io: HostIO):
         herald_pipeline_step_host(self.c, io)
+
+    # ---- CUDA graphs: one captured block step per pool parity (launch-bound inner loop, no per-launch host cost) ----
+    def capture(self, io: HostIO = None):
+        """Capture herald_pipeline_step (or the host-IO variant) twice, once per value of ``active``, into two CUDA
+        graphs whose root is the main stream; the retrieval stream joins the capture through the fork/join events.
+        Run at least one eager step first (function attributes and tensor maps are set up on first use)."""
+        graphs = {}
+        start = self.active
+        for _ in range(2):
+            parity = self.active
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=self.main_stream, capture_error_mode="thread_local"):
+                if io is None:
+                    herald_pipeline_step(self.c)
+                else:
+                    herald_pipeline_step_host(self.c, io)
+            graphs[parity] = g                      # the capture flipped ->active exactly like an eager step
+        assert self.active == start
+        return graphs
+
+    def replay(self, graphs):
+        """Launch the captured step for the current parity on the main stream and flip ``active``."""
+        with torch.cuda.stream(self.main_stream):
+            graphs[self.active].replay()
+        self.c.active = 1 - self.c.active
