@@ -302,7 +302,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     const int per = (n_tiles + S - 1) / S;
     const int t0 = split * per, t1 = min(n_tiles, t0 + per);
     const int nt = max(t1 - t0, 0);                          // tile j of this CTA is key tile t0 + j
-    const int rows_own = (kTcBM + S - 1) / S;                // tile rows merged and written by each CTA of the cluster
+    const int rows_own = (rows_box + S - 1) / S;             // tile rows merged and written by each CTA of the cluster (zero rows past the box are nobody's)
     const int ml_stride = (rows_own + 1) & ~1;               // float2 per source, padded to 16 bytes
     const int g_inv = (65536 + G - 1) / G;                   // (r * g_inv) >> 16 == r / G for r < 128, G <= 8
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -583,7 +583,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
 #pragma unroll
             for (int i = 0; i < 32; ++i) o[i] = 0.f;
         }
-        if (owner != split) {
+        if (owner != split && row < rows_box) {
             // stage this quarter row (unnormalised) and (m, l) for its owner; slots skip the sender / the owner itself
             const int d = owner < split ? owner : owner - 1;
             float4* dst = reinterpret_cast<float4*>(sgen + kTcPushO + ((d * rows_own + row_l) * kTcRowFloats + cq * 32) * 4);
@@ -611,11 +611,13 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
             dsmem_bulk_copy(map_to_cta(sbase + kTcRecvML + src_slot * ml_stride * 8, dst_cta),
                             sbase + push_ml_off + d * ml_stride * 8, ml_stride * 8, bar_remote);
     }
-    if (warp < kTcSoftmaxWarps && owner == split) {
-        if (S > 1) mbar_wait(bar(kBarMerge), 0);
-        if (tid == 0) HERALD_STAMP(3);
+    if (warp < kTcSoftmaxWarps && S > 1) {
+        mbar_wait(bar(kBarMerge), 0);
         // every partial row addressed to this CTA has landed: release the senders (they may not exit before)
-        if (S > 1 && cq == 0 && row_l < S - 1) mbar_arrive_remote(map_to_cta(bar(kBarAck), row_l < split ? row_l : row_l + 1));
+        if (tid < S - 1) mbar_arrive_remote(map_to_cta(bar(kBarAck), tid < split ? tid : tid + 1));
+    }
+    if (tid == 0) HERALD_STAMP(3);
+    if (warp < kTcSoftmaxWarps && owner == split) {
         if (row < rows_valid) {
             const float* recv_o = reinterpret_cast<const float*>(sgen + kTcRecvO);
             const float2* recv_ml = reinterpret_cast<const float2*>(sgen + kTcRecvML);

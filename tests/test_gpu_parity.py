@@ -203,6 +203,27 @@ def test_sparse_attn_split_kv_is_consistent(H, cuda, splits, monkeypatch):
     assert np.abs(out.cpu().numpy() - ref).max() <= ATTN_TOL
 
 
+@pytest.mark.parametrize("splits", [7, 8])
+def test_sparse_attn_more_splits_than_tile_rows(H, cuda, splits, monkeypatch):
+    """G = 1, B = 8: the M tile has 8 real rows, so with 7 or 8 KV splits some CTAs of the cluster own no row at all;
+    they still send their partials and are still acknowledged."""
+    monkeypatch.setenv("HERALD_ATTN_SPLITS", str(splits))
+    batch, B, Hq, Hkv, cap = 2, 8, 2, 2, 1100
+    q, kb, vb, pk, pv, pl = _attn_case(cuda, batch, B, Hq, Hkv, cap, [[1100, 900], [130, 0]], seed=78)
+    shape = H.make_shape(batch, Hq, Hkv, B, 16, 1, cap)
+    out = torch.full((batch, B, Hq, 128), float("nan"), dtype=torch.float32, device=cuda)
+    lse = torch.empty((batch, B, Hq), dtype=torch.float32, device=cuda)
+    ws = H.alloc_workspace(H.herald_attn_workspace_bytes(shape), cuda)
+    H.herald_sparse_attn(shape, pk, pv, pl, q, kb, vb, out, lse, ws)
+    torch.cuda.synchronize()
+    pv_clean = pv.clone()
+    pv_clean[torch.isnan(pv_clean)] = 0
+    ref, lse_ref = O.sparse_attn(synth.to_u16(q), synth.to_u16(kb), synth.to_u16(vb), synth.to_u16(pk),
+                                 synth.to_u16(pv_clean), pl.cpu().numpy(), 128 ** -0.5)
+    assert np.abs(out.cpu().numpy() - ref).max() <= ATTN_TOL
+    assert np.abs(lse.cpu().numpy() - lse_ref).max() <= 2e-3
+
+
 def _layer_inputs(w, inp, ks, cuda):
     return dict(k_pages=inp["k_pages"], v_pages=inp["v_pages"], page_table=inp["page_table"], seq_lens=inp["seq_lens"],
                 q_rep=inp["q_rep"], k_per_seq=torch.tensor(ks, dtype=torch.int32, device=cuda),
