@@ -1,18 +1,25 @@
 // Exact per-(sequence, KV head) top-k of the score plane (step a3 of DESIGN.md).
 //
 // The paper keeps a min-heap on the CPU; on the GPU the same result (the k largest scores, ties to
-// the lower position, emitted in ascending position) is a three-level MSB-first radix select on an
-// order-preserving 32-bit key (12 + 10 + 10 bits) followed by an ordered compaction:
-//   level 1 histogram : already accumulated by the scan kernel's epilogue (hist1),
-//   level 2, 3        : histograms of the elements inside the threshold bin (few smem atomics),
-//   compaction        : keys > T, plus the first `need` keys == T in position order, via block scans.
-// One 1024-thread CTA per unit; the score plane (<= 512 KB per unit) is read from L2.
+// the lower position, emitted in ascending position) is an MSB-first radix select on an order-preserving
+// 32-bit key (12 + 10 + 10 bits).  One 1024-thread CTA per unit.
+//   level 1 histogram : already accumulated by the scan kernel's epilogue (hist1) -> threshold bin b1
+//   fast path (the threshold bin holds <= kTopkCandCap scores, positions < 32 * kTopkBitmapWords):
+//     ONE pass over the score plane: scores above bin b1 set their bit in a shared-memory position bitmap,
+//     scores inside bin b1 are appended (key, position) to a shared-memory candidate list (warp-aggregated);
+//     levels 2 and 3 run on the candidate list; exact ties keep the lowest positions through a second bitmap
+//     and a block prefix sum; the result is emitted in ascending position from the bitmap (popcount prefix).
+//   slow path (anything else, e.g. all scores equal): levels 2 and 3 re-read the plane from L2 and an ordered
+//     compaction by block prefix sums emits the positions.
 #pragma once
 #include "common.cuh"
 
 namespace herald {
 
 constexpr int kTopkThreads = 1024;
+constexpr int kTopkCandCap = 12288;                 // (key, position) pairs of the threshold bin held in shared memory
+constexpr int kTopkBitmapWords = 8192;              // one bit per position: fast path for L <= 262144
+constexpr int kTopkSmemBytes = kTopkCandCap * 8 + 2 * kTopkBitmapWords * 4;   // candidates, selected bitmap, tie bitmap
 
 // Find bin j with  count(bins > j) < kk <= count(bins >= j).  Returns j, *above = count(bins > j).
 // hist has nbins (multiple of blockDim) entries in shared memory; every thread must call.
@@ -55,6 +62,7 @@ __global__ void __launch_bounds__(kTopkThreads, 1) topk_kernel(const TopkParams 
     __shared__ uint32_t s_hist[kBins1];
     __shared__ uint32_t s_warp[33];
     __shared__ uint32_t s_res[2];
+    __shared__ uint32_t s_ncand;
 
     const int unit = blockIdx.x;
     const int b = unit / p.n_kv_heads;
@@ -68,13 +76,113 @@ __global__ void __launch_bounds__(kTopkThreads, 1) topk_kernel(const TopkParams 
     int32_t* out = p.sel_idx + (int64_t)unit * p.cap;
     const int tid = threadIdx.x;
 
-    if (tid == 0) { s_res[0] = 0; s_res[1] = 0; }
+    if (tid == 0) { s_res[0] = 0; s_res[1] = 0; s_ncand = 0; }
     for (int i = tid; i < kBins1; i += kTopkThreads) s_hist[i] = p.hist1[(int64_t)unit * kBins1 + i];
     __syncthreads();
     uint32_t above1, above2, above3;
     const uint32_t b1 = find_threshold_bin(s_hist, kBins1, (uint32_t)kk, s_warp, s_res, &above1);
     const uint32_t k2 = kk - above1;
 
+    const uint32_t n_c = s_hist[b1];                   // scores inside the threshold bin
+    if (n_c <= (uint32_t)kTopkCandCap && L <= 32 * kTopkBitmapWords) {
+        // ---------------- fast path: one pass over the plane ----------------
+        extern __shared__ __align__(16) uint8_t topk_smem[];
+        uint2* cand = reinterpret_cast<uint2*>(topk_smem);                                   // (key, position)
+        uint32_t* bitmap = reinterpret_cast<uint32_t*>(topk_smem + kTopkCandCap * 8);        // selected positions
+        uint32_t* tiemap = bitmap + kTopkBitmapWords;                                        // positions with key == T
+        const int n_words = (L + 31) >> 5;
+        const int lane = tid & 31;
+        for (int i = tid; i < n_words; i += kTopkThreads) { bitmap[i] = 0; tiemap[i] = 0; }
+        __syncthreads();
+        for (int tile = 0; tile < L; tile += kTopkThreads * 4) {
+            const int i = tile + tid * 4;
+            float ve[4] = {0.f, 0.f, 0.f, 0.f};
+            if (i < L) {
+                const float4 v = *reinterpret_cast<const float4*>(sc + i);
+                ve[0] = v.x; ve[1] = v.y; ve[2] = v.z; ve[3] = v.w;
+            }
+            uint32_t above = 0;
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const bool in = i + e < L;
+                const uint32_t key = score_key(ve[e]);
+                const uint32_t bin = key >> (32 - kBits1);
+                if (in && bin > b1) above |= 1u << e;
+                const bool is_c = in && bin == b1;
+                const uint32_t m = __ballot_sync(0xffffffffu, is_c);
+                if (m) {
+                    uint32_t base = 0;
+                    if (lane == 0) base = atomicAdd(&s_ncand, (uint32_t)__popc(m));
+                    base = __shfl_sync(0xffffffffu, base, 0);
+                    if (is_c) cand[base + __popc(m & ((1u << lane) - 1u))] = make_uint2(key, (uint32_t)(i + e));
+                }
+            }
+            // the 4 positions of a thread share one bitmap word (i is a multiple of 4)
+            if (above) atomicOr(&bitmap[i >> 5], above << (i & 31));
+        }
+        __syncthreads();
+        // levels 2 and 3 on the candidates: the k2 largest of the low 20 key bits
+        for (int i = tid; i < kBins2; i += kTopkThreads) s_hist[i] = 0;
+        __syncthreads();
+        for (uint32_t c = tid; c < n_c; c += kTopkThreads) atomicAdd(&s_hist[(cand[c].x >> kBits3) & (kBins2 - 1)], 1u);
+        __syncthreads();
+        uint32_t above2f, above3f;
+        const uint32_t b2f = find_threshold_bin(s_hist, kBins2, k2, s_warp, s_res, &above2f);
+        const uint32_t k3f = k2 - above2f;
+        __syncthreads();
+        for (int i = tid; i < kBins3; i += kTopkThreads) s_hist[i] = 0;
+        __syncthreads();
+        for (uint32_t c = tid; c < n_c; c += kTopkThreads) {
+            const uint32_t key = cand[c].x;
+            if (((key >> kBits3) & (kBins2 - 1)) == b2f) atomicAdd(&s_hist[key & (kBins3 - 1)], 1u);
+        }
+        __syncthreads();
+        const uint32_t b3f = find_threshold_bin(s_hist, kBins3, k3f, s_warp, s_res, &above3f);
+        const uint32_t need_f = k3f - above3f;          // exact ties (key == T) to keep, lowest positions first
+        const uint32_t T = (b1 << (32 - kBits1)) | (b2f << kBits3) | b3f;
+        for (uint32_t c = tid; c < n_c; c += kTopkThreads) {
+            const uint2 kc = cand[c];
+            if (kc.x > T) atomicOr(&bitmap[kc.y >> 5], 1u << (kc.y & 31));
+            else if (kc.x == T) atomicOr(&tiemap[kc.y >> 5], 1u << (kc.y & 31));
+        }
+        __syncthreads();
+        const int wpt = (n_words + kTopkThreads - 1) / kTopkThreads;   // words per thread (<= 8), contiguous
+        const int w0 = tid * wpt, w1 = min(n_words, w0 + wpt);
+        {   // ties: keep the first need_f in position order
+            uint32_t cnt = 0;
+            for (int wd = w0; wd < w1; ++wd) cnt += __popc(tiemap[wd]);
+            uint32_t total;
+            uint32_t before = block_exclusive_scan(cnt, s_warp, &total);
+            for (int wd = w0; wd < w1 && before < need_f; ++wd) {
+                uint32_t t = tiemap[wd], keep = 0;
+                while (t && before < need_f) {
+                    const uint32_t bit = t & (0u - t);
+                    keep |= bit;
+                    t ^= bit;
+                    ++before;
+                }
+                bitmap[wd] |= keep;                     // this thread owns word wd in this phase
+            }
+        }
+        __syncthreads();
+        {   // emit the set positions in ascending order
+            uint32_t cnt = 0;
+            for (int wd = w0; wd < w1; ++wd) cnt += __popc(bitmap[wd]);
+            uint32_t total;
+            uint32_t at = block_exclusive_scan(cnt, s_warp, &total);
+            for (int wd = w0; wd < w1; ++wd) {
+                uint32_t t = bitmap[wd];
+                while (t) {
+                    out[at++] = wd * 32 + __ffs(t) - 1;
+                    t &= t - 1;
+                }
+            }
+        }
+        if (tid == 0) p.sel_cnt[unit] = kk;
+        return;
+    }
+
+    // ---------------- slow path: levels 2 and 3 and the compaction re-read the plane ----------------
     // level 2: next 10 bits, restricted to level-1 bin b1
     __syncthreads();
     for (int i = tid; i < kBins2; i += kTopkThreads) s_hist[i] = 0;
