@@ -379,7 +379,13 @@ int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, cons
     tp.n_kv_heads = shape->n_kv_heads;
     tp.max_seq_len = shape->max_seq_len;
     tp.cap = shape->pool_capacity;
-    topk_kernel<<<units, kTopkThreads, 0, stream>>>(tp);
+    static bool topk_attr_set = false;
+    if (!topk_attr_set) {
+        e = cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTopkSmemBytes);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(topk)");
+        topk_attr_set = true;
+    }
+    topk_kernel<<<units, kTopkThreads, kTopkSmemBytes, stream>>>(tp);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "topk launch");
     if (prof && prof->topk_end) cudaEventRecord(static_cast<cudaEvent_t>(prof->topk_end), stream);
