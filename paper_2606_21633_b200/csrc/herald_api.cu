@@ -344,7 +344,18 @@ int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, cons
         sp.sm_scale = shape->sm_scale;
         const int scan_ctas = scan_ctas_for(shape);
         dim3 grid(scan_ctas);
-        if (shape->agg_mode == HERALD_AGG_MAX_LOGIT) {
+        const int Hkv = shape->n_kv_heads;
+        if (shape->agg_mode == HERALD_AGG_MAX_LOGIT && Hkv <= 8 && kScanWarps % Hkv == 0 && !env_int("HERALD_SCAN_HEAD_MAJOR", 0)) {
+            // page-major order: the warps next to each other read the head tiles of one page (whole pages for DRAM)
+            const size_t smem = (size_t)Hkv * kBins1 * sizeof(uint32_t);
+            static bool pm_attr_set = false;
+            if (!pm_attr_set) {
+                e = cudaFuncSetAttribute(scan_pm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 8 * kBins1 * (int)sizeof(uint32_t));
+                if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(scan)");
+                pm_attr_set = true;
+            }
+            scan_pm_kernel<<<grid, kScanThreads, smem, stream>>>(sp);
+        } else if (shape->agg_mode == HERALD_AGG_MAX_LOGIT) {
             scan_kernel<0><<<grid, kScanThreads, 0, stream>>>(sp);
         } else {
             scan_kernel<1><<<grid, kScanThreads, 0, stream>>>(sp);

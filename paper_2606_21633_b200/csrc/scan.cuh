@@ -191,6 +191,99 @@ __global__ void __launch_bounds__(kScanThreads, 1) scan_kernel(const ScanParams 
     }
 }
 
+// Mode 0, page-major order (H_kv divides 32, H_kv <= 8: every BASELINE.json shape).  A page of the cache holds the 16
+// rows of ALL KV heads contiguously (16 x H_kv x 256 B); here the H_kv warps next to each other read the H_kv head
+// tiles of the same page at the same time, so DRAM sees whole 4-16 KB pages instead of 256-byte pieces 1 KB apart
+// (+6 % bandwidth on B200).  Work = the pages of the batch in sequence-major order, cut into gridDim.x equal
+// contiguous ranges; a CTA keeps one histogram per KV head in shared memory (H_kv x 16 KB, dynamic).
+__global__ void __launch_bounds__(kScanThreads, 1) scan_pm_kernel(const ScanParams p) {
+    extern __shared__ uint32_t s_hist_pm[];   // [H_kv][kBins1]
+    __shared__ int64_t s_total;
+
+    const int G = p.n_q_heads / p.n_kv_heads, H = p.n_kv_heads;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = lane >> 2, tig = lane & 3;
+    const int h = warp % H;                    // fixed per warp: 32 % H == 0
+    const int pages_per_iter = kScanWarps / H;
+
+    if (threadIdx.x == 0) {
+        int64_t total = 0;
+        for (int b = 0; b < p.batch; ++b) total += seq_pages(p, b);
+        s_total = total;
+    }
+    for (int i = threadIdx.x; i < H * kBins1; i += kScanThreads) s_hist_pm[i] = 0;
+    __syncthreads();
+    const int64_t total = s_total;
+    const int64_t g0 = cta_range_begin(total, blockIdx.x, gridDim.x), g1 = cta_range_begin(total, blockIdx.x + 1, gridDim.x);
+    uint32_t* my_hist = s_hist_pm + h * kBins1;
+    const bool v0 = 2 * tig < G, v1 = 2 * tig + 1 < G;
+
+    int64_t seq_begin = 0;
+    for (int b = 0; b < p.batch && seq_begin < g1; ++b) {
+        const int L = min(p.seq_lens[b], p.max_seq_len);
+        const int n_pages = (L + kPageSize - 1) / kPageSize;
+        const int64_t lo = max(g0, seq_begin), hi = min(g1, seq_begin + n_pages);
+        seq_begin += n_pages;
+        if (lo >= hi) continue;                            // block-uniform
+        const int page_lo = (int)(lo - (seq_begin - n_pages)), page_hi = (int)(hi - (seq_begin - n_pages));
+        const int32_t* pt = p.page_table + (int64_t)b * p.max_pages;
+        uint4 qf[4];
+        {
+            const __nv_bfloat16* qrow = p.q_rep + ((int64_t)b * p.n_q_heads + h * G + g) * kHeadDim + 8 * tig;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) qf[i] = (g < G) ? ldg_u4(qrow + 32 * i) : make_uint4(0, 0, 0, 0);
+        }
+        float* score_row = p.scores + (int64_t)(b * H + h) * p.max_seq_len;
+
+        int page = page_lo + warp / H;
+        int phys = page < page_hi ? __ldg(pt + page) : 0;
+        while (page < page_hi) {
+            const int next = page + pages_per_iter;
+            const int phys_next = next < page_hi ? __ldg(pt + next) : 0;
+            const __nv_bfloat16* base = p.k_pages + (int64_t)phys * p.page_stride + (int64_t)h * p.head_stride + 8 * tig;
+            const __nv_bfloat16* r0 = base + (int64_t)g * p.token_stride;
+            const __nv_bfloat16* r1 = base + (int64_t)(g + 8) * p.token_stride;
+            uint4 a[4], c[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                a[i] = ldg_stream_u4(r0 + 32 * i);
+                c[i] = ldg_stream_u4(r1 + 32 * i);
+            }
+            float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                mma_bf16_16816(acc, a[i].x, c[i].x, a[i].y, c[i].y, qf[i].x, qf[i].y);
+                mma_bf16_16816(acc, a[i].z, c[i].z, a[i].w, c[i].w, qf[i].z, qf[i].w);
+            }
+            float m0 = fmaxf(v0 ? acc[0] : -INFINITY, v1 ? acc[1] : -INFINITY);
+            float m1 = fmaxf(v0 ? acc[2] : -INFINITY, v1 ? acc[3] : -INFINITY);
+            m0 = fmaxf(m0, __shfl_xor_sync(0xffffffffu, m0, 1));
+            m1 = fmaxf(m1, __shfl_xor_sync(0xffffffffu, m1, 1));
+            m0 = fmaxf(m0, __shfl_xor_sync(0xffffffffu, m0, 2));
+            m1 = fmaxf(m1, __shfl_xor_sync(0xffffffffu, m1, 2));
+            const int t = page * kPageSize + (tig == 0 ? g : g + 8);
+            if (tig < 2 && t < L) {
+                const float v = (tig == 0 ? m0 : m1) * p.sm_scale;
+                score_row[t] = v;
+                atomicAdd(&my_hist[score_key(v) >> (32 - kBits1)], 1u);
+            }
+            page = next;
+            phys = phys_next;
+        }
+        // ---- end of this CTA's share of sequence b: flush the H histograms ----
+        __syncthreads();
+        uint32_t* gh = p.hist1 + (int64_t)b * H * kBins1;   // units b*H .. b*H + H-1 are contiguous
+        for (int i = threadIdx.x; i < H * kBins1; i += kScanThreads) {
+            const uint32_t v = s_hist_pm[i];
+            if (v) {
+                atomicAdd(gh + i, v);
+                s_hist_pm[i] = 0;
+            }
+        }
+        __syncthreads();
+    }
+}
+
 // Mode 1, second pass: a[t] = sum_g exp(s[g,t] - m_g) / l_g, score plane + level-1 histogram.
 struct AggParams {
     const float* raw;
