@@ -30,6 +30,9 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/r1_*), by workload
+NCU_ATTN_DRAM_BYTES = {"C2": 30.7e6}
+NCU_SCAN_DRAM_BYTES = {"C2": 274.2e6}
 METRIC = "selection-scan HBM GB/s (% of 8 TB/s); sparse-attn TFLOP/s; block tokens/s"
 WORKLOAD = "C2"
 SEED = 21633 + 1000 * 2
@@ -189,7 +192,8 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": "tokens/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{WORKLOAD}: Qwen2.5-7B-shaped layer 28/4/128, batch 8 x 32768, B=32, T=16, 5% budget",
+            "config": {"workload": f"{WORKLOAD}: single layer 28/4/128 heads, batch 8 x 32768 paged (16-token pages), B=32, T=16 "
+                                   "(15 attention steps), budget 5% k=1639, structure planted",
                        "note": f"oracle timed on a bounded sample: {n_seq} of {w.batch} sequences per step"},
             "cpu_baseline": {"value": value, "unit": "tokens/s", "cores": blas_threads(), "kind": "oracle",
                              "sample": f"{n_seq} of {w.batch} sequences of {WORKLOAD} per step"},
@@ -218,10 +222,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="herald", choices=["herald", "reference"])
     ap.add_argument("--workload", default=WORKLOAD)
-    ap.add_argument("--start-after-step", type=int, default=0)
+    ap.add_argument("--start-after-step", type=int, default=None,
+                    help="denoising steps before the retrieval stream starts (default: 0 or T-1, calibrated)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--retrieval-sms", type=int, default=None,
-                    help="SMs the overlapped score scan may occupy (default: the SMs the attention grid leaves free)")
+    ap.add_argument("--scan-ctas", type=int, default=None,
+                    help="grid of the overlapped score scan (default: calibrated before the timed region)")
     ap.add_argument("--no-graph", action="store_true", help="launch every kernel eagerly instead of replaying the captured block step")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -246,7 +251,7 @@ def main():
     k_per_seq = torch.tensor(ks, dtype=torch.int32, device=dev)
     layer = dict(k_pages=inp["k_pages"], v_pages=inp["v_pages"], page_table=inp["page_table"], seq_lens=inp["seq_lens"],
                  q_rep=inp["q_rep"], k_per_seq=k_per_seq, q_blk=inp["q_blk"], k_blk=inp["k_blk"], v_blk=inp["v_blk"])
-    pipe = H.BlockPipeline(shape, [layer], n_steps, args.start_after_step, dev, retrieval_sms=args.retrieval_sms)
+    pipe = H.BlockPipeline(shape, [layer], n_steps, args.start_after_step or 0, dev, scan_ctas=args.scan_ctas)
     units = w.batch * w.n_kv_heads
     G, M = w.group, w.block_size * w.group
 
@@ -266,6 +271,10 @@ def main():
     for _ in range(max(args.warmup, 3)):
         pipe.step()
     torch.cuda.synchronize()
+    rs_sweep = None
+    if args.scan_ctas is None:
+        # untimed calibration: which SM budget for the overlapped score scan gives the shortest block step
+        rs_sweep = pipe.tune_schedule(tune_start=args.start_after_step is None)
     graphs = None
     if not args.no_graph:
         # the block step is launch-bound (18 kernels of 5-60 us): capture it once per pool parity and replay
@@ -403,10 +412,12 @@ def main():
     attn_tflops_live = attn_flops / (attn_live_ms * 1e-3) / 1e12
     roofline = {"kernel": "attn_tc_kernel", "bound": "tensor", "achieved": attn_tflops_live,
                 "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s", "frac": attn_tflops_live / peaks["bf16_tflops_sustained"],
-                "traffic": None, "peak_source": peaks["source"] + " (sustained bf16, kernel timed inside a long step)",
-                "note": "dominant kernel by time share; achieved = 4*M*(n+B)*128 FLOP per launch / (step time / 15 launches)"}
-    roofline_scan = {"kernel": "scan_kernel<0>", "bound": "hbm", "achieved": scan_gbs_live, "peak": peaks["hbm_gbs"],
-                     "unit": "GB/s", "frac": scan_gbs_live / peaks["hbm_gbs"], "traffic": None,
+                "traffic": NCU_ATTN_DRAM_BYTES.get(w.name),
+                "peak_source": peaks["source"] + " (sustained bf16, kernel timed inside a long step)",
+                "note": f"dominant kernel by time share; achieved = 4*M*(n+B)*128 FLOP per launch / (step time / {n_steps} launches); "
+                        "traffic = dram__bytes_read+write per launch of the committed ncu capture (profiles/), cold L2"}
+    roofline_scan = {"kernel": "scan_pm_kernel", "bound": "hbm", "achieved": scan_gbs_live, "peak": peaks["hbm_gbs"],
+                     "unit": "GB/s", "frac": scan_gbs_live / peaks["hbm_gbs"], "traffic": NCU_SCAN_DRAM_BYTES.get(w.name),
                      "achieved_alone": scan_gbs_alone, "frac_alone": scan_gbs_alone / peaks["hbm_gbs"],
                      "pct_of_8TBs_alone": 100.0 * scan_gbs_alone / 8000.0, "peak_source": peaks["source"],
                      "note": "live = CUDA events on the retrieval stream inside the timed region (shares HBM/SMs with "
@@ -415,11 +426,14 @@ def main():
         "metric": METRIC, "value": tokens_per_s, "unit": "tokens/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": f"{w.name}: Qwen2.5-7B-shaped layer 28/4/128, batch 8 x 32768 paged (16-token pages), "
-                               f"B=32, T=16 ({n_steps} attention steps), 5% budget k=1639, 0.5% planted keys",
+        "config": {"workload": f"{w.name}: single layer {w.n_q_heads}/{w.n_kv_heads}/128 heads, batch {w.batch} x {w.max_seq_len} "
+                               f"paged (16-token pages), B={w.block_size}, T={w.denoise_steps} ({n_steps} attention steps), "
+                               f"budget {w.permille / 10:g}% k={max(ks)}, structure {w.structure}",
                    "parallelism": "replicas" if world > 1 else "single GPU",
-                   "l2": "K cache 256 MiB > 126 MB L2 (no flush needed); the 27 MB active pool is reused by all 15 steps by design",
-                   "start_after_step": args.start_after_step, "retrieval_sms": int(pipe.c.retrieval_sms),
+                   "l2": f"K cache {tokens * w.n_kv_heads * 256 / 2**20:.0f} MiB > 126 MB L2 (no flush needed); the active pool "
+                         f"({rows * 512 / 1e6:.0f} MB) is reused by all {n_steps} steps by design",
+                   "start_after_step": int(pipe.c.start_after_step), "scan_ctas": int(pipe.c.scan_ctas),
+                   "schedule_sweep_ms (scan_ctas/start_after_step, untimed calibration, eager)": rs_sweep,
                    "attn_grid_ctas": H.herald_attn_grid_ctas(shape),
                    "launch": "eager" if graphs is None else "one CUDA graph per pool parity, replayed"},
         "breakdown": {

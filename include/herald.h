@@ -94,7 +94,7 @@ size_t herald_attn_workspace_bytes(const herald_shape_t* shape);
 
 /* Number of thread blocks (one per SM) herald_sparse_attn launches for this shape: KV splits x M tiles x
  * batch x n_kv_heads.  A caller that overlaps selection with denoising gives the retrieval
- * stream the SMs this leaves free (herald_pipeline_t.retrieval_sms).  Host only; 0 on an invalid shape. */
+ * stream the SMs this leaves free (herald_pipeline_t.scan_ctas).  Host only; 0 on an invalid shape. */
 int32_t herald_attn_grid_ctas(const herald_shape_t* shape);
 
 /* Representative-query selection (Eq.(1)).
@@ -161,10 +161,14 @@ typedef struct herald_pipeline {
     int32_t n_steps;          /* T-1 attention steps per block (reading 13) */
     int32_t start_after_step; /* 0 .. n_steps                                           */
     int32_t active;           /* index of the ACTIVE pool buffer; flipped on success    */
-    int32_t retrieval_sms;    /* SMs the retrieval stream's score scan may occupy (its grid: one block per SM);
-                                 0 = the whole device.  The scan is a long bandwidth-bound kernel: sized to the SMs
-                                 the attention grid leaves free, it streams K beside the denoising steps instead of
-                                 taking their SMs (the paper's "bound by the slower stream")        */
+    int32_t scan_ctas;        /* grid of the retrieval stream's score scan (1024-thread blocks, one per SM; each takes
+                                 1/scan_ctas of the cache); 0 = one block per SM of the device.  The scan is a long
+                                 bandwidth-bound kernel and the attention blocks need whole SMs:
+                                   <= the SMs the attention grid leaves free: the scan streams K beside the denoising
+                                      steps without ever taking their SMs (denoising-bound shapes);
+                                   a multiple of the SM count: short blocks in several waves, time-sliced with the
+                                      attention launches (selection-bound shapes; "bound by the slower
+                                      stream", Fig. 14)                                              */
     herald_layer_t* layers;   /* host array [n_layers]                                  */
     int32_t* sel_idx;         /* int32 [batch][H_kv][pool_capacity] scratch (retrieval stream) */
     void* ws_select;

@@ -88,14 +88,14 @@ static int sm_count() {
     return n;
 }
 
-// SMs the retrieval-stream kernels may occupy (0 = all); set by herald_pipeline_step around its select/gather calls
-static thread_local int g_retrieval_sms = 0;
+// grid of the score scan (0 = one block per SM); set by herald_pipeline_step around its select calls
+static thread_local int g_scan_ctas = 0;
 
-// Grid of the scan = number of SMs it may occupy (one 1024-thread CTA per SM).
+// Grid of the scan: one 1024-thread CTA per SM it may occupy, or several waves of them.
 static int scan_ctas_for(const herald_shape_t* s) {
     (void)s;
     int n = env_int("HERALD_SCAN_CTAS", 0);
-    if (n <= 0) n = g_retrieval_sms > 0 ? g_retrieval_sms : sm_count();
+    if (n <= 0) n = g_scan_ctas > 0 ? g_scan_ctas : sm_count();
     if (n > kScanMaxCtas) n = kScanMaxCtas;
     return n;
 }
@@ -514,7 +514,7 @@ static int check_pipeline(const herald_pipeline_t* p) {
     if (p->n_steps < 0 || p->start_after_step < 0 || p->start_after_step > p->n_steps)
         return fail(HERALD_ERR_INVALID_ARG, "pipeline: bad n_steps / start_after_step");
     if (p->active != 0 && p->active != 1) return fail(HERALD_ERR_INVALID_ARG, "pipeline: active must be 0 or 1");
-    if (p->retrieval_sms < 0) return fail(HERALD_ERR_INVALID_ARG, "pipeline: retrieval_sms must be >= 0");
+    if (p->scan_ctas < 0) return fail(HERALD_ERR_INVALID_ARG, "pipeline: scan_ctas must be >= 0");
     if (!p->sel_idx || !p->ws_select || !p->ws_attn || !p->ev_fork || !p->ev_join)
         return fail(HERALD_ERR_INVALID_ARG, "pipeline: NULL scratch / workspace / event");
     if (p->main_stream == p->retrieval_stream)
@@ -542,11 +542,11 @@ int herald_pipeline_step(herald_pipeline_t* p) {
         for (int l = 0; l < p->n_layers; ++l) {
             herald_layer_t* ly = &p->layers[l];
             g_prof_armed = (l == p->n_layers - 1);
-            g_retrieval_sms = p->retrieval_sms;
+            g_scan_ctas = p->scan_ctas;
             int r = herald_select(sh, &ly->cache, ly->q_rep, ly->k_per_seq, p->sel_idx, ly->pool_len[idle], nullptr,
                                   p->ws_select, p->ws_select_bytes, s_ret);
             g_prof_armed = false;
-            g_retrieval_sms = 0;
+            g_scan_ctas = 0;
             if (r) return r;
             r = herald_gather(sh, &ly->cache, p->sel_idx, ly->pool_len[idle], ly->pool_k[idle], ly->pool_v[idle], s_ret);
             if (r) return r;

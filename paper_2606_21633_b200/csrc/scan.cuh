@@ -17,7 +17,7 @@ namespace herald {
 
 constexpr int kScanThreads = 1024;             // one CTA per SM: 32 warps x 8 x 16-byte loads in flight per lane
 constexpr int kScanWarps = kScanThreads / 32;
-constexpr int kScanMaxCtas = 512;              // bound on the grid (sizes the mode-1 partial statistics)
+constexpr int kScanMaxCtas = 2048;             // bound on the grid (sizes the mode-1 partial statistics)
 
 struct ScanParams {
     const __nv_bfloat16* k_pages;

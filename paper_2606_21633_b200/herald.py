@@ -55,7 +55,7 @@ class Layer(C.Structure):
 
 class Pipeline(C.Structure):
     _fields_ = [("shape", Shape), ("n_layers", C.c_int32), ("n_steps", C.c_int32),
-                ("start_after_step", C.c_int32), ("active", C.c_int32), ("retrieval_sms", C.c_int32),
+                ("start_after_step", C.c_int32), ("active", C.c_int32), ("scan_ctas", C.c_int32),
                 ("layers", C.POINTER(Layer)),
                 ("sel_idx", C.c_void_p), ("ws_select", C.c_void_p), ("ws_select_bytes", C.c_size_t),
                 ("ws_attn", C.c_void_p), ("ws_attn_bytes", C.c_size_t),
@@ -207,7 +207,7 @@ class BlockPipeline:
     """Owns the device buffers of a dual-stream block pipeline (pools, workspaces, streams, events)
     and the ctypes structs that describe them.  Marshalling and memory ownership only."""
 
-    def __init__(self, shape: Shape, layers, n_steps: int, start_after_step: int = 0, device="cuda", retrieval_sms=None):
+    def __init__(self, shape: Shape, layers, n_steps: int, start_after_step: int = 0, device="cuda", scan_ctas=None):
         """layers: list of dicts with torch tensors k_pages, v_pages, page_table, seq_lens, q_rep, k_per_seq,
         q_blk, k_blk, v_blk ([n_steps, ...])."""
         dev = torch.device(device)
@@ -243,11 +243,11 @@ class BlockPipeline:
             self.ev_join.record(self.retrieval_stream)
         p = Pipeline()
         p.shape, p.n_layers, p.n_steps, p.start_after_step, p.active = shape, len(layers), n_steps, start_after_step, 0
-        if retrieval_sms is None:
+        if scan_ctas is None:
             # the score scan takes the SMs the attention grid leaves free (at least 1/8 of the device)
             n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
-            retrieval_sms = max(n_sm - herald_attn_grid_ctas(shape), n_sm // 8)
-        p.retrieval_sms = int(retrieval_sms)
+            scan_ctas = max(n_sm - herald_attn_grid_ctas(shape), n_sm // 8)
+        p.scan_ctas = int(scan_ctas)
         p.layers = C.cast(self.layer_arr, C.POINTER(Layer))
         p.sel_idx = _ptr(self.sel_idx)
         p.ws_select, p.ws_select_bytes = _ptr(self.ws_select), self.ws_select.numel()
@@ -277,6 +277,41 @@ class BlockPipeline:
 
     def step_host(self, io: HostIO):
         herald_pipeline_step_host(self.c, io)
+
+    def tune_schedule(self, candidates=None, reps=4, tune_start=True):
+        """Pick how the retrieval stream shares the device with the denoising steps by timing eager block steps
+        (CUDA events on the main stream) for a few schedules (scan_ctas, start_after_step):
+          * scan grid = the SMs the attention grid leaves free: the scan streams K beside the attention launches
+            (denoising-bound shapes);
+          * scan grid = every SM, started with the block or only after the last denoising step (selection-bound
+            shapes, where both streams are HBM-bound and overlapping them buys nothing: "bound by the
+            slower stream", Fig. 14).
+        Returns {"scan_ctas/start_after_step": ms per step}; leaves the fastest schedule set.  Pool contents stay
+        valid (every step is a complete block step)."""
+        n_sm = torch.cuda.get_device_properties(self.device).multi_processor_count
+        if candidates is None:
+            spare = n_sm - herald_attn_grid_ctas(self.shape)
+            start0 = int(self.c.start_after_step)
+            candidates = [(c, start0) for c in sorted({c for c in (spare - 2, spare, n_sm // 8) if c >= 8})]
+            candidates.append((n_sm, start0))
+            if tune_start and start0 != self.n_steps:
+                candidates.append((n_sm, self.n_steps))
+        table = {}
+        for ctas, start in candidates:
+            self.c.scan_ctas, self.c.start_after_step = int(ctas), int(start)
+            for _ in range(2):
+                self.step()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize(self.device)
+            a.record(self.main_stream)
+            for _ in range(reps):
+                self.step()
+            b.record(self.main_stream)
+            torch.cuda.synchronize(self.device)
+            table[(int(ctas), int(start))] = a.elapsed_time(b) / reps
+        best = min(table, key=table.get)
+        self.c.scan_ctas, self.c.start_after_step = best
+        return {f"{c}/{st}": ms for (c, st), ms in table.items()}
 
     # ---- CUDA graphs: one captured block step per pool parity (launch-bound inner loop, no per-launch host cost) ----
     def capture(self, io: HostIO = None):
