@@ -297,11 +297,6 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     const int i0 = mtile * p.ipt;                            // first block row of this M tile
     const int rows_valid = min(p.ipt, B - i0) * G;           // tile rows that are real queries
     const int rows_box = p.ipt * G;                          // tile rows the Q box writes (zeros past the block)
-    const int n_pool = max(0, min(p.pool_len[unit], p.cap));
-    const int n_tiles = 1 + (n_pool + kTcBN - 1) / kTcBN;    // key tile 0 = the in-block rows, tile t >= 1 = pool rows [128(t-1), 128t)
-    const int per = (n_tiles + S - 1) / S;
-    const int t0 = split * per, t1 = min(n_tiles, t0 + per);
-    const int nt = max(t1 - t0, 0);                          // tile j of this CTA is key tile t0 + j
     const int rows_own = (rows_box + S - 1) / S;             // tile rows merged and written by each CTA of the cluster (zero rows past the box are nobody's)
     const int ml_stride = (rows_own + 1) & ~1;               // float2 per source, padded to 16 bytes
     const int g_inv = (65536 + G - 1) / G;                   // (r * g_inv) >> 16 == r / G for r < 128, G <= 8
@@ -357,6 +352,16 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     tc_fence_after();
     const uint32_t tmem = *tmem_ptr_gen;
     if (tid == 0) HERALD_STAMP(1);
+
+    // Programmatic dependent launch: this grid may have been scheduled while the previous kernel of the stream was
+    // still draining.  Everything above is on-chip; nothing is read from global memory before that kernel has
+    // completed and flushed.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    const int n_pool = max(0, min(p.pool_len[unit], p.cap));
+    const int n_tiles = 1 + (n_pool + kTcBN - 1) / kTcBN;    // key tile 0 = the in-block rows, tile t >= 1 = pool rows [128(t-1), 128t)
+    const int per = (n_tiles + S - 1) / S;
+    const int t0 = split * per, t1 = min(n_tiles, t0 + per);
+    const int nt = max(t1 - t0, 0);                          // tile j of this CTA is key tile t0 + j
 
     auto tile_valid = [&](int j) {  // valid keys of this CTA's j-th tile (>= 1)
         const int t = t0 + j;
@@ -567,6 +572,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     // The V ring of this CTA is dead once its softmax warps have seen the last PV complete (every MMA and every TMA
     // write of the CTA is then done): it stages what this CTA sends and the rows it writes out.  The K ring receives
     // the other CTAs' partial rows, so nothing is sent before the cluster barrier that every CTA passes after its main loop.
+    // the next kernel of the stream may be scheduled from here on: its blocks take the SMs as this grid's blocks exit
+    asm volatile("griddepcontrol.launch_dependents;");
     const int owner = row / rows_own, row_l = row - owner * rows_own;
     const int push_ml_off = kTcPushO + (S - 1) * rows_own * kTcRowFloats * 4;
     const int stage_off = push_ml_off + (S - 1) * ml_stride * 8;

@@ -494,13 +494,24 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
     cfg.blockDim = dim3(kTcThreads);
     cfg.dynamicSmemBytes = kTcSmemBytes;
     cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = a.n_splits;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
+    cudaLaunchAttribute attr[2];
+    int n_attr = 0;
+    if (a.n_splits > 1) {
+        attr[n_attr].id = cudaLaunchAttributeClusterDimension;
+        attr[n_attr].val.clusterDim.x = a.n_splits;
+        attr[n_attr].val.clusterDim.y = 1;
+        attr[n_attr].val.clusterDim.z = 1;
+        ++n_attr;
+    }
+    if (env_int("HERALD_ATTN_PDL", 1)) {
+        // consecutive denoising steps: the next grid is scheduled while this one runs its merge and takes each SM as
+        // it is released (the kernel itself waits, griddepcontrol.wait, before its first global read)
+        attr[n_attr].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[n_attr].val.programmaticStreamSerializationAllowed = 1;
+        ++n_attr;
+    }
     cfg.attrs = attr;
-    cfg.numAttrs = a.n_splits > 1 ? 1 : 0;
+    cfg.numAttrs = n_attr;
     cudaError_t e = cudaLaunchKernelEx(&cfg, attn_tc_kernel, *tm_k, *tm_v, *tm_q, *tm_kb, *tm_vb, ap);
     if (e != cudaSuccess) return cuda_fail(e, "attention launch");
     return HERALD_OK;
