@@ -222,6 +222,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="herald", choices=["herald", "reference"])
     ap.add_argument("--workload", default=WORKLOAD)
+    ap.add_argument("--layers", type=int, default=None, help="layers of the stack (default: the workload's; C5 has 28)")
     ap.add_argument("--start-after-step", type=int, default=None,
                     help="denoising steps before the retrieval stream starts (default: 0 or T-1, calibrated)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -242,16 +243,29 @@ def main():
     peaks = load_peaks()
 
     w = synth.config(args.workload)
-    inp = synth.make_inputs(w, SEED + rank, dev)
     ks = [H.herald_budget_rows(L, w.permille) for L in w.seq_lens]
     cap = max(ks) + w.block_size
     n_steps = w.n_attn_steps
+    # layers of the stack (C5): every layer has its own cache, q_rep, block inputs, pools and outputs; keep what fits
+    n_layers = args.layers or w.n_layers
+    if n_layers > 1:
+        pages = sum((L + 15) // 16 for L in w.seq_lens)
+        per_layer = (pages * 16 * w.n_kv_heads * 256 * 2 + 4 * w.batch * w.n_kv_heads * cap * 256
+                     + n_steps * w.batch * w.block_size * (w.n_q_heads * (512 + 256) + w.n_kv_heads * 512))
+        free_b, _ = torch.cuda.mem_get_info(dev)
+        fit = int((free_b * 0.92 - 3e9) // per_layer)
+        if fit < n_layers:
+            print(f"bench.py: {n_layers} layers need {n_layers * per_layer / 1e9:.0f} GB, {free_b / 1e9:.0f} GB are free: "
+                  f"running {max(fit, 1)} layers", file=sys.stderr)
+            n_layers = max(fit, 1)
+    inps = [synth.make_inputs(w, SEED + rank + 97 * l, dev) for l in range(n_layers)]
+    inp = inps[0]
     shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, (w.max_seq_len + 15) // 16 * 16,
                          inp["page_table"].shape[1], cap)
     k_per_seq = torch.tensor(ks, dtype=torch.int32, device=dev)
-    layer = dict(k_pages=inp["k_pages"], v_pages=inp["v_pages"], page_table=inp["page_table"], seq_lens=inp["seq_lens"],
-                 q_rep=inp["q_rep"], k_per_seq=k_per_seq, q_blk=inp["q_blk"], k_blk=inp["k_blk"], v_blk=inp["v_blk"])
-    pipe = H.BlockPipeline(shape, [layer], n_steps, args.start_after_step or 0, dev, scan_ctas=args.scan_ctas)
+    layers = [dict(k_pages=x["k_pages"], v_pages=x["v_pages"], page_table=x["page_table"], seq_lens=x["seq_lens"],
+                   q_rep=x["q_rep"], k_per_seq=k_per_seq, q_blk=x["q_blk"], k_blk=x["k_blk"], v_blk=x["v_blk"]) for x in inps]
+    pipe = H.BlockPipeline(shape, layers, n_steps, args.start_after_step or 0, dev, scan_ctas=args.scan_ctas)
     units = w.batch * w.n_kv_heads
     G, M = w.group, w.block_size * w.group
 
@@ -356,6 +370,12 @@ def main():
     act = pipe.active
     out1 = torch.empty((w.batch, w.block_size, w.n_q_heads, 128), dtype=torch.float32, device=dev)
     select_alone_ms = time_isolated(lambda: H.herald_select(shape, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, None, ws_sel, side))
+    # the paper's aggregation (softmax-normalised sum over the group; reading 1) beside the north-star one
+    shape_m1 = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, shape.max_seq_len, shape.max_pages_per_seq, cap,
+                            agg_mode=H.AGG_SOFTMAX_SUM)
+    ws_sel_m1 = H.alloc_workspace(H.herald_select_workspace_bytes(shape_m1), dev)
+    select_mode1_alone_ms = time_isolated(lambda: H.herald_select(shape_m1, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, None, ws_sel_m1, side))
+    del ws_sel_m1
     gather_alone_ms = time_isolated(lambda: H.herald_gather(shape, cache, sel_idx, sel_cnt, pipe.pools_k[0][1 - act], pipe.pools_v[0][1 - act], side))
     step_i = [0]
 
@@ -369,30 +389,36 @@ def main():
     # time select with k=0 (top-k exits immediately): scan + histogram + launch of an empty top-k
     k_zero = torch.zeros_like(k_per_seq)
     scan_alone_ms = time_isolated(lambda: H.herald_select(shape, cache, inp["q_rep"], k_zero, sel_idx, sel_cnt, None, ws_sel, side))
-    denoise_alone_ms = attn_alone_ms * n_steps
+    denoise_alone_ms = attn_alone_ms * n_steps * n_layers        # stage timings are per layer (layer 0), the block has n_layers
+    select_alone_ms, select_mode1_alone_ms = select_alone_ms * n_layers, select_mode1_alone_ms * n_layers
+    gather_alone_ms_block = gather_alone_ms * n_layers
 
     # ---- end to end through the host-buffer entry point ----
-    host = {n: inp[n].cpu().pin_memory() for n in ("q_rep", "q_blk", "k_blk", "v_blk")}
-    host["out"] = torch.empty(pipe.outs[0].shape, dtype=torch.float32).pin_memory()
-    io = pipe.make_host_io([host])
-    h2d = sum(host[n].numel() * host[n].element_size() for n in ("q_rep", "q_blk", "k_blk", "v_blk"))
-    d2h = host["out"].numel() * 4
-    for _ in range(3):
+    hosts = []
+    for l in range(n_layers):
+        host = {n: inps[l][n].cpu().pin_memory() for n in ("q_rep", "q_blk", "k_blk", "v_blk")}
+        host["out"] = torch.empty(pipe.outs[l].shape, dtype=torch.float32).pin_memory()
+        hosts.append(host)
+    io = pipe.make_host_io(hosts)
+    h2d = sum(h[n].numel() * h[n].element_size() for h in hosts for n in ("q_rep", "q_blk", "k_blk", "v_blk"))
+    d2h = sum(h["out"].numel() * 4 for h in hosts)
+    e2e_steps = args.steps if n_layers == 1 else min(args.steps, 3)
+    for _ in range(3 if n_layers == 1 else 1):
         pipe.step_host(io)
     torch.cuda.synchronize()
     barrier()
     a, b = ev(), ev()
     a.record(pipe.main_stream)
-    for _ in range(args.steps):
+    for _ in range(e2e_steps):
         pipe.step_host(io)
     b.record(pipe.main_stream)
     torch.cuda.synchronize()
-    e2e_ms = max_over_ranks(a.elapsed_time(b), dev) / args.steps
+    e2e_ms = max_over_ranks(a.elapsed_time(b), dev) / e2e_steps
     e2e_tokens = world * w.batch * w.block_size / (e2e_ms * 1e-3)
 
     # ---- oracle on the host cores (rank 0, N=1 only) ----
     cpu_baseline = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and n_layers == 1:
         from oracle import herald_oracle as O
         assert ks == [O.budget_rows(L, w.permille) for L in w.seq_lens]
         n_seq = 1
@@ -403,12 +429,12 @@ def main():
         return 0
 
     attn_tflops_step = attn_flops / (attn_alone_ms * 1e-3) / 1e12
-    attn_share = denoise_alone_ms / (denoise_alone_ms + select_alone_ms + gather_alone_ms)
+    attn_share = denoise_alone_ms / (denoise_alone_ms + select_alone_ms + gather_alone_ms_block)
     scan_gbs_live = scan_bytes / (scan_ms * 1e-3) / 1e9
     scan_gbs_alone = scan_bytes / (scan_alone_ms * 1e-3) / 1e9
     # attention inside the step: the main stream runs nothing else, so its per-launch time inside the timed
     # region is (step time) / n_steps when the retrieval stream is hidden
-    attn_live_ms = ms_step / n_steps
+    attn_live_ms = ms_step / (n_steps * n_layers)
     attn_tflops_live = attn_flops / (attn_live_ms * 1e-3) / 1e12
     roofline = {"kernel": "attn_tc_kernel", "bound": "tensor", "achieved": attn_tflops_live,
                 "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s", "frac": attn_tflops_live / peaks["bf16_tflops_sustained"],
@@ -426,7 +452,8 @@ def main():
         "metric": METRIC, "value": tokens_per_s, "unit": "tokens/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": f"{w.name}: single layer {w.n_q_heads}/{w.n_kv_heads}/128 heads, batch {w.batch} x {w.max_seq_len} "
+        "config": {"workload": f"{w.name}: {n_layers} layer(s) {w.n_q_heads}/{w.n_kv_heads}/128 heads, batch {w.batch} x "
+                               f"{'ragged ' + str(min(w.seq_lens)) + '..' + str(w.max_seq_len) if len(set(w.seq_lens)) > 1 else w.max_seq_len} "
                                f"paged (16-token pages), B={w.block_size}, T={w.denoise_steps} ({n_steps} attention steps), "
                                f"budget {w.permille / 10:g}% k={max(ks)}, structure {w.structure}",
                    "parallelism": "replicas" if world > 1 else "single GPU",
@@ -439,19 +466,21 @@ def main():
         "breakdown": {
             "scan_gbs_alone": scan_gbs_alone, "scan_pct_of_8TBs_alone": 100.0 * scan_gbs_alone / 8000.0,
             "scan_gbs_in_pipeline": scan_gbs_live, "scan_ms_in_pipeline": scan_ms, "topk_ms_in_pipeline": topk_ms,
-            "gather_ms_in_pipeline": gather_ms, "select_alone_ms": select_alone_ms, "scan_alone_ms": scan_alone_ms,
+            "gather_ms_in_pipeline": gather_ms, "select_alone_ms": select_alone_ms, "select_softmax_sum_mode_alone_ms": select_mode1_alone_ms,
+            "scan_alone_ms": scan_alone_ms,
             "gather_alone_ms": gather_alone_ms, "gather_gbs_alone": gather_bytes / (gather_alone_ms * 1e-3) / 1e9,
             "attn_step_alone_ms": attn_alone_ms, "attn_tflops_alone": attn_tflops_step,
             "attn_tflops_in_pipeline": attn_tflops_live, "denoise_alone_ms": denoise_alone_ms,
             "block_latency_ms": ms_step, "exposed_selection_ms": ms_step - denoise_alone_ms,
-            "overlap_efficiency": (denoise_alone_ms + select_alone_ms + gather_alone_ms - ms_step) / (select_alone_ms + gather_alone_ms),
+            "overlap_efficiency": (denoise_alone_ms + select_alone_ms + gather_alone_ms_block - ms_step) / (select_alone_ms + gather_alone_ms_block),
+            "n_layers": n_layers,
             "attn_time_share_alone": attn_share,
             "algorithmic": {"scan_bytes": scan_bytes, "gather_bytes": gather_bytes, "attn_flops_per_step": attn_flops,
                             "attn_bytes_per_step": attn_bytes}},
         "roofline": roofline, "roofline_scan": roofline_scan,
         "cpu_baseline": cpu_baseline,
         "e2e": {"value": e2e_tokens, "unit": "tokens/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-        "gpu_launches": args.steps * (3 + n_steps),   # per block step: scan, top-k, gather, T-1 x attention (timed region only)
+        "gpu_launches": args.steps * n_layers * (3 + n_steps),   # per block step: scan, top-k, gather, T-1 x attention (timed region only)
         "clocks": clock_info,
     }
     print(json.dumps(line))

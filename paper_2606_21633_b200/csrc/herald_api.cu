@@ -168,8 +168,9 @@ static EncodeTiledFn encode_tiled_fn() {
     return fn;
 }
 
-// Encoding a tensor map costs about a microsecond of host time and the same few maps come back every denoising
-// step, so the last encodings are kept per thread, keyed by (base pointer, extents).
+// Encoding a tensor map costs about a microsecond of host time and the same maps come back every denoising step
+// (5 per launch, ~50 per layer and block), so encodings are kept per thread in a small hash table keyed by
+// (base pointer, extents).  Callers copy the map out at once: a later insertion may evict any slot.
 struct MapKey {
     const void* ptr;
     int32_t d[4];
@@ -180,35 +181,49 @@ struct MapSlot {
     CUtensorMap map;
     bool used;
 };
-constexpr int kMapSlots = 64;
+constexpr int kMapSlots = 4096;      // power of two
+constexpr int kMapProbe = 8;
 static thread_local MapSlot g_maps[kMapSlots];
-static thread_local int g_map_next = 0;
 
-static const CUtensorMap* cached_map(const MapKey& key) {
-    for (int i = 0; i < kMapSlots; ++i)
-        if (g_maps[i].used && g_maps[i].key == key) return &g_maps[i].map;
-    return nullptr;
+static uint32_t map_hash(const MapKey& k) {
+    uint64_t h = reinterpret_cast<uintptr_t>(k.ptr) * 0x9E3779B97F4A7C15ull;
+    h ^= (uint64_t)(uint32_t)k.d[3] * 0xC2B2AE3D27D4EB4Full + (uint64_t)(uint32_t)k.d[0] * 31u + (uint32_t)k.d[1];
+    return (uint32_t)(h >> 40) & (kMapSlots - 1);
 }
-static CUtensorMap* new_map_slot(const MapKey& key) {
-    MapSlot* s = &g_maps[g_map_next];
-    g_map_next = (g_map_next + 1) % kMapSlots;
+static bool cached_map(const MapKey& key, CUtensorMap* out) {
+    const uint32_t h = map_hash(key);
+    for (int i = 0; i < kMapProbe; ++i) {
+        const MapSlot& s = g_maps[(h + i) & (kMapSlots - 1)];
+        if (s.used && s.key == key) {
+            *out = s.map;
+            return true;
+        }
+    }
+    return false;
+}
+static void store_map(const MapKey& key, const CUtensorMap& map) {
+    const uint32_t h = map_hash(key);
+    MapSlot* s = &g_maps[h];                      // full neighbourhood: evict the home slot
+    for (int i = 0; i < kMapProbe; ++i) {
+        MapSlot* c = &g_maps[(h + i) & (kMapSlots - 1)];
+        if (!c->used) {
+            s = c;
+            break;
+        }
+    }
     s->key = key;
-    s->used = false;   // set by the caller once the encode succeeded
-    return &s->map;
-}
-static void commit_map_slot(const CUtensorMap* m) {
-    for (int i = 0; i < kMapSlots; ++i)
-        if (&g_maps[i].map == m) g_maps[i].used = true;
+    s->map = map;
+    s->used = true;
 }
 
 // bf16 pool [units][cap][128] as a 3-D tensor (d, row, unit); box = 64 channels x 128 rows, 128-byte swizzle:
 // the box lands in shared memory exactly in the UMMA canonical layout (K-major for K, MN-major for V).
-static int make_pool_map(const CUtensorMap** out, const void* pool, int units, int cap) {
+static int make_pool_map(CUtensorMap* out, const void* pool, int units, int cap) {
     const MapKey key{pool, {units, cap, 0, 3}};
-    if ((*out = cached_map(key)) != nullptr) return HERALD_OK;
+    if (cached_map(key, out)) return HERALD_OK;
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
-    CUtensorMap* map = new_map_slot(key);
+    CUtensorMap* map = out;
     const cuuint64_t rows = cap > 0 ? cap : 1;
     const cuuint64_t dims[3] = {(cuuint64_t)kHeadDim, rows, (cuuint64_t)units};
     const cuuint64_t strides[2] = {(cuuint64_t)kRowBytes, rows * kRowBytes};
@@ -218,8 +233,7 @@ static int make_pool_map(const CUtensorMap** out, const void* pool, int units, i
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled(pool) failed with CUresult %d", (int)r);
-    commit_map_slot(map);
-    *out = map;
+    store_map(key, *map);
     return HERALD_OK;
 }
 
@@ -227,12 +241,12 @@ static int make_pool_map(const CUtensorMap** out, const void* pool, int units, i
 // block rows: one box is one half of the Q tile of an (unit, M tile), rows ordered (block row, head), zero-filled past B.
 // bf16 k_blk / v_blk [batch][B][H_kv][128] as a 4-D tensor (d, head, block row, sequence); box = 64 channels x 1 head x
 // B block rows: one half of the in-block key tile of a unit.
-static int make_blk_map(const CUtensorMap** out, const void* blk, const herald_shape_t* s) {
+static int make_blk_map(CUtensorMap* out, const void* blk, const herald_shape_t* s) {
     const MapKey key{blk, {s->batch, s->block_size, s->n_kv_heads, 5}};
-    if ((*out = cached_map(key)) != nullptr) return HERALD_OK;
+    if (cached_map(key, out)) return HERALD_OK;
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
-    CUtensorMap* map = new_map_slot(key);
+    CUtensorMap* map = out;
     const cuuint64_t dims[4] = {(cuuint64_t)kHeadDim, (cuuint64_t)s->n_kv_heads, (cuuint64_t)s->block_size, (cuuint64_t)s->batch};
     const cuuint64_t strides[3] = {(cuuint64_t)kRowBytes, (cuuint64_t)s->n_kv_heads * kRowBytes,
                                    (cuuint64_t)s->block_size * s->n_kv_heads * kRowBytes};
@@ -242,17 +256,16 @@ static int make_blk_map(const CUtensorMap** out, const void* blk, const herald_s
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled(k_blk/v_blk) failed with CUresult %d", (int)r);
-    commit_map_slot(map);
-    *out = map;
+    store_map(key, *map);
     return HERALD_OK;
 }
 
-static int make_q_map(const CUtensorMap** out, const void* q_blk, const herald_shape_t* s, int ipt) {
+static int make_q_map(CUtensorMap* out, const void* q_blk, const herald_shape_t* s, int ipt) {
     const MapKey key{q_blk, {s->batch, s->block_size, s->n_q_heads, 4 | (ipt << 8) | (s->n_kv_heads << 16)}};
-    if ((*out = cached_map(key)) != nullptr) return HERALD_OK;
+    if (cached_map(key, out)) return HERALD_OK;
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
-    CUtensorMap* map = new_map_slot(key);
+    CUtensorMap* map = out;
     const int G = s->n_q_heads / s->n_kv_heads;
     const cuuint64_t dims[4] = {(cuuint64_t)kHeadDim, (cuuint64_t)s->n_q_heads, (cuuint64_t)s->block_size, (cuuint64_t)s->batch};
     const cuuint64_t strides[3] = {(cuuint64_t)kRowBytes, (cuuint64_t)s->n_q_heads * kRowBytes,
@@ -263,8 +276,7 @@ static int make_q_map(const CUtensorMap** out, const void* q_blk, const herald_s
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled(q_blk) failed with CUresult %d", (int)r);
-    commit_map_slot(map);
-    *out = map;
+    store_map(key, *map);
     return HERALD_OK;
 }
 
@@ -462,7 +474,7 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(attn)");
         attr_set = true;
     }
-    const CUtensorMap *tm_k, *tm_v, *tm_q, *tm_kb, *tm_vb;
+    CUtensorMap tm_k, tm_v, tm_q, tm_kb, tm_vb;
     rc = make_pool_map(&tm_k, pool_k, units, shape->pool_capacity);
     if (rc) return rc;
     rc = make_pool_map(&tm_v, pool_v, units, shape->pool_capacity);
@@ -512,7 +524,7 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
     }
     cfg.attrs = attr;
     cfg.numAttrs = n_attr;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, attn_tc_kernel, *tm_k, *tm_v, *tm_q, *tm_kb, *tm_vb, ap);
+    cudaError_t e = cudaLaunchKernelEx(&cfg, attn_tc_kernel, tm_k, tm_v, tm_q, tm_kb, tm_vb, ap);
     if (e != cudaSuccess) return cuda_fail(e, "attention launch");
     return HERALD_OK;
 }

@@ -56,7 +56,7 @@ class Workload:
 
 
 def config(name: str) -> Workload:
-    """BASELINE.json ``configs`` C1..C4 (C5, the 28-layer ragged stack, is a later round)."""
+    """BASELINE.json ``configs`` C1..C5 (one layer's inputs per make_inputs call; C5 draws one set per layer)."""
     if name == "C1":   # single layer, 1 sequence, L=4096, 4/1 heads, B=16, T=8, 5 %, 32 planted keys
         return Workload("C1", 1, (4096,), 4, 1, 16, 8, 50, "planted", 32, identity_pages=True)
     if name == "C2":   # Qwen2.5-7B-shaped layer: 28/4, batch 8 x 32768, B=32, T=16, 5 %, 0.5 % planted
@@ -66,6 +66,12 @@ def config(name: str) -> Workload:
     if name.startswith("C4"):  # Qwen3-8B-shaped: 32/8, batch 16 x 65536, B=16, T=8, budgets 2.5/5/10 %
         permille = {"C4": 50, "C4@2.5": 25, "C4@5": 50, "C4@10": 100}[name]
         return Workload(name, 16, (65536,) * 16, 32, 8, 16, 8, permille, "zipf")
+    if name.startswith("C5"):  # 28-layer stack (28/4/128), batch 32, ragged contexts U{8192..131072}, B=32, T=16, 5 %
+        n_layers = int(name[3:]) if name.startswith("C5x") else 28      # "C5x4" = the same stack cut to 4 layers
+        gen = torch.Generator(device="cpu")
+        gen.manual_seed(21633 + 5006)          # fixed draw: mean context 66.8 K tokens, 4.3 GB of K+V per layer
+        lens = torch.randint(8192, 131073, (32,), generator=gen)
+        return Workload(name, 32, tuple(int(x) for x in lens), 28, 4, 32, 16, 50, "plain", n_layers=n_layers)
     raise KeyError(name)
 
 

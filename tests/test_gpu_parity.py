@@ -347,6 +347,7 @@ FULL_CASES = {
     "C2": ("C2", (0, 7), (0, 14)),
     "C3": ("C3", (1,), (0,)),
     "C4@5": ("C4@5", (3,), (6,)),
+    "C5x2": ("C5x2", (26, 14), (9,)),     # two layers of the ragged 28-layer stack (contexts 9574..128375)
 }
 
 
@@ -354,11 +355,14 @@ FULL_CASES = {
 def test_full_size_block_step_sampled(H, cuda, case):
     name, seqs, steps = FULL_CASES[case]
     w = synth.config(name)
-    inp = synth.make_inputs(w, seed=21633 + 1000 * int(name[1]), device=cuda)
+    inps = [synth.make_inputs(w, seed=21633 + 1000 * int(name[1]) + 97 * l, device=cuda) for l in range(w.n_layers)]
+    lc = w.n_layers - 1               # the layer the oracle checks
+    inp = inps[lc]
     ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
     cap = max(ks) + w.block_size
-    shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, w.max_seq_len, inp["page_table"].shape[1], cap)
-    pipe = H.BlockPipeline(shape, [_layer_inputs(w, inp, ks, cuda)], w.n_attn_steps, 0, cuda)
+    shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, (w.max_seq_len + 15) // 16 * 16,
+                         inp["page_table"].shape[1], cap)
+    pipe = H.BlockPipeline(shape, [_layer_inputs(w, x, ks, cuda) for x in inps], w.n_attn_steps, 0, cuda)
     pipe.step()                       # block 0 (eager): attention over the empty pool, selection for block 1
     graphs = pipe.capture()           # the configuration bench.py times: one CUDA graph per pool parity
     pipe.replay(graphs)               # block 1: attention over the selected pool, selection again (same q_rep)
@@ -366,7 +370,7 @@ def test_full_size_block_step_sampled(H, cuda, case):
     assert pipe.active == 0
     G, Hkv = w.group, w.n_kv_heads
     pt = inp["page_table"].cpu().numpy()
-    outs = pipe.outs[0]
+    outs = pipe.outs[lc]
     differing = 0
     for b in seqs:
         L = w.seq_lens[b]
@@ -378,9 +382,9 @@ def test_full_size_block_step_sampled(H, cuda, case):
         sel_o, sc_o = O.select(synth.to_u16(inp["q_rep"][b:b + 1]), kp, ident, np.array([L]), [ks[b]], Hkv, 128 ** -0.5)
         pk_o, pv_o, pl_o = O.gather(kp, vp, ident, sel_o, cap)
         for buf in (0, 1):            # both selections used the same q_rep: both pools hold the same rows
-            pl = pipe.pool_lens[0][buf][b].cpu().numpy()
+            pl = pipe.pool_lens[lc][buf][b].cpu().numpy()
             assert np.array_equal(pl, pl_o[0])
-        pk_g, pv_g = synth.to_u16(pipe.pools_k[0][1][b]), synth.to_u16(pipe.pools_v[0][1][b])
+        pk_g, pv_g = synth.to_u16(pipe.pools_k[lc][1][b]), synth.to_u16(pipe.pools_v[lc][1][b])
         for h in range(Hkv):
             n = ks[b]
             if np.array_equal(pk_g[h, :n], pk_o[0, h, :n]) and np.array_equal(pv_g[h, :n], pv_o[0, h, :n]):
@@ -394,8 +398,8 @@ def test_full_size_block_step_sampled(H, cuda, case):
             check_selection(got, n, sc_o[0][h], ks[b], L, f"{case} b{b} h{h}")
             assert np.array_equal(pv_g[h, :n], O.cached_rows(vp, ident, 0, L, h)[got])
         for s in steps:
-            pool_k = synth.to_u16(pipe.pools_k[0][1][b:b + 1])
-            pool_v = synth.to_u16(pipe.pools_v[0][1][b:b + 1])
+            pool_k = synth.to_u16(pipe.pools_k[lc][1][b:b + 1])
+            pool_v = synth.to_u16(pipe.pools_v[lc][1][b:b + 1])
             ref, _ = O.sparse_attn(synth.to_u16(inp["q_blk"][s, b:b + 1]), synth.to_u16(inp["k_blk"][s, b:b + 1]),
                                    synth.to_u16(inp["v_blk"][s, b:b + 1]), pool_k, pool_v, pl_o, 128 ** -0.5)
             err = np.abs(outs[s, b:b + 1].cpu().numpy() - ref).max()
