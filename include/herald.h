@@ -173,8 +173,8 @@ typedef struct herald_pipeline {
     int32_t* sel_idx;         /* int32 [batch][H_kv][pool_capacity] scratch (retrieval stream) */
     void* ws_select;
     size_t ws_select_bytes;
-    void* ws_attn;
-    size_t ws_attn_bytes;
+    void* ws_attn;            /* >= herald_attn_workspace_bytes(); with n_layers times that, a multi-wave attention grid over   */
+    size_t ws_attn_bytes;     /* ragged pools is dispatched longest pool first (one slice per layer holds the unit order)      */
     herald_stream_t main_stream;
     herald_stream_t retrieval_stream;
     herald_event_t ev_fork; /* recorded on the main stream, waited on by the retrieval stream */

@@ -90,6 +90,7 @@ static_assert(kTcMiscMax + 2 * 4 * 128 * 2 <= kTcMiscBytes, "exchange buffer ove
 
 struct AttnParams {
     const int32_t* pool_len;
+    const int32_t* unit_order;   // optional [units]: units by decreasing pool length (attn_plan_kernel); NULL = identity
     float* out;
     float* lse;
     int32_t n_q_heads, n_kv_heads, block_size, cap, n_splits;
@@ -290,9 +291,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     uint8_t* sgen = smem_raw;
     if (sbase & 1023u) __trap();   // the 128B-swizzled tiles need a 1024 B aligned base
 
-    const int split = blockIdx.x, mtile = blockIdx.y, unit = blockIdx.z;   // split == rank of this CTA in its cluster
+    const int split = blockIdx.x, mtile = blockIdx.y;        // split == rank of this CTA in its cluster
     const int S = p.n_splits;
-    const int b = unit / p.n_kv_heads, h = unit % p.n_kv_heads;
     const int G = p.n_q_heads / p.n_kv_heads, B = p.block_size;
     const int i0 = mtile * p.ipt;                            // first block row of this M tile
     const int rows_valid = min(p.ipt, B - i0) * G;           // tile rows that are real queries
@@ -357,6 +357,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     // still draining.  Everything above is on-chip; nothing is read from global memory before that kernel has
     // completed and flushed.
     asm volatile("griddepcontrol.wait;" ::: "memory");
+    // blocks are dispatched in blockIdx order: with a plan (attn_plan_kernel) slot z holds the unit with the z-th longest
+    // pool, so that the long units start first and the short ones fill the tail of a multi-wave grid
+    const int unit = p.unit_order ? p.unit_order[blockIdx.z] : (int)blockIdx.z;
+    const int b = unit / p.n_kv_heads, h = unit % p.n_kv_heads;
     const int n_pool = max(0, min(p.pool_len[unit], p.cap));
     const int n_tiles = 1 + (n_pool + kTcBN - 1) / kTcBN;    // key tile 0 = the in-block rows, tile t >= 1 = pool rows [128(t-1), 128t)
     const int per = (n_tiles + S - 1) / S;
@@ -676,6 +680,20 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     if (warp == kTcMmaWarp) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(kTcTmemCols));
+    }
+}
+
+// Longest-pool-first order of the units for a ragged batch: order[rank] = unit, rank by (pool_len descending, unit ascending).
+// One block; O(units^2 / threads) comparisons, units is a few hundred.
+__global__ void __launch_bounds__(1024) attn_plan_kernel(const int32_t* __restrict__ pool_len, int cap, int units, int32_t* __restrict__ order) {
+    for (int i = threadIdx.x; i < units; i += blockDim.x) {
+        const int li = max(0, min(pool_len[i], cap));
+        int rank = 0;
+        for (int j = 0; j < units; ++j) {
+            const int lj = max(0, min(pool_len[j], cap));
+            rank += (lj > li) || (lj == li && j < i);
+        }
+        order[rank] = i;
     }
 }
 

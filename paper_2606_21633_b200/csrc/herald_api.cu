@@ -145,7 +145,8 @@ static AttnGeom attn_geom(const herald_shape_t* s) {
     if (splits > kTcMaxSplits) splits = kTcMaxSplits;
     if (splits < 1) splits = 1;
     a.n_splits = splits;
-    a.total = 256;   // split-KV partials are merged on chip (DSMEM): the workspace is reserved, not used
+    // split-KV partials are merged on chip (DSMEM); the workspace only holds the longest-first unit order of a layer
+    a.total = align_up((size_t)(units > 0 ? units : 1) * sizeof(int32_t), 256);
     return a;
 }
 
@@ -451,9 +452,9 @@ int herald_gather(const herald_shape_t* shape, const herald_cache_t* cache, cons
     return HERALD_OK;
 }
 
-int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const void* pool_v, const int32_t* pool_len,
-                       const void* q_blk, const void* k_blk, const void* v_blk, float* out, float* lse, void* ws,
-                       size_t ws_bytes, herald_stream_t stream_) {
+static int sparse_attn_impl(const herald_shape_t* shape, const void* pool_k, const void* pool_v, const int32_t* pool_len,
+                            const void* q_blk, const void* k_blk, const void* v_blk, float* out, float* lse, void* ws,
+                            size_t ws_bytes, herald_stream_t stream_, const int32_t* unit_order) {
     int rc = check_shape(shape);
     if (rc) return rc;
     if (!pool_k || !pool_v || !pool_len || !q_blk || !k_blk || !v_blk || !out || !ws)
@@ -487,6 +488,7 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
     if (rc) return rc;
     AttnParams ap{};
     ap.pool_len = pool_len;
+    ap.unit_order = unit_order;
     ap.out = out;
     ap.lse = lse;
     ap.n_q_heads = shape->n_q_heads;
@@ -526,6 +528,22 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
     cfg.numAttrs = n_attr;
     cudaError_t e = cudaLaunchKernelEx(&cfg, attn_tc_kernel, tm_k, tm_v, tm_q, tm_kb, tm_vb, ap);
     if (e != cudaSuccess) return cuda_fail(e, "attention launch");
+    return HERALD_OK;
+}
+
+int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const void* pool_v, const int32_t* pool_len,
+                       const void* q_blk, const void* k_blk, const void* v_blk, float* out, float* lse, void* ws,
+                       size_t ws_bytes, herald_stream_t stream_) {
+    return sparse_attn_impl(shape, pool_k, pool_v, pool_len, q_blk, k_blk, v_blk, out, lse, ws, ws_bytes, stream_, nullptr);
+}
+
+// Longest-pool-first unit order of one layer into `order` (device, [units]); enqueued on `stream`.
+static int attn_plan(const herald_shape_t* shape, const int32_t* pool_len, int32_t* order, cudaStream_t stream) {
+    const int units = shape->batch * shape->n_kv_heads;
+    if (units == 0) return HERALD_OK;
+    attn_plan_kernel<<<1, 1024, 0, stream>>>(pool_len, shape->pool_capacity, units, order);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "attention plan launch");
     return HERALD_OK;
 }
 
@@ -581,6 +599,16 @@ int herald_pipeline_step(herald_pipeline_t* p) {
         return HERALD_OK;
     };
 
+    // A multi-wave attention grid (more blocks than SMs) over ragged pools is dispatched longest pool first: one tiny plan
+    // kernel per layer and block writes the unit order into that layer's slice of the attention workspace.
+    const size_t ws_layer = attn_geom(sh).total;
+    const bool planned = herald_attn_grid_ctas(sh) > sm_count() && p->ws_attn_bytes >= ws_layer * (size_t)p->n_layers && p->n_steps > 0;
+    if (planned) {
+        for (int l = 0; l < p->n_layers; ++l) {
+            rc = attn_plan(sh, p->layers[l].pool_len[act], reinterpret_cast<int32_t*>(static_cast<uint8_t*>(p->ws_attn) + ws_layer * l), s_main);
+            if (rc) return rc;
+        }
+    }
     bool forked = false;
     for (int s = 0; s <= p->n_steps; ++s) {
         if (s == p->start_after_step && !forked) {
@@ -591,11 +619,12 @@ int herald_pipeline_step(herald_pipeline_t* p) {
         if (s == p->n_steps) break;
         for (int l = 0; l < p->n_layers; ++l) {
             herald_layer_t* ly = &p->layers[l];
-            rc = herald_sparse_attn(sh, ly->pool_k[act], ly->pool_v[act], ly->pool_len[act],
-                                    static_cast<const __nv_bfloat16*>(ly->q_blk) + s * q_step,
-                                    static_cast<const __nv_bfloat16*>(ly->k_blk) + s * kv_step,
-                                    static_cast<const __nv_bfloat16*>(ly->v_blk) + s * kv_step,
-                                    ly->out + s * q_step, nullptr, p->ws_attn, p->ws_attn_bytes, s_main);
+            rc = sparse_attn_impl(sh, ly->pool_k[act], ly->pool_v[act], ly->pool_len[act],
+                                  static_cast<const __nv_bfloat16*>(ly->q_blk) + s * q_step,
+                                  static_cast<const __nv_bfloat16*>(ly->k_blk) + s * kv_step,
+                                  static_cast<const __nv_bfloat16*>(ly->v_blk) + s * kv_step,
+                                  ly->out + s * q_step, nullptr, p->ws_attn, p->ws_attn_bytes, s_main,
+                                  planned ? reinterpret_cast<const int32_t*>(static_cast<const uint8_t*>(p->ws_attn) + ws_layer * l) : nullptr);
             if (rc) return rc;
         }
     }

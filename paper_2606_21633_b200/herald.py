@@ -234,7 +234,7 @@ class BlockPipeline:
             self.keep.append(ly)
         self.sel_idx = torch.zeros((max(units, 1), max(cap, 1)), dtype=torch.int32, device=dev)
         self.ws_select = alloc_workspace(herald_select_workspace_bytes(shape), dev)
-        self.ws_attn = alloc_workspace(herald_attn_workspace_bytes(shape), dev)
+        self.ws_attn = alloc_workspace(herald_attn_workspace_bytes(shape) * max(len(layers), 1), dev)   # one slice per layer
         self.main_stream = torch.cuda.Stream(device=dev, priority=-1)
         self.retrieval_stream = torch.cuda.Stream(device=dev, priority=0)
         self.ev_fork, self.ev_join = torch.cuda.Event(), torch.cuda.Event()
