@@ -440,7 +440,7 @@ def main():
                 "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s", "frac": attn_tflops_live / peaks["bf16_tflops_sustained"],
                 "traffic": NCU_ATTN_DRAM_BYTES.get(w.name),
                 "peak_source": peaks["source"] + " (sustained bf16, kernel timed inside a long step)",
-                "note": f"dominant kernel by time share; achieved = 4*M*(n+B)*128 FLOP per launch / (step time / {n_steps} launches); "
+                "note": f"dominant kernel by time share; achieved = 4*M*(n+B)*128 FLOP per launch / (step time / {n_steps * n_layers} launches); "
                         "traffic = dram__bytes_read+write per launch of the committed ncu capture (profiles/), cold L2"}
     roofline_scan = {"kernel": "scan_pm_kernel", "bound": "hbm", "achieved": scan_gbs_live, "peak": peaks["hbm_gbs"],
                      "unit": "GB/s", "frac": scan_gbs_live / peaks["hbm_gbs"], "traffic": NCU_SCAN_DRAM_BYTES.get(w.name),
