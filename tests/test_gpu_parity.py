@@ -405,3 +405,30 @@ def test_full_size_block_step_sampled(H, cuda, case):
             err = np.abs(outs[s, b:b + 1].cpu().numpy() - ref).max()
             assert err <= ATTN_TOL, (case, b, s, err)
     assert differing <= 1, f"{differing} units with in-band index swaps among {len(seqs) * Hkv}"
+
+
+def test_repeated_block_steps_are_bit_identical(H, cuda):
+    """Race detector of last resort (compute-sanitizer is closed on this pool): every kernel reduces in a fixed order,
+    so replaying the same block step must reproduce pools, pool lengths and attention outputs bit for bit."""
+    w = synth.Workload("rep", 3, (9000, 5555, 2049), 28, 4, 32, 6, 50, "planted", 10)
+    inp = synth.make_inputs(w, seed=77, device=cuda, spare_pages=2, hostile_tails=True)
+    ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
+    cap = max(ks) + w.block_size
+    shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, (w.max_seq_len + 15) // 16 * 16,
+                         inp["page_table"].shape[1], cap)
+    pipe = H.BlockPipeline(shape, [_layer_inputs(w, inp, ks, cuda)], w.n_attn_steps, 0, cuda)
+    pipe.step()
+    pipe.step()
+    graphs = pipe.capture()
+    ref = None
+    for it in range(40):
+        pipe.replay(graphs)
+        pipe.replay(graphs)          # two blocks: back to the same parity
+        torch.cuda.synchronize()
+        snap = (pipe.outs[0].clone(), pipe.pools_k[0][0].clone(), pipe.pools_v[0][1].clone(), pipe.pool_lens[0][0].clone())
+        if ref is None:
+            ref = snap
+            assert torch.isfinite(ref[0]).all()
+        else:
+            for a, b in zip(ref, snap):
+                assert torch.equal(a.view(torch.uint8), b.view(torch.uint8)), f"iteration {it} differs"
