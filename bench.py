@@ -389,6 +389,10 @@ def main():
     # time select with k=0 (top-k exits immediately): scan + histogram + launch of an empty top-k
     k_zero = torch.zeros_like(k_per_seq)
     scan_alone_ms = time_isolated(lambda: H.herald_select(shape, cache, inp["q_rep"], k_zero, sel_idx, sel_cnt, None, ws_sel, side))
+    # NEXT-1 of SURVEY 8(f): a layer that keeps its full KV attends over the paged cache itself
+    dense_attn_ms = time_isolated(lambda: H.herald_dense_attn(shape, cache, inp["q_blk"][0], inp["k_blk"][0], inp["v_blk"][0], out1, None,
+                                                              ws_att, side), reps=4, warm=2, timed=3)
+    dense_flops = sum(4 * M * (L + w.block_size) * 128 for L in w.seq_lens) * w.n_kv_heads
     denoise_alone_ms = attn_alone_ms * n_steps * n_layers        # stage timings are per layer (layer 0), the block has n_layers
     select_alone_ms, select_mode1_alone_ms = select_alone_ms * n_layers, select_mode1_alone_ms * n_layers
     gather_alone_ms_block = gather_alone_ms * n_layers
@@ -474,6 +478,7 @@ def main():
             "block_latency_ms": ms_step, "exposed_selection_ms": ms_step - denoise_alone_ms,
             "overlap_efficiency": (denoise_alone_ms + select_alone_ms + gather_alone_ms_block - ms_step) / (select_alone_ms + gather_alone_ms_block),
             "n_layers": n_layers,
+            "dense_attn_full_cache_ms": dense_attn_ms, "dense_attn_tflops": dense_flops / (dense_attn_ms * 1e-3) / 1e12,
             "attn_time_share_alone": attn_share,
             "algorithmic": {"scan_bytes": scan_bytes, "gather_bytes": gather_bytes, "attn_flops_per_step": attn_flops,
                             "attn_bytes_per_step": attn_bytes}},

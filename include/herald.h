@@ -133,6 +133,16 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
                        const int32_t* pool_len, const void* q_blk, const void* k_blk, const void* v_blk,
                        float* out, float* lse, void* ws, size_t ws_bytes, herald_stream_t stream);
 
+/* Dense attention of the block queries over the FULL paged cache + in-block KV, for layers that keep their whole KV
+ * ("the first two layers ... retain the full KV cache"; = herald_sparse_attn at a 100 % budget without
+ * the gather):
+ *   out[b][i][hq][:] = softmax_j( sm_scale * q_blk[b][i][hq][:] . K'_j ) . V'_j ,   h = hq / G,
+ *   K' = K[b, 0 .. seq_lens[b]), h, :] read through the page table, followed by k_blk[b][0..B)[h]  (no mask).
+ * Same tensor-core kernel; the key tiles are TMA boxes of the cache pages themselves.  Arguments as herald_sparse_attn;
+ * ws >= herald_attn_workspace_bytes(shape). */
+int herald_dense_attn(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_blk, const void* k_blk,
+                      const void* v_blk, float* out, float* lse, void* ws, size_t ws_bytes, herald_stream_t stream);
+
 /* Per-layer state of the dual-stream block step.  Host POD holding device pointers. */
 typedef struct herald_layer {
     herald_cache_t cache;      /* this layer's full KV pool                                                   */

@@ -16,6 +16,8 @@
 //             warps never wait for the tensor pipe and the pipe never waits for one softmax
 //   keys    = key tile 0 holds the B in-block rows (one TMA box of k_blk / v_blk), key tile t >= 1 holds pool rows
 //             [128(t-1), 128t) (one TMA box of the pool; softmax is invariant to the key order)
+//             (dense mode, herald_dense_attn: tile t >= 1 holds tokens [128(t-1), 128t) of the paged cache itself, one
+//             TMA box per 16-token page)
 //   warp 16   K producer (+ Q): tiles arrive by TMA (cp.async.bulk.tensor, 128B swizzle) into a 3-stage ring; a
 //             stage is released as soon as QK^T has read it.  Rows past the valid keys of a tile (stale pool rows,
 //             zero fill) give logits that the softmax masks.
@@ -91,6 +93,11 @@ static_assert(kTcMiscMax + 2 * 4 * 128 * 2 <= kTcMiscBytes, "exchange buffer ove
 struct AttnParams {
     const int32_t* pool_len;
     const int32_t* unit_order;   // optional [units]: units by decreasing pool length (attn_plan_kernel); NULL = identity
+    // dense mode (layers that keep their full KV): the keys of tile t >= 1 are tokens [128(t-1), 128t) of the
+    // paged cache itself -- 8 pages, one TMA box each -- and pool_len is unused
+    const int32_t* page_table;   // [batch][max_pages]; NULL = sparse mode (keys from the pool)
+    const int32_t* seq_lens;     // [batch]
+    int32_t max_pages, max_seq_len;
     float* out;
     float* lse;
     int32_t n_q_heads, n_kv_heads, block_size, cap, n_splits;
@@ -361,7 +368,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     // pool, so that the long units start first and the short ones fill the tail of a multi-wave grid
     const int unit = p.unit_order ? p.unit_order[blockIdx.z] : (int)blockIdx.z;
     const int b = unit / p.n_kv_heads, h = unit % p.n_kv_heads;
-    const int n_pool = max(0, min(p.pool_len[unit], p.cap));
+    const bool paged = p.page_table != nullptr;
+    const int n_pool = paged ? max(0, min(p.seq_lens[b], p.max_seq_len)) : max(0, min(p.pool_len[unit], p.cap));
     const int n_tiles = 1 + (n_pool + kTcBN - 1) / kTcBN;    // key tile 0 = the in-block rows, tile t >= 1 = pool rows [128(t-1), 128t)
     const int per = (n_tiles + S - 1) / S;
     const int t0 = split * per, t1 = min(n_tiles, t0 + per);
@@ -413,13 +421,26 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                         mbar_arrive_expect_tx(land, (uint32_t)B * 256u);
                         tma_load_4d(dst, map_blk, 0, h, 0, b, land);
                         tma_load_4d(dst + kTcHalfBytes, map_blk, 64, h, 0, b, land);
-                    } else {        // pool rows: box = (64 channels, pool_box rows, 1 unit) per half; rows past cap are zero-filled
+                    } else if (!paged) {   // pool rows: box = (64 channels, pool_box rows, 1 unit) per half; rows past cap are zero-filled
                         mbar_arrive_expect_tx(land, (uint32_t)p.pool_box * 256u);
                         tma_load_3d(dst, map, 0, (t - 1) * kTcBN, unit, land);
                         tma_load_3d(dst + kTcHalfBytes, map, 64, (t - 1) * kTcBN, unit, land);
                     }
                 }
                 __syncwarp();
+                if (paged && t > 0) {
+                    // dense mode: the 128 tokens of the tile are 8 pages of the cache; page i lands on tile rows [16i, 16i+16)
+                    // (2 KB per half: a whole number of 1 KB swizzle atoms).  Pages past the sequence are not requested.
+                    const int page0 = (t - 1) * (kTcBN / kPageSize), n_pg = (valid + kPageSize - 1) / kPageSize;
+                    const int my_phys = lane < n_pg ? __ldg(p.page_table + (int64_t)b * p.max_pages + page0 + lane) : 0;
+                    if (lane == 0) mbar_arrive_expect_tx(land, (uint32_t)n_pg * kPageSize * 256u);
+                    __syncwarp();
+                    if (lane < n_pg) {
+                        tma_load_4d(dst + lane * (kPageSize * 128), map, 0, h, 0, my_phys, land);
+                        tma_load_4d(dst + kTcHalfBytes + lane * (kPageSize * 128), map, 64, h, 0, my_phys, land);
+                    }
+                    __syncwarp();
+                }
                 if (is_k && j == 0) named_bar_sync(9, 64);
                 if (fix) {
                     mbar_wait(bar(kBarVTail), n_fixed & 1);

@@ -127,7 +127,7 @@ struct AttnGeom {
     size_t total;
 };
 
-static AttnGeom attn_geom(const herald_shape_t* s) {
+static AttnGeom attn_geom(const herald_shape_t* s, bool dense = false) {
     AttnGeom a{};
     const int G = s->n_q_heads / s->n_kv_heads;
     const int units = s->batch * s->n_kv_heads;
@@ -136,7 +136,8 @@ static AttnGeom attn_geom(const herald_shape_t* s) {
     a.m_tiles = (s->block_size + rows_cap - 1) / rows_cap;
     a.ipt = (s->block_size + a.m_tiles - 1) / a.m_tiles;
     // one CTA per SM: split the keys of a unit over a cluster until the grid covers the 148 SMs once
-    const int max_tiles = 1 + (s->pool_capacity + kTcBN - 1) / kTcBN;   // the in-block rows are a key tile of their own
+    const int max_keys = dense ? s->max_seq_len : s->pool_capacity;
+    const int max_tiles = 1 + (max_keys + kTcBN - 1) / kTcBN;   // the in-block rows are a key tile of their own
     const int target = env_int("HERALD_ATTN_TOTAL_CTAS", 148);
     int splits = units > 0 ? target / (units * a.m_tiles) : 1;
     const int forced = env_int("HERALD_ATTN_SPLITS", 0);
@@ -257,6 +258,27 @@ static int make_blk_map(CUtensorMap* out, const void* blk, const herald_shape_t*
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled(k_blk/v_blk) failed with CUresult %d", (int)r);
+    store_map(key, *map);
+    return HERALD_OK;
+}
+
+// Paged bf16 cache [n_pages][16][H_kv][128] (any strides) as a 4-D tensor (d, head, slot, page); box = 64 channels x 1 head x
+// 16 slots x 1 page: the 16 rows of one head of one page, one half.  The page extent is unknown to the ABI (page ids are
+// trusted): the map is given 2^24 pages.
+static int make_paged_map(CUtensorMap* out, const void* pages, const herald_cache_t* c, int n_kv_heads) {
+    const MapKey key{pages, {(int32_t)c->page_stride, (int32_t)c->token_stride, (int32_t)c->head_stride, 6 | (n_kv_heads << 8)}};
+    if (cached_map(key, out)) return HERALD_OK;
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
+    CUtensorMap* map = out;
+    const cuuint64_t dims[4] = {(cuuint64_t)kHeadDim, (cuuint64_t)n_kv_heads, (cuuint64_t)kPageSize, (cuuint64_t)1 << 24};
+    const cuuint64_t strides[3] = {(cuuint64_t)c->head_stride * 2, (cuuint64_t)c->token_stride * 2, (cuuint64_t)c->page_stride * 2};
+    const cuuint32_t box[4] = {64u, 1u, (cuuint32_t)kPageSize, 1u};
+    const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(pages), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled(paged cache) failed with CUresult %d", (int)r);
     store_map(key, *map);
     return HERALD_OK;
 }
@@ -454,15 +476,17 @@ int herald_gather(const herald_shape_t* shape, const herald_cache_t* cache, cons
 
 static int sparse_attn_impl(const herald_shape_t* shape, const void* pool_k, const void* pool_v, const int32_t* pool_len,
                             const void* q_blk, const void* k_blk, const void* v_blk, float* out, float* lse, void* ws,
-                            size_t ws_bytes, herald_stream_t stream_, const int32_t* unit_order) {
+                            size_t ws_bytes, herald_stream_t stream_, const int32_t* unit_order,
+                            const herald_cache_t* dense_cache = nullptr) {
+    const bool dense = dense_cache != nullptr;
     int rc = check_shape(shape);
     if (rc) return rc;
-    if (!pool_k || !pool_v || !pool_len || !q_blk || !k_blk || !v_blk || !out || !ws)
-        return fail(HERALD_ERR_INVALID_ARG, "herald_sparse_attn: NULL pointer");
+    if (!pool_k || !pool_v || (!dense && !pool_len) || !q_blk || !k_blk || !v_blk || !out || !ws)
+        return fail(HERALD_ERR_INVALID_ARG, "herald_sparse_attn / herald_dense_attn: NULL pointer");
     if (!aligned16(pool_k) || !aligned16(pool_v) || !aligned16(q_blk) || !aligned16(k_blk) || !aligned16(v_blk) ||
         !aligned16(out) || (reinterpret_cast<uintptr_t>(ws) & 255u))
         return fail(HERALD_ERR_INVALID_ARG, "herald_sparse_attn: misaligned pointer (16 B; workspace 256 B)");
-    const AttnGeom a = attn_geom(shape);
+    const AttnGeom a = attn_geom(shape, dense);
     if (ws_bytes < a.total) return fail(HERALD_ERR_WORKSPACE_TOO_SMALL, "herald_sparse_attn: workspace %zu < %zu", ws_bytes, a.total);
     const int units = shape->batch * shape->n_kv_heads;
     if (units == 0) return HERALD_OK;
@@ -476,9 +500,9 @@ static int sparse_attn_impl(const herald_shape_t* shape, const void* pool_k, con
         attr_set = true;
     }
     CUtensorMap tm_k, tm_v, tm_q, tm_kb, tm_vb;
-    rc = make_pool_map(&tm_k, pool_k, units, shape->pool_capacity);
+    rc = dense ? make_paged_map(&tm_k, pool_k, dense_cache, shape->n_kv_heads) : make_pool_map(&tm_k, pool_k, units, shape->pool_capacity);
     if (rc) return rc;
-    rc = make_pool_map(&tm_v, pool_v, units, shape->pool_capacity);
+    rc = dense ? make_paged_map(&tm_v, pool_v, dense_cache, shape->n_kv_heads) : make_pool_map(&tm_v, pool_v, units, shape->pool_capacity);
     if (rc) return rc;
     rc = make_q_map(&tm_q, q_blk, shape, a.ipt);
     if (rc) return rc;
@@ -489,6 +513,10 @@ static int sparse_attn_impl(const herald_shape_t* shape, const void* pool_k, con
     AttnParams ap{};
     ap.pool_len = pool_len;
     ap.unit_order = unit_order;
+    ap.page_table = dense ? dense_cache->page_table : nullptr;
+    ap.seq_lens = dense ? dense_cache->seq_lens : nullptr;
+    ap.max_pages = shape->max_pages_per_seq;
+    ap.max_seq_len = shape->max_seq_len;
     ap.out = out;
     ap.lse = lse;
     ap.n_q_heads = shape->n_q_heads;
@@ -535,6 +563,15 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
                        const void* q_blk, const void* k_blk, const void* v_blk, float* out, float* lse, void* ws,
                        size_t ws_bytes, herald_stream_t stream_) {
     return sparse_attn_impl(shape, pool_k, pool_v, pool_len, q_blk, k_blk, v_blk, out, lse, ws, ws_bytes, stream_, nullptr);
+}
+
+int herald_dense_attn(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_blk, const void* k_blk,
+                      const void* v_blk, float* out, float* lse, void* ws, size_t ws_bytes, herald_stream_t stream_) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    rc = check_cache(cache, true);
+    if (rc) return rc;
+    return sparse_attn_impl(shape, cache->k_pages, cache->v_pages, nullptr, q_blk, k_blk, v_blk, out, lse, ws, ws_bytes, stream_, nullptr, cache);
 }
 
 // Longest-pool-first unit order of one layer into `order` (device, [units]); enqueued on `stream`.

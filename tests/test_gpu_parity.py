@@ -432,3 +432,35 @@ def test_repeated_block_steps_are_bit_identical(H, cuda):
         else:
             for a, b in zip(ref, snap):
                 assert torch.equal(a.view(torch.uint8), b.view(torch.uint8)), f"iteration {it} differs"
+
+
+DENSE_CASES = {
+    # name: (workload, spare pages, hostile tails)
+    "ragged_g7": (synth.Workload("dg7", 3, (2000, 777, 1), 28, 4, 32, 3, 1000, "plain"), 2, True),
+    "g4_b16": (synth.Workload("dg4", 2, (4096, 130), 8, 2, 16, 2, 1000, "plain"), 0, True),
+    "empty_and_short": (synth.Workload("dshort", 3, (0, 15, 16), 4, 1, 16, 2, 1000, "plain"), 1, True),
+}
+
+
+@pytest.mark.parametrize("case", list(DENSE_CASES))
+def test_dense_attn_over_the_paged_cache_matches_oracle(H, cuda, case):
+    """herald_dense_attn (layers that keep their full KV) against the oracle's attention over a pool that
+    holds the whole prefix (budget 100 %: select = identity, gather = un-paging)."""
+    w, spare, hostile = DENSE_CASES[case]
+    inp = synth.make_inputs(w, seed=500 + len(case), device=cuda, spare_pages=spare, hostile_tails=hostile)
+    msl = max((w.max_seq_len + 15) // 16 * 16, 16)
+    shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, msl, inp["page_table"].shape[1], 16)
+    cache = H.make_cache(inp["k_pages"], inp["v_pages"], inp["page_table"], inp["seq_lens"])
+    out = torch.full((w.batch, w.block_size, w.n_q_heads, 128), float("nan"), dtype=torch.float32, device=cuda)
+    lse = torch.empty((w.batch, w.block_size, w.n_q_heads), dtype=torch.float32, device=cuda)
+    ws = H.alloc_workspace(H.herald_attn_workspace_bytes(shape), cuda)
+    H.herald_dense_attn(shape, cache, inp["q_blk"][0], inp["k_blk"][0], inp["v_blk"][0], out, lse, ws)
+    torch.cuda.synchronize()
+    oi = oracle_inputs(inp)
+    sel = [[np.arange(L, dtype=np.int32) for _ in range(w.n_kv_heads)] for L in w.seq_lens]
+    pk, pv, pl = O.gather(oi["k_pages"], oi["v_pages"], oi["page_table"], sel, max(w.max_seq_len, 1))
+    ref, lse_ref = O.sparse_attn(synth.to_u16(inp["q_blk"][0]), synth.to_u16(inp["k_blk"][0]), synth.to_u16(inp["v_blk"][0]),
+                                 pk, pv, pl, 128 ** -0.5)
+    err = np.abs(out.cpu().numpy().astype(np.float64) - ref).max()
+    assert np.isfinite(err) and err <= ATTN_TOL, (case, err)
+    assert np.abs(lse.cpu().numpy() - lse_ref).max() <= 2e-3
