@@ -23,7 +23,7 @@ Data conventions (same as include/herald.h, but HOST NumPy arrays):
   * query head ``hq`` belongs to KV head ``hq // G`` with ``G = H_q // H_kv``
     (section IV-B4: "G is the number of query heads that share one KV head under GQA").
 
-Pin status (see tests/test_oracle_pins.py, all ``-m "not gpu"``): every function
+Pin status (see tests/test_oracle_pins.py, all ``-m "not gpu"``; ``rep_attn`` included): every function
 below is pinned against something other than itself -- closed forms, brute
 force pure-Python loops, library SDPA / softmax, invariants.  No function is
 "parity unpinned".
@@ -250,3 +250,33 @@ def pipeline_step(layers, n_steps, sm_scale, agg_mode=AGG_MAX_LOGIT):
         pk, pv, pl = gather(ly["k_pages"], ly["v_pages"], ly["page_table"], sel, ly["pool_capacity"])
         results.append(dict(outs=outs, next_pool_k=pk, next_pool_v=pv, next_pool_len=pl, sel=sel))
     return results
+
+
+# ----------------------------------------------------------------------------
+# NEXT-2: attention output of the representative query itself
+# (section IV-B4: the fused kernel "maintains the FlashAttention statistics (m_g, l_g, o_g)"
+#  next to the raw scores; the output o_g goes back to the GPU for the layer's FFN)
+# ----------------------------------------------------------------------------
+def rep_attn(q_rep_u16, k_pages_u16, v_pages_u16, page_table, seq_lens, n_kv_heads, sm_scale):
+    """o[b, hq, :] = softmax_t(sm_scale * q_rep[b, hq] . K[b, t, h]) . V[b, t, h, :] over every cached t < seq_lens[b]
+    (h = hq // G), the plain definition.  Returns (out fp64 [batch, H_q, d], lse fp64 [batch, H_q]); a sequence with no
+    cached token gives out = 0 and lse = -inf."""
+    batch, H_q, d = q_rep_u16.shape
+    G = H_q // n_kv_heads
+    out = np.zeros((batch, H_q, d), dtype=np.float64)
+    lse = np.full((batch, H_q), -np.inf, dtype=np.float64)
+    for b in range(batch):
+        L = int(seq_lens[b])
+        if L == 0:
+            continue
+        for h in range(n_kv_heads):
+            K = bf16_bits_to_f64(cached_rows(k_pages_u16, page_table, b, L, h))      # [L, d]
+            V = bf16_bits_to_f64(cached_rows(v_pages_u16, page_table, b, L, h))
+            s = raw_scores(q_rep_u16[b, h * G:(h + 1) * G, :], cached_rows(k_pages_u16, page_table, b, L, h), sm_scale)   # [G, L]
+            m = s.max(axis=1, keepdims=True)
+            p = np.exp(s - m)
+            z = p.sum(axis=1, keepdims=True)
+            out[b, h * G:(h + 1) * G, :] = (p @ V) / z
+            lse[b, h * G:(h + 1) * G] = (m + np.log(z))[:, 0]
+            del K
+    return out, lse

@@ -407,3 +407,48 @@ def test_pipeline_step_is_the_sequential_composition():
         for h in range(2):
             planted = set(inp["planted"][b][h].tolist())
             assert len(planted & set(sel[b][h].tolist())) >= len(planted) - 1
+
+
+# ---- NEXT-2: attention output of the representative query ---------------------------------------
+def _rep_inputs(seed, seq_lens=(37, 5, 0), Hq=4, Hkv=2):
+    w = synth.Workload("rep", len(seq_lens), tuple(seq_lens), Hq, Hkv, 16, 2, 100, "plain")
+    inp = synth.make_inputs(w, seed, "cpu", spare_pages=1, hostile_tails=True, with_block_inputs=False)
+    return w, (synth.to_u16(inp["q_rep"]), synth.to_u16(inp["k_pages"]), synth.to_u16(inp["v_pages"]),
+               inp["page_table"].numpy(), inp["seq_lens"].numpy())
+
+
+def test_rep_attn_matches_library_sdpa_and_ignores_tails():
+    w, (q, kp, vp, pt, sl) = _rep_inputs(31)
+    out, lse = O.rep_attn(q, kp, vp, pt, sl, w.n_kv_heads, 128 ** -0.5)
+    G = w.group
+    for b, L in enumerate(w.seq_lens):
+        for h in range(w.n_kv_heads):
+            if L == 0:
+                assert np.all(out[b] == 0) and np.all(np.isneginf(lse[b]))
+                continue
+            K = torch.as_tensor(O.bf16_bits_to_f64(O.cached_rows(kp, pt, b, L, h)))
+            V = torch.as_tensor(O.bf16_bits_to_f64(O.cached_rows(vp, pt, b, L, h)))
+            Q = torch.as_tensor(O.bf16_bits_to_f64(q[b, h * G:(h + 1) * G]))                  # [G, d]
+            ref = torch.nn.functional.scaled_dot_product_attention(Q[None, :, None, :], K[None, None].expand(1, G, -1, -1),
+                                                                   V[None, None].expand(1, G, -1, -1), scale=128 ** -0.5)
+            assert np.allclose(out[b, h * G:(h + 1) * G], ref[0, :, 0].numpy(), rtol=0, atol=1e-12)
+            logits = (Q @ K.T).numpy() * 128 ** -0.5
+            assert np.allclose(lse[b, h * G:(h + 1) * G], np.log(np.exp(logits).sum(axis=1)), rtol=0, atol=1e-12)
+
+
+def test_rep_attn_closed_forms():
+    # one cached token => its V row; constant V => that constant; the softmax weights are those of aggregate mode 1
+    w, (q, kp, vp, pt, sl) = _rep_inputs(32, seq_lens=(1, 64), Hq=2, Hkv=1)
+    out, _ = O.rep_attn(q, kp, vp, pt, sl, 1, 128 ** -0.5)
+    v0 = O.bf16_bits_to_f64(O.cached_rows(vp, pt, 0, 1, 0))[0]
+    assert np.allclose(out[0, 0], v0, atol=1e-15) and np.allclose(out[0, 1], v0, atol=1e-15)
+    vp2 = vp.copy()
+    vp2[:] = bf16_bits(np.float32(0.75))
+    out2, _ = O.rep_attn(q, kp, vp2, pt, sl, 1, 128 ** -0.5)
+    assert np.allclose(out2, 0.75, atol=1e-14)
+    s = O.raw_scores(q[1], O.cached_rows(kp, pt, 1, 64, 0), 128 ** -0.5)                     # [G, 64]
+    p = np.exp(s - s.max(axis=1, keepdims=True))
+    p /= p.sum(axis=1, keepdims=True)
+    assert np.allclose(p.sum(axis=0), O.aggregate(s, O.AGG_SOFTMAX_SUM), atol=1e-14)        # ŝ_h[s] of PAPER.md:209
+    V = O.bf16_bits_to_f64(O.cached_rows(vp, pt, 1, 64, 0))
+    assert np.allclose(out[1], p @ V, atol=1e-13)
