@@ -392,6 +392,10 @@ def main():
     # NEXT-1 of SURVEY 8(f): a layer that keeps its full KV attends over the paged cache itself
     dense_attn_ms = time_isolated(lambda: H.herald_dense_attn(shape, cache, inp["q_blk"][0], inp["k_blk"][0], inp["v_blk"][0], out1, None,
                                                               ws_att, side), reps=4, warm=2, timed=3)
+    # NEXT-2: the representative query's own attention output (second HBM stream, over K and V)
+    rep_out = torch.empty((w.batch, w.n_q_heads, 128), dtype=torch.float32, device=dev)
+    ws_rep = H.alloc_workspace(H.herald_rep_attn_workspace_bytes(shape), dev)
+    rep_attn_ms = time_isolated(lambda: H.herald_rep_attn(shape, cache, inp["q_rep"], rep_out, None, ws_rep, side), reps=4, warm=2, timed=3)
     dense_flops = sum(4 * M * (L + w.block_size) * 128 for L in w.seq_lens) * w.n_kv_heads
     denoise_alone_ms = attn_alone_ms * n_steps * n_layers        # stage timings are per layer (layer 0), the block has n_layers
     select_alone_ms, select_mode1_alone_ms = select_alone_ms * n_layers, select_mode1_alone_ms * n_layers
@@ -478,6 +482,7 @@ def main():
             "block_latency_ms": ms_step, "exposed_selection_ms": ms_step - denoise_alone_ms,
             "overlap_efficiency": (denoise_alone_ms + select_alone_ms + gather_alone_ms_block - ms_step) / (select_alone_ms + gather_alone_ms_block),
             "n_layers": n_layers,
+            "rep_attn_ms": rep_attn_ms, "rep_attn_gbs": tokens * w.n_kv_heads * 512 / (rep_attn_ms * 1e-3) / 1e9,
             "dense_attn_full_cache_ms": dense_attn_ms, "dense_attn_tflops": dense_flops / (dense_attn_ms * 1e-3) / 1e12,
             "attn_time_share_alone": attn_share,
             "algorithmic": {"scan_bytes": scan_bytes, "gather_bytes": gather_bytes, "attn_flops_per_step": attn_flops,

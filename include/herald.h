@@ -143,6 +143,16 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
 int herald_dense_attn(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_blk, const void* k_blk,
                       const void* v_blk, float* out, float* lse, void* ws, size_t ws_bytes, herald_stream_t stream);
 
+/* Attention output of the representative query itself (the fused selection kernel keeps the
+ * FlashAttention statistics (m_g, l_g, o_g); o_g returns to the layer's FFN):
+ *   out[b][hq][:] = softmax_t( sm_scale * q_rep[b][hq][:] . K[b,t,h,:] ) . V[b,t,h,:]  over all t < seq_lens[b], h = hq / G
+ *   q_rep bf16 [batch][H_q][128]; out fp32 [batch][H_q][128]; lse optional fp32 [batch][H_q] (= log sum_t exp(logit_t)).
+ *   A sequence without cached tokens gives zeros (lse = -inf).  ws >= herald_rep_attn_workspace_bytes(shape), 256-byte aligned.
+ * A second HBM stream over K and V (512 B per token and KV head); fp32 accumulation. */
+size_t herald_rep_attn_workspace_bytes(const herald_shape_t* shape);
+int herald_rep_attn(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep, float* out, float* lse,
+                    void* ws, size_t ws_bytes, herald_stream_t stream);
+
 /* Per-layer state of the dual-stream block step.  Host POD holding device pointers. */
 typedef struct herald_layer {
     herald_cache_t cache;      /* this layer's full KV pool                                                   */

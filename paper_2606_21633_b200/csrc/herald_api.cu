@@ -10,6 +10,7 @@
 #include "attn_tc.cuh"
 #include "common.cuh"
 #include "gather.cuh"
+#include "rep_attn.cuh"
 #include "scan.cuh"
 #include "topk.cuh"
 
@@ -572,6 +573,57 @@ int herald_dense_attn(const herald_shape_t* shape, const herald_cache_t* cache, 
     rc = check_cache(cache, true);
     if (rc) return rc;
     return sparse_attn_impl(shape, cache->k_pages, cache->v_pages, nullptr, q_blk, k_blk, v_blk, out, lse, ws, ws_bytes, stream_, nullptr, cache);
+}
+
+static int rep_chunks(const herald_shape_t* s) {
+    const int c = (s->max_seq_len + kRepChunkTokens - 1) / kRepChunkTokens;
+    return c > 0 ? c : 1;
+}
+
+size_t herald_rep_attn_workspace_bytes(const herald_shape_t* shape) {
+    if (check_shape(shape) != HERALD_OK) return 0;
+    const size_t units = (size_t)shape->batch * shape->n_kv_heads;
+    return align_up((units > 0 ? units : 1) * rep_chunks(shape) * kRepPartFloats * sizeof(float), 256);
+}
+
+int herald_rep_attn(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep, float* out, float* lse,
+                    void* ws, size_t ws_bytes, herald_stream_t stream_) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    rc = check_cache(cache, true);
+    if (rc) return rc;
+    if (!q_rep || !out || !ws) return fail(HERALD_ERR_INVALID_ARG, "herald_rep_attn: NULL pointer");
+    if (!aligned16(q_rep) || !aligned16(out) || (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return fail(HERALD_ERR_INVALID_ARG, "herald_rep_attn: misaligned pointer (16 B; workspace 256 B)");
+    const size_t need = herald_rep_attn_workspace_bytes(shape);
+    if (ws_bytes < need) return fail(HERALD_ERR_WORKSPACE_TOO_SMALL, "herald_rep_attn: workspace %zu < %zu", ws_bytes, need);
+    const int units = shape->batch * shape->n_kv_heads;
+    if (units == 0) return HERALD_OK;
+    g_err[0] = 0;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    RepAttnParams rp{};
+    rp.k_pages = static_cast<const __nv_bfloat16*>(cache->k_pages);
+    rp.v_pages = static_cast<const __nv_bfloat16*>(cache->v_pages);
+    rp.page_stride = cache->page_stride;
+    rp.token_stride = cache->token_stride;
+    rp.head_stride = cache->head_stride;
+    rp.page_table = cache->page_table;
+    rp.seq_lens = cache->seq_lens;
+    rp.q_rep = static_cast<const __nv_bfloat16*>(q_rep);
+    rp.part = static_cast<float*>(ws);
+    rp.out = out;
+    rp.lse = lse;
+    rp.n_q_heads = shape->n_q_heads;
+    rp.n_kv_heads = shape->n_kv_heads;
+    rp.max_seq_len = shape->max_seq_len;
+    rp.max_pages = shape->max_pages_per_seq;
+    rp.n_chunks = rep_chunks(shape);
+    rp.scale_log2 = shape->sm_scale * 1.4426950408889634f;
+    rep_attn_kernel<<<dim3(rp.n_chunks, units), kRepThreads, 0, stream>>>(rp);
+    rep_attn_merge_kernel<<<units, kHeadDim, 0, stream>>>(rp);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "rep_attn launch");
+    return HERALD_OK;
 }
 
 // Longest-pool-first unit order of one layer into `order` (device, [units]); enqueued on `stream`.

@@ -464,3 +464,38 @@ def test_dense_attn_over_the_paged_cache_matches_oracle(H, cuda, case):
     err = np.abs(out.cpu().numpy().astype(np.float64) - ref).max()
     assert np.isfinite(err) and err <= ATTN_TOL, (case, err)
     assert np.abs(lse.cpu().numpy() - lse_ref).max() <= 2e-3
+
+
+REP_CASES = {
+    "ragged_g7": (synth.Workload("rg7", 4, (5000, 2049, 16, 0), 28, 4, 32, 2, 50, "planted", 8), 2, True),
+    "g8_h8": (synth.Workload("rg8", 2, (4096, 33), 64, 8, 16, 2, 50, "zipf"), 0, True),
+    "g1": (synth.Workload("rg1", 2, (1, 700), 2, 2, 16, 2, 50, "plain"), 1, True),
+}
+
+
+@pytest.mark.parametrize("case", list(REP_CASES))
+def test_rep_attn_matches_oracle(H, cuda, case):
+    """herald_rep_attn: the representative query's own attention output over the whole cache."""
+    w, spare, hostile = REP_CASES[case]
+    inp = synth.make_inputs(w, seed=600 + len(case), device=cuda, spare_pages=spare, hostile_tails=hostile, with_block_inputs=False)
+    # uninitialised-looking V tails: the kernel must not let 0 x NaN through
+    pt = inp["page_table"].cpu().numpy()
+    for b, L in enumerate(w.seq_lens):
+        if L % 16:
+            inp["v_pages"][int(pt[b, L // 16]), L % 16:] = float("nan")
+    msl = max((w.max_seq_len + 15) // 16 * 16, 16)
+    shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, msl, inp["page_table"].shape[1], 16)
+    cache = H.make_cache(inp["k_pages"], inp["v_pages"], inp["page_table"], inp["seq_lens"])
+    out = torch.full((w.batch, w.n_q_heads, 128), float("nan"), dtype=torch.float32, device=cuda)
+    lse = torch.full((w.batch, w.n_q_heads), float("nan"), dtype=torch.float32, device=cuda)
+    ws = H.alloc_workspace(H.herald_rep_attn_workspace_bytes(shape), cuda)
+    H.herald_rep_attn(shape, cache, inp["q_rep"], out, lse, ws)
+    torch.cuda.synchronize()
+    oi = oracle_inputs(inp)
+    vp = oi["v_pages"].copy()
+    ref, lse_ref = O.rep_attn(oi["q_rep"], oi["k_pages"], vp, oi["page_table"], oi["seq_lens"], w.n_kv_heads, 128 ** -0.5)
+    got, got_lse = out.cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64)
+    assert np.isfinite(got).all()
+    assert np.abs(got - ref).max() <= 1e-4, (case, np.abs(got - ref).max())     # fp32 P and accumulation: no bf16 rounding of P here
+    fin = np.isfinite(lse_ref)
+    assert np.array_equal(np.isneginf(got_lse), ~fin) and np.abs(got_lse[fin] - lse_ref[fin]).max() <= 1e-3
