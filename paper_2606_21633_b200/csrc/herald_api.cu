@@ -428,11 +428,18 @@ int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, cons
     tp.cap = shape->pool_capacity;
     static bool topk_attr_set = false;
     if (!topk_attr_set) {
-        e = cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTopkSmemBytes);
+        e = cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTopkMaxSmemBytes);
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(topk)");
         topk_attr_set = true;
     }
-    topk_kernel<<<units, kTopkThreads, kTopkSmemBytes, stream>>>(tp);
+    // shared memory of the one-pass path: a bit per position and room for 1/8 of the positions in the threshold bin
+    // (N(0,1)-like scores put 1-5 % of them there); what does not fit takes the multi-pass path
+    tp.bitmap_words = (shape->max_seq_len + 31) / 32;
+    if (tp.bitmap_words > kTopkMaxBitmapWords) tp.bitmap_words = kTopkMaxBitmapWords;
+    tp.cand_cap = shape->max_seq_len / 8;
+    if (tp.cand_cap < 2048) tp.cand_cap = 2048;
+    if (tp.cand_cap > kTopkMaxCandCap) tp.cand_cap = kTopkMaxCandCap;
+    topk_kernel<<<units, kTopkThreads, (size_t)tp.cand_cap * 8 + 2 * (size_t)tp.bitmap_words * 4, stream>>>(tp);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "topk launch");
     if (prof && prof->topk_end) cudaEventRecord(static_cast<cudaEvent_t>(prof->topk_end), stream);

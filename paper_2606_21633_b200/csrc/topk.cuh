@@ -4,7 +4,8 @@
 // the lower position, emitted in ascending position) is an MSB-first radix select on an order-preserving
 // 32-bit key (12 + 10 + 10 bits).  One 1024-thread CTA per unit.
 //   level 1 histogram : already accumulated by the scan kernel's epilogue (hist1) -> threshold bin b1
-//   fast path (the threshold bin holds <= kTopkCandCap scores, positions < 32 * kTopkBitmapWords):
+//   fast path (the threshold bin holds <= cand_cap scores, positions < 32 * bitmap_words; both sized by the launcher
+//   from max_seq_len so that two CTAs share an SM on the common shapes):
 //     ONE pass over the score plane: scores above bin b1 set their bit in a shared-memory position bitmap,
 //     scores inside bin b1 are appended (key, position) to a shared-memory candidate list (warp-aggregated);
 //     levels 2 and 3 run on the candidate list; exact ties keep the lowest positions through a second bitmap
@@ -17,9 +18,9 @@
 namespace herald {
 
 constexpr int kTopkThreads = 1024;
-constexpr int kTopkCandCap = 12288;                 // (key, position) pairs of the threshold bin held in shared memory
-constexpr int kTopkBitmapWords = 8192;              // one bit per position: fast path for L <= 262144
-constexpr int kTopkSmemBytes = kTopkCandCap * 8 + 2 * kTopkBitmapWords * 4;   // candidates, selected bitmap, tie bitmap
+constexpr int kTopkMaxCandCap = 12288;              // (key, position) pairs of the threshold bin held in shared memory, at most
+constexpr int kTopkMaxBitmapWords = 8192;           // one bit per position: fast path for L <= 262144
+constexpr int kTopkMaxSmemBytes = kTopkMaxCandCap * 8 + 2 * kTopkMaxBitmapWords * 4;   // candidates, selected bitmap, tie bitmap
 
 // Find bin j with  count(bins > j) < kk <= count(bins >= j).  Returns j, *above = count(bins > j).
 // hist has nbins (multiple of blockDim) entries in shared memory; every thread must call.
@@ -56,9 +57,10 @@ struct TopkParams {
     int32_t* sel_idx;          // [units][cap]
     int32_t* sel_cnt;          // [units]
     int32_t n_kv_heads, max_seq_len, cap;
+    int32_t cand_cap, bitmap_words;   // dynamic shared memory = cand_cap * 8 + 2 * bitmap_words * 4 bytes
 };
 
-__global__ void __launch_bounds__(kTopkThreads, 1) topk_kernel(const TopkParams p) {
+__global__ void __launch_bounds__(kTopkThreads, 2) topk_kernel(const TopkParams p) {
     __shared__ uint32_t s_hist[kBins1];
     __shared__ uint32_t s_warp[33];
     __shared__ uint32_t s_res[2];
@@ -84,12 +86,12 @@ __global__ void __launch_bounds__(kTopkThreads, 1) topk_kernel(const TopkParams 
     const uint32_t k2 = kk - above1;
 
     const uint32_t n_c = s_hist[b1];                   // scores inside the threshold bin
-    if (n_c <= (uint32_t)kTopkCandCap && L <= 32 * kTopkBitmapWords) {
+    if (n_c <= (uint32_t)p.cand_cap && L <= 32 * p.bitmap_words) {
         // ---------------- fast path: one pass over the plane ----------------
         extern __shared__ __align__(16) uint8_t topk_smem[];
         uint2* cand = reinterpret_cast<uint2*>(topk_smem);                                   // (key, position)
-        uint32_t* bitmap = reinterpret_cast<uint32_t*>(topk_smem + kTopkCandCap * 8);        // selected positions
-        uint32_t* tiemap = bitmap + kTopkBitmapWords;                                        // positions with key == T
+        uint32_t* bitmap = reinterpret_cast<uint32_t*>(topk_smem + (size_t)p.cand_cap * 8);  // selected positions
+        uint32_t* tiemap = bitmap + p.bitmap_words;                                          // positions with key == T
         const int n_words = (L + 31) >> 5;
         const int lane = tid & 31;
         for (int i = tid; i < n_words; i += kTopkThreads) { bitmap[i] = 0; tiemap[i] = 0; }
