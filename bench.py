@@ -419,7 +419,7 @@ def main():
     a.record(pipe.main_stream)
     for _ in range(e2e_steps):
         pipe.step_host(io)
-    b.record(pipe.main_stream)
+    b.record(pipe.retrieval_stream)          # the last download of the outputs runs on the retrieval stream
     torch.cuda.synchronize()
     e2e_ms = max_over_ranks(a.elapsed_time(b), dev) / e2e_steps
     e2e_tokens = world * w.batch * w.block_size / (e2e_ms * 1e-3)

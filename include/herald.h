@@ -220,8 +220,10 @@ int herald_pipeline_set_profile(const herald_profile_t* prof);
  *   herald_pipeline_step
  *   D2H  layers[l].out -> host_out[l]
  * Each host_* is a host array of n_layers host pointers with the same extents as the device tensors.
- * The KV cache stays resident in HBM (it is the state, not a per-step input).  The caller
- * synchronises main_stream before reading host_out. */
+ * The KV cache stays resident in HBM (it is the state, not a per-step input).  Uploads run on the main stream and
+ * downloads on the retrieval stream, so that the upload of a block overlaps the download of the previous one; the next
+ * call orders its attention after that download by itself.  The caller synchronises BOTH streams before reading
+ * host_out (or before touching the host input buffers again). */
 typedef struct herald_host_io {
     const void* const* host_q_rep;
     const void* const* host_q_blk;

@@ -748,11 +748,15 @@ int herald_pipeline_step_host(herald_pipeline_t* p, const herald_host_io_t* io) 
     if (!io || !io->host_q_rep || !io->host_q_blk || !io->host_k_blk || !io->host_v_blk || !io->host_out)
         return fail(HERALD_ERR_INVALID_ARG, "pipeline_step_host: NULL host io");
     cudaStream_t s_main = static_cast<cudaStream_t>(p->main_stream);
+    cudaStream_t s_ret = static_cast<cudaStream_t>(p->retrieval_stream);
+    cudaEvent_t ev_fork = static_cast<cudaEvent_t>(p->ev_fork), ev_join = static_cast<cudaEvent_t>(p->ev_join);
     const herald_shape_t* sh = &p->shape;
     const size_t q_step = (size_t)sh->batch * sh->block_size * sh->n_q_heads * kHeadDim;
     const size_t kv_step = (size_t)sh->batch * sh->block_size * sh->n_kv_heads * kHeadDim;
     const size_t q_rep_bytes = (size_t)sh->batch * sh->n_q_heads * kHeadDim * 2;
     cudaError_t e;
+    // The two copy directions run on the two streams so that the upload of this block overlaps the download of the
+    // previous one (full-duplex link, two copy engines): uploads on the main stream, downloads on the retrieval stream.
     for (int l = 0; l < p->n_layers; ++l) {
         herald_layer_t* ly = &p->layers[l];
         // inputs are enqueued on the main stream; the fork event orders the retrieval stream after them
@@ -765,13 +769,21 @@ int herald_pipeline_step_host(herald_pipeline_t* p, const herald_host_io_t* io) 
             e = cudaMemcpyAsync(const_cast<void*>(ly->v_blk), io->host_v_blk[l], kv_step * p->n_steps * 2, cudaMemcpyHostToDevice, s_main);
         if (e != cudaSuccess) return cuda_fail(e, "H2D copy");
     }
+    // this block's attention overwrites `out`: the previous call's download (last record of ev_join) must have read it
+    e = cudaStreamWaitEvent(s_main, ev_join, 0);
+    if (e != cudaSuccess) return cuda_fail(e, "wait previous download");
     rc = herald_pipeline_step(p);
     if (rc) return rc;
+    e = cudaEventRecord(ev_fork, s_main);                    // outputs of this block are complete
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s_ret, ev_fork, 0);
+    if (e != cudaSuccess) return cuda_fail(e, "order download after the block");
     for (int l = 0; l < p->n_layers; ++l) {
         herald_layer_t* ly = &p->layers[l];
-        e = cudaMemcpyAsync(io->host_out[l], ly->out, q_step * p->n_steps * sizeof(float), cudaMemcpyDeviceToHost, s_main);
+        e = cudaMemcpyAsync(io->host_out[l], ly->out, q_step * p->n_steps * sizeof(float), cudaMemcpyDeviceToHost, s_ret);
         if (e != cudaSuccess) return cuda_fail(e, "D2H copy");
     }
+    e = cudaEventRecord(ev_join, s_ret);                     // download done: the next call waits on it
+    if (e != cudaSuccess) return cuda_fail(e, "record download");
     return HERALD_OK;
 }
 
