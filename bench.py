@@ -31,8 +31,8 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/r1_*), by workload
-NCU_ATTN_DRAM_BYTES = {"C2": 29.7e6}
-NCU_SCAN_DRAM_BYTES = {"C2": 274.0e6}
+NCU_ATTN_DRAM_BYTES = {"C2": 30.7e6}
+NCU_SCAN_DRAM_BYTES = {"C2": 275.5e6}
 METRIC = "selection-scan HBM GB/s (% of 8 TB/s); sparse-attn TFLOP/s; block tokens/s"
 WORKLOAD = "C2"
 SEED = 21633 + 1000 * 2
