@@ -280,3 +280,40 @@ def rep_attn(q_rep_u16, k_pages_u16, v_pages_u16, page_table, seq_lens, n_kv_hea
             lse[b, h * G:(h + 1) * G] = (m + np.log(z))[:, 0]
             del K
     return out, lse
+
+
+# ----------------------------------------------------------------------------
+# NEXT-3: block-boundary cache operations
+# (the draft KV of block n is "appended temporarily" to the full KV pool; at the end of
+#  the block the true KV is "written to both block n+1's GPU pool and the full KV pool, replacing the draft")
+# ----------------------------------------------------------------------------
+def cache_write_block(k_pages_u16, v_pages_u16, page_table, write_pos, k_new_u16, v_new_u16):
+    """K[b, write_pos[b] + i, h, :] = k_new[b, i, h, :] for i < B (same for V), through the page table: appends the B
+    rows of a block (draft or true) at logical position write_pos[b], or replaces rows already there.  Bit copies, in
+    place on copies of the page arrays, which are returned."""
+    kp, vp = k_pages_u16.copy(), v_pages_u16.copy()
+    page_size = kp.shape[1]
+    batch, B = k_new_u16.shape[0], k_new_u16.shape[1]
+    for b in range(batch):
+        for i in range(B):
+            t = int(write_pos[b]) + i
+            phys, slot = int(page_table[b, t // page_size]), t % page_size
+            kp[phys, slot] = k_new_u16[b, i]
+            vp[phys, slot] = v_new_u16[b, i]
+    return kp, vp
+
+
+def pool_append_block(pool_k_u16, pool_v_u16, pool_len, k_new_u16, v_new_u16):
+    """pool[b, h, pool_len[b, h] + i, :] = k_new[b, i, h, :] for i < B, then pool_len += B (the completed block joins the
+    next block's pool; reading 10 of DESIGN.md: pool_capacity >= k + B).  Returns copies."""
+    pk, pv, pl = pool_k_u16.copy(), pool_v_u16.copy(), np.array(pool_len, dtype=np.int32).copy()
+    batch, H_kv, cap, _ = pk.shape
+    B = k_new_u16.shape[1]
+    for b in range(batch):
+        for h in range(H_kv):
+            n = int(pl[b, h])
+            assert n + B <= cap
+            pk[b, h, n:n + B] = k_new_u16[b, :, h]
+            pv[b, h, n:n + B] = v_new_u16[b, :, h]
+            pl[b, h] = n + B
+    return pk, pv, pl

@@ -452,3 +452,39 @@ def test_rep_attn_closed_forms():
     assert np.allclose(p.sum(axis=0), O.aggregate(s, O.AGG_SOFTMAX_SUM), atol=1e-14)        # ŝ_h[s] of PAPER.md:209
     V = O.bf16_bits_to_f64(O.cached_rows(vp, pt, 1, 64, 0))
     assert np.allclose(out[1], p @ V, atol=1e-13)
+
+
+# ---- NEXT-3: block-boundary cache operations ------------------------------------------------------
+def test_cache_write_block_roundtrip_and_locality():
+    w = synth.Workload("cw", 2, (40, 23), 4, 2, 16, 2, 100, "plain")
+    inp = synth.make_inputs(w, 41, "cpu", spare_pages=2)
+    kp, vp = synth.to_u16(inp["k_pages"]), synth.to_u16(inp["v_pages"])
+    pt = inp["page_table"].numpy()
+    rng = np.random.default_rng(3)
+    k_new = rng.integers(0, 2 ** 16, size=(2, 8, 2, 128), dtype=np.uint16)
+    v_new = rng.integers(0, 2 ** 16, size=(2, 8, 2, 128), dtype=np.uint16)
+    pos = np.array([32, 7])                         # sequence 0: rows 32..39 (replace), sequence 1: rows 7..14 (crosses no page end... 7..14 stays in page 0)
+    kp2, vp2 = O.cache_write_block(kp, vp, pt, pos, k_new, v_new)
+    for b in range(2):
+        for h in range(2):
+            rows = O.cached_rows(kp2, pt, b, w.seq_lens[b], h)
+            old = O.cached_rows(kp, pt, b, w.seq_lens[b], h)
+            p0 = int(pos[b])
+            assert np.array_equal(rows[p0:p0 + 8], k_new[b, :, h])                       # what was written is read back
+            assert np.array_equal(rows[:p0], old[:p0]) and np.array_equal(rows[p0 + 8:], old[p0 + 8:])   # nothing else moved
+            assert np.array_equal(O.cached_rows(vp2, pt, b, w.seq_lens[b], h)[p0:p0 + 8], v_new[b, :, h])
+    touched = np.unique(np.nonzero((kp2 != kp).any(axis=(1, 2, 3)))[0])
+    assert set(touched) <= {int(pt[0, 2]), int(pt[1, 0])}                                 # only the pages that hold those rows
+
+
+def test_pool_append_block_then_attention_sees_the_rows():
+    q, kb, vb, pk, pv, pl = _attn_inputs(42, batch=1, B=4, Hq=2, Hkv=1, n=(3, 0), cap=12)
+    pk2, pv2, pl2 = O.pool_append_block(pk, pv, pl, kb, vb)
+    assert pl2.tolist() == [[7]] and np.array_equal(pk2[0, 0, 3:7], kb[0, :, 0]) and np.array_equal(pk2[0, 0, :3], pk[0, 0, :3])
+    # attention over (pool + appended block) with an EMPTY in-block set == attention over pool with that block in-block
+    ref, _ = O.sparse_attn(q, kb, vb, pk, pv, pl, 0.2)
+    K = np.concatenate([O.bf16_bits_to_f64(pk2[0, 0, :7])]); V = O.bf16_bits_to_f64(pv2[0, 0, :7])
+    for hq in range(2):
+        logits = 0.2 * O.bf16_bits_to_f64(q[0, :, hq]) @ K.T
+        p = np.exp(logits - logits.max(axis=1, keepdims=True)); p /= p.sum(axis=1, keepdims=True)
+        assert np.allclose(ref[0, :, hq], p @ V, atol=1e-6)
