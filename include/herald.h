@@ -153,6 +153,19 @@ size_t herald_rep_attn_workspace_bytes(const herald_shape_t* shape);
 int herald_rep_attn(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep, float* out, float* lse,
                     void* ws, size_t ws_bytes, herald_stream_t stream);
 
+/* Block-boundary cache operations.
+ * herald_cache_write_block: K[b, write_pos[b] + i, h, :] = k_new[b][i][h][:] for i < block_size (same for V), through
+ *   the page table -- appends the rows of a block (the draft KV, "appended temporarily" to the full KV pool,
+ *   PAPER.md:189) or replaces rows already there (the true KV "replacing the draft").  The pages must be
+ *   mapped; seq_lens is the caller's to advance.  write_pos int32 [batch] (device); k_new / v_new bf16
+ *   [batch][B][H_kv][128].  Bit copies.  The cache pages are written: pass them non-const in `cache`.
+ * herald_pool_append_block: pool[b][h][pool_len[b][h] + i][:] = k_new[b][i][h][:], then pool_len[b][h] += B (clamped to
+ *   pool_capacity): the completed block joins block n+1's pool (reading 10). */
+int herald_cache_write_block(const herald_shape_t* shape, const herald_cache_t* cache, const int32_t* write_pos,
+                             const void* k_new, const void* v_new, herald_stream_t stream);
+int herald_pool_append_block(const herald_shape_t* shape, void* pool_k, void* pool_v, int32_t* pool_len,
+                             const void* k_new, const void* v_new, herald_stream_t stream);
+
 /* Per-layer state of the dual-stream block step.  Host POD holding device pointers. */
 typedef struct herald_layer {
     herald_cache_t cache;      /* this layer's full KV pool                                                   */

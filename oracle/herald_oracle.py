@@ -23,7 +23,7 @@ Data conventions (same as include/herald.h, but HOST NumPy arrays):
   * query head ``hq`` belongs to KV head ``hq // G`` with ``G = H_q // H_kv``
     (section IV-B4: "G is the number of query heads that share one KV head under GQA").
 
-Pin status (see tests/test_oracle_pins.py, all ``-m "not gpu"``; ``rep_attn`` included): every function
+Pin status (see tests/test_oracle_pins.py, all ``-m "not gpu"``; ``rep_attn``, ``cache_write_block`` and ``pool_append_block`` included): every function
 below is pinned against something other than itself -- closed forms, brute
 force pure-Python loops, library SDPA / softmax, invariants.  No function is
 "parity unpinned".

@@ -9,6 +9,7 @@
 
 #include "attn_tc.cuh"
 #include "common.cuh"
+#include "cache_ops.cuh"
 #include "gather.cuh"
 #include "rep_attn.cuh"
 #include "scan.cuh"
@@ -580,6 +581,65 @@ int herald_dense_attn(const herald_shape_t* shape, const herald_cache_t* cache, 
     rc = check_cache(cache, true);
     if (rc) return rc;
     return sparse_attn_impl(shape, cache->k_pages, cache->v_pages, nullptr, q_blk, k_blk, v_blk, out, lse, ws, ws_bytes, stream_, nullptr, cache);
+}
+
+int herald_cache_write_block(const herald_shape_t* shape, const herald_cache_t* cache, const int32_t* write_pos,
+                             const void* k_new, const void* v_new, herald_stream_t stream_) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    rc = check_cache(cache, true);
+    if (rc) return rc;
+    if (!write_pos || !k_new || !v_new) return fail(HERALD_ERR_INVALID_ARG, "herald_cache_write_block: NULL pointer");
+    if (!aligned16(k_new) || !aligned16(v_new)) return fail(HERALD_ERR_INVALID_ARG, "herald_cache_write_block: misaligned pointer");
+    const int rows = shape->batch * shape->block_size * shape->n_kv_heads;
+    if (rows == 0) return HERALD_OK;
+    g_err[0] = 0;
+    CacheWriteParams cp{};
+    cp.k_pages = static_cast<__nv_bfloat16*>(const_cast<void*>(cache->k_pages));
+    cp.v_pages = static_cast<__nv_bfloat16*>(const_cast<void*>(cache->v_pages));
+    cp.page_stride = cache->page_stride;
+    cp.token_stride = cache->token_stride;
+    cp.head_stride = cache->head_stride;
+    cp.page_table = cache->page_table;
+    cp.write_pos = write_pos;
+    cp.k_new = static_cast<const __nv_bfloat16*>(k_new);
+    cp.v_new = static_cast<const __nv_bfloat16*>(v_new);
+    cp.batch = shape->batch;
+    cp.block_size = shape->block_size;
+    cp.n_kv_heads = shape->n_kv_heads;
+    cp.max_pages = shape->max_pages_per_seq;
+    int grid = (rows + 15) / 16;
+    if (grid > 4 * sm_count()) grid = 4 * sm_count();
+    cache_write_block_kernel<<<grid, 256, 0, static_cast<cudaStream_t>(stream_)>>>(cp);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "cache_write_block launch");
+    return HERALD_OK;
+}
+
+int herald_pool_append_block(const herald_shape_t* shape, void* pool_k, void* pool_v, int32_t* pool_len, const void* k_new,
+                             const void* v_new, herald_stream_t stream_) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    if (!pool_k || !pool_v || !pool_len || !k_new || !v_new) return fail(HERALD_ERR_INVALID_ARG, "herald_pool_append_block: NULL pointer");
+    if (!aligned16(pool_k) || !aligned16(pool_v) || !aligned16(k_new) || !aligned16(v_new))
+        return fail(HERALD_ERR_INVALID_ARG, "herald_pool_append_block: misaligned pointer");
+    const int units = shape->batch * shape->n_kv_heads;
+    if (units == 0 || shape->pool_capacity == 0) return HERALD_OK;
+    g_err[0] = 0;
+    PoolAppendParams pp{};
+    pp.pool_k = static_cast<__nv_bfloat16*>(pool_k);
+    pp.pool_v = static_cast<__nv_bfloat16*>(pool_v);
+    pp.pool_len = pool_len;
+    pp.k_new = static_cast<const __nv_bfloat16*>(k_new);
+    pp.v_new = static_cast<const __nv_bfloat16*>(v_new);
+    pp.batch = shape->batch;
+    pp.block_size = shape->block_size;
+    pp.n_kv_heads = shape->n_kv_heads;
+    pp.cap = shape->pool_capacity;
+    pool_append_block_kernel<<<units, 256, 0, static_cast<cudaStream_t>(stream_)>>>(pp);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "pool_append_block launch");
+    return HERALD_OK;
 }
 
 static int rep_chunks(const herald_shape_t* s) {

@@ -26,6 +26,7 @@ AGG_MAX_LOGIT, AGG_SOFTMAX_SUM = 0, 1
 EXPORTS = ("herald_last_error", "herald_budget_rows", "herald_select_workspace_bytes",
            "herald_attn_workspace_bytes", "herald_attn_grid_ctas", "herald_select", "herald_gather", "herald_sparse_attn",
            "herald_dense_attn", "herald_rep_attn_workspace_bytes", "herald_rep_attn",
+           "herald_cache_write_block", "herald_pool_append_block",
            "herald_pipeline_step", "herald_pipeline_step_host", "herald_pipeline_set_profile")
 
 
@@ -100,6 +101,10 @@ _lib.herald_rep_attn_workspace_bytes.argtypes = [C.POINTER(Shape)]
 _lib.herald_rep_attn.restype = C.c_int
 _lib.herald_rep_attn.argtypes = [C.POINTER(Shape), C.POINTER(Cache), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t,
                                  C.c_void_p]
+_lib.herald_cache_write_block.restype = C.c_int
+_lib.herald_cache_write_block.argtypes = [C.POINTER(Shape), C.POINTER(Cache), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.herald_pool_append_block.restype = C.c_int
+_lib.herald_pool_append_block.argtypes = [C.POINTER(Shape)] + [C.c_void_p] * 6
 _lib.herald_pipeline_step.restype = C.c_int
 _lib.herald_pipeline_step.argtypes = [C.POINTER(Pipeline)]
 _lib.herald_pipeline_step_host.restype = C.c_int
@@ -203,6 +208,15 @@ def herald_rep_attn(shape, cache, q_rep, out, lse, ws, stream=None):
     ws_ptr, ws_bytes = _ws(ws)
     _check(_lib.herald_rep_attn(C.byref(shape), C.byref(cache), _ptr(q_rep), _ptr(out), _ptr(lse), ws_ptr, ws_bytes,
                                 _stream(stream)))
+
+
+def herald_cache_write_block(shape, cache, write_pos, k_new, v_new, stream=None):
+    _check(_lib.herald_cache_write_block(C.byref(shape), C.byref(cache), _ptr(write_pos), _ptr(k_new), _ptr(v_new), _stream(stream)))
+
+
+def herald_pool_append_block(shape, pool_k, pool_v, pool_len, k_new, v_new, stream=None):
+    _check(_lib.herald_pool_append_block(C.byref(shape), _ptr(pool_k), _ptr(pool_v), _ptr(pool_len), _ptr(k_new), _ptr(v_new),
+                                         _stream(stream)))
 
 
 def herald_pipeline_step(pipe: Pipeline):

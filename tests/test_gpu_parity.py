@@ -499,3 +499,41 @@ def test_rep_attn_matches_oracle(H, cuda, case):
     assert np.abs(got - ref).max() <= 1e-4, (case, np.abs(got - ref).max())     # fp32 P and accumulation: no bf16 rounding of P here
     fin = np.isfinite(lse_ref)
     assert np.array_equal(np.isneginf(got_lse), ~fin) and np.abs(got_lse[fin] - lse_ref[fin]).max() <= 1e-3
+
+
+def test_block_boundary_cache_ops_are_bit_exact(H, cuda):
+    """herald_cache_write_block (draft rows appended to / true rows replacing the tail of the paged cache)
+    and herald_pool_append_block (the completed block joins the next pool) against the oracle, bit for bit."""
+    w = synth.Workload("cw", 3, (300, 77, 4096), 28, 4, 32, 2, 100, "plain")
+    inp = synth.make_inputs(w, seed=700, device=cuda, spare_pages=3)
+    B, Hkv = w.block_size, w.n_kv_heads
+    shape = H.make_shape(w.batch, w.n_q_heads, Hkv, B, 4096, inp["page_table"].shape[1], 600)
+    cache = H.make_cache(inp["k_pages"], inp["v_pages"], inp["page_table"], inp["seq_lens"])
+    g = torch.Generator(device=cuda)
+    g.manual_seed(1)
+    k_new = torch.randn((w.batch, B, Hkv, 128), generator=g, device=cuda).to(torch.bfloat16)
+    v_new = torch.randn((w.batch, B, Hkv, 128), generator=g, device=cuda).to(torch.bfloat16)
+    pos = [300 - B, 77 - B - 5, 4096 - B]                # rows that exist (the block is the tail of the sequence, or inside it)
+    write_pos = torch.tensor(pos, dtype=torch.int32, device=cuda)
+    oi = oracle_inputs(inp)
+    kp_o, vp_o = O.cache_write_block(oi["k_pages"], oi["v_pages"], oi["page_table"], pos, synth.to_u16(k_new), synth.to_u16(v_new))
+    H.herald_cache_write_block(shape, cache, write_pos, k_new, v_new)
+    torch.cuda.synchronize()
+    assert np.array_equal(synth.to_u16(inp["k_pages"]), kp_o) and np.array_equal(synth.to_u16(inp["v_pages"]), vp_o)
+    # pool append, one unit already at capacity - B + 3 (the last 3 rows do not fit: dropped, length clamps)
+    cap = shape.pool_capacity
+    canary = 0x7FC1
+    pk = torch.full((w.batch, Hkv, cap, 128), canary, dtype=torch.int16, device=cuda).view(torch.bfloat16)
+    pv = torch.full((w.batch, Hkv, cap, 128), canary, dtype=torch.int16, device=cuda).view(torch.bfloat16)
+    lens = [[0, 5, 100, cap - B], [17, 17, 17, 17], [cap - B, 1, 2, 3]]
+    pl = torch.tensor(lens, dtype=torch.int32, device=cuda)
+    pk_o, pv_o, pl_o = O.pool_append_block(synth.to_u16(pk), synth.to_u16(pv), np.array(lens), synth.to_u16(k_new), synth.to_u16(v_new))
+    H.herald_pool_append_block(shape, pk, pv, pl, k_new, v_new)
+    torch.cuda.synchronize()
+    assert np.array_equal(pl.cpu().numpy(), pl_o)
+    assert np.array_equal(synth.to_u16(pk), pk_o) and np.array_equal(synth.to_u16(pv), pv_o)     # canaries included
+    pl2 = torch.full((w.batch, Hkv), cap - B + 3, dtype=torch.int32, device=cuda)
+    H.herald_pool_append_block(shape, pk, pv, pl2, k_new, v_new)
+    torch.cuda.synchronize()
+    assert (pl2 == cap).all()
+    assert np.array_equal(synth.to_u16(pk)[0, 0, cap - B + 3:], synth.to_u16(k_new)[0, :B - 3, 0])
