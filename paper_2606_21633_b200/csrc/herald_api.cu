@@ -686,8 +686,14 @@ int herald_rep_attn(const herald_shape_t* shape, const herald_cache_t* cache, co
     rp.max_pages = shape->max_pages_per_seq;
     rp.n_chunks = rep_chunks(shape);
     rp.scale_log2 = shape->sm_scale * 1.4426950408889634f;
-    rep_attn_kernel<<<dim3(rp.n_chunks, units), kRepThreads, 0, stream>>>(rp);
-    rep_attn_merge_kernel<<<units, kHeadDim, 0, stream>>>(rp);
+    const dim3 rgrid(rp.n_chunks, units);
+    static thread_local bool rep_attr_set = false;   // over the 48 KB default: opt in once
+    if (!rep_attr_set) {
+        cudaFuncSetAttribute(rep_attn_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kRepSmemBytes);
+        rep_attr_set = true;
+    }
+    rep_attn_kernel<<<rgrid, kRepThreads, kRepSmemBytes, stream>>>(rp);
+    rep_attn_merge_kernel<<<units, dim3(kHeadDim, shape->n_q_heads / shape->n_kv_heads), 0, stream>>>(rp);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "rep_attn launch");
     return HERALD_OK;

@@ -6,11 +6,15 @@
 //
 // One query row per head: there is no dense contraction to give to tcgen05 (M = G <= 8), and the kernel is a second
 // HBM stream, now over K AND V (512 B per token and KV head).  Scores come from the same mma.sync trick as the score
-// scan (16 tokens x 16 channels x 8 heads per MMA, fed from 128-bit global loads); the P.V product is G x 128 FMAs per
-// token on the CUDA cores with each lane owning 4 channels, p broadcast from shared memory.
+// scan (fed from 128-bit global loads); the P.V product runs on mma.sync too (G x 128 FMAs per token on the CUDA cores
+// made the kernel FMA-pipe bound at G = 7), in the transposed form described at the kernel.
 //   grid = (chunks of kRepChunkTokens tokens, units); 8 warps stride over the pages of their chunk with an online
 //   softmax per warp; warps merge in shared memory; one partial (m, l, o) per (unit, chunk) goes to the workspace and
 //   rep_attn_merge_kernel combines the chunks of a unit.
+//   Each warp keeps its NEXT page in flight while it works on the current one: the K fragments of page i+1 are loaded
+//   into the fragment registers as soon as the score MMAs of page i have consumed them, and the V rows of page i+1 go
+//   by cp.async into the other half of a per-warp double buffer (2 x 4 KB).  Without that each page costs a warp one
+//   exposed DRAM round trip and the kernel is latency-bound.
 #pragma once
 #include "common.cuh"
 
@@ -20,6 +24,17 @@ constexpr int kRepThreads = 256;
 constexpr int kRepWarps = kRepThreads / 32;
 constexpr int kRepChunkTokens = 2048;                 // tokens per CTA (128 pages)
 constexpr int kRepPartFloats = 8 * (kHeadDim + 2);    // per (unit, chunk): 8 head slots x (128 channels, m, l)
+constexpr int kRepVStageBytes = kPageSize * kHeadDim * 2;                 // one page of V rows of one head: 4 KB
+constexpr int kRepSmemV = kRepWarps * 2 * kRepVStageBytes;                 // V double buffers; reused as s_o after the loop
+constexpr int kRepSmemBytes = kRepSmemV;
+static_assert(kRepWarps * 8 * (kHeadDim + 4) * 4 <= kRepSmemV, "s_o must fit in the V stages it reuses");
+
+__device__ __forceinline__ void cp_async_16(uint32_t dst, const void* src, uint32_t src_bytes) {   // src_bytes 0: zero fill
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 struct RepAttnParams {
     const __nv_bfloat16* k_pages;
@@ -35,9 +50,21 @@ struct RepAttnParams {
     float scale_log2;     // sm_scale * log2(e): the softmax runs in base 2
 };
 
+__device__ __forceinline__ void ldmatrix_x4_trans(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
+                 : "r"(addr));
+}
+
+// Both products run TRANSPOSED on mma.sync so that the weights never leave the registers:
+//   S^T[head, token]   = Q[head, :] . K[token, :]      A = Q (rows 8..15 zero), B = K fragments straight from global
+//   O^T[channel, head] += V^T[channel, token] P^T[token, head]
+// The accumulator of the first product (head g; tokens 2tig, 2tig+1, 8+2tig, 9+2tig) IS the B fragment of the second
+// once exponentiated and packed; V^T comes from ldmatrix.trans on the V rows staged in shared memory (16-byte columns
+// XOR-swizzled by the row).  P goes in as a bf16 pair hi + lo (two MMAs): the weights keep ~16 mantissa bits.
 __global__ void __launch_bounds__(kRepThreads, 2) rep_attn_kernel(const RepAttnParams p) {
-    __shared__ __align__(16) float s_p[kRepWarps][16][8];       // this page's weights of each warp: [token][head]
-    __shared__ __align__(16) float s_o[kRepWarps][8][kHeadDim + 4];   // per-warp results for the merge (rows of 528 B: float4 stores)
+    extern __shared__ __align__(128) unsigned char rep_smem[];
+    float (*s_o)[8][kHeadDim + 4] = reinterpret_cast<float (*)[8][kHeadDim + 4]>(rep_smem);   // per-warp results for the merge (rows of 528 B), over the V stages
     const int chunk = blockIdx.x, unit = blockIdx.y;
     const int b = unit / p.n_kv_heads, h = unit % p.n_kv_heads;
     const int G = p.n_q_heads / p.n_kv_heads;
@@ -51,123 +78,135 @@ __global__ void __launch_bounds__(kRepThreads, 2) rep_attn_kernel(const RepAttnP
         return;
     }
 
-    uint4 qf[4];              // B operand of the score MMA: query head g (zeros for g >= G), channel-permuted like A
+    uint4 qf[4];              // A operand of the score MMA: query head g (zeros for g >= G), channel-permuted like K
     {
         const __nv_bfloat16* qrow = p.q_rep + ((int64_t)b * p.n_q_heads + h * G + g) * kHeadDim + 8 * tig;
 #pragma unroll
         for (int i = 0; i < 4; ++i) qf[i] = (g < G) ? ldg_u4(qrow + 32 * i) : make_uint4(0, 0, 0, 0);
     }
-    float m_run[8], l_run[8], o[8][4];     // online softmax of this warp, per head; lane owns channels [4*lane, 4*lane+4)
+    // online softmax of this warp: the lane keeps head g's running maximum (equal in the 4 lanes of a head) and its
+    // share of the row sum; o[c] = O^T[channels 16c+g, 16c+g+8][heads 2tig, 2tig+1]
+    float m_run = -INFINITY, l_run = 0.f, o[8][4];
 #pragma unroll
-    for (int q = 0; q < 8; ++q) {
-        m_run[q] = -INFINITY;
-        l_run[q] = 0.f;
+    for (int c = 0; c < 8; ++c) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) o[q][c] = 0.f;
+        for (int j = 0; j < 4; ++j) o[c][j] = 0.f;
     }
 
     const int32_t* pt = p.page_table + (int64_t)b * p.max_pages;
     const int page_end = (t_end + kPageSize - 1) / kPageSize;
-    for (int page = t_begin / kPageSize + warp; page < page_end; page += kRepWarps) {
-        const int phys = __ldg(pt + page);
+    const uint32_t v_stage = smem_u32(rep_smem + warp * 2 * kRepVStageBytes);
+    // ldmatrix row address of this lane inside a stage, for channel tile 0: matrix j = lane/8 is (tokens 8(j/2).., 16-byte
+    // column j%2), row lane%8; the column index is XORed with (token & 7) = lane%8
+    const int lm_tok = (lane & 7) + 8 * (lane >> 4), lm_col = (lane >> 3) & 1;
+    uint4 a[4], c[4];         // K fragments (as in the score scan) of the page in flight: token rows g and g+8
+    // issue the loads of one page: K fragments into (a, c), V rows into stage `st` (rows past t_end zero-filled: their
+    // weight is 0, but 0 x NaN of an unwritten cache slot is NaN)
+    auto issue_page = [&](int pg, int phys, int st) {
         const int64_t tile = (int64_t)phys * p.page_stride + (int64_t)h * p.head_stride;
-        // K fragments (as in the score scan) and the V rows of the page: lane reads 8 bytes (4 channels) of each of the 16 rows
         const __nv_bfloat16* r0 = p.k_pages + tile + (int64_t)g * p.token_stride + 8 * tig;
         const __nv_bfloat16* r1 = p.k_pages + tile + (int64_t)(g + 8) * p.token_stride + 8 * tig;
-        uint4 a[4], c[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             a[i] = ldg_stream_u4(r0 + 32 * i);
             c[i] = ldg_stream_u4(r1 + 32 * i);
         }
-        uint2 v[16];
 #pragma unroll
-        for (int t = 0; t < 16; ++t)
-            v[t] = __ldg(reinterpret_cast<const uint2*>(p.v_pages + tile + (int64_t)t * p.token_stride + 4 * lane));
-        float acc[4] = {0.f, 0.f, 0.f, 0.f};
+        for (int j = 0; j < 8; ++j) {            // 256 x 16 B: row = 2j + lane/16, 16-byte column = lane % 16
+            const int row = 2 * j + (lane >> 4), col = lane & 15;
+            cp_async_16(v_stage + st * kRepVStageBytes + row * (kHeadDim * 2) + ((col ^ (row & 7)) << 4),
+                        p.v_pages + tile + (int64_t)row * p.token_stride + 8 * col, pg * kPageSize + row < t_end ? 16u : 0u);
+        }
+    };
+    int page = t_begin / kPageSize + warp;
+    int phys_next = 0;
+    if (page < page_end) {
+        issue_page(page, __ldg(pt + page), 0);
+        if (page + kRepWarps < page_end) phys_next = __ldg(pt + page + kRepWarps);
+    }
+    cp_async_commit();
+    for (int st = 0; page < page_end; page += kRepWarps, st ^= 1) {
+        float sa[4] = {0.f, 0.f, 0.f, 0.f}, sb[4] = {0.f, 0.f, 0.f, 0.f};   // tokens 0..7 / 8..15 of the page
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-            mma_bf16_16816(acc, a[i].x, c[i].x, a[i].y, c[i].y, qf[i].x, qf[i].y);
-            mma_bf16_16816(acc, a[i].z, c[i].z, a[i].w, c[i].w, qf[i].z, qf[i].w);
+            mma_bf16_16816(sa, qf[i].x, 0u, qf[i].y, 0u, a[i].x, a[i].y);
+            mma_bf16_16816(sa, qf[i].z, 0u, qf[i].w, 0u, a[i].z, a[i].w);
+            mma_bf16_16816(sb, qf[i].x, 0u, qf[i].y, 0u, c[i].x, c[i].y);
+            mma_bf16_16816(sb, qf[i].z, 0u, qf[i].w, 0u, c[i].z, c[i].w);
         }
-#pragma unroll
-        for (int t = 0; t < 16; ++t)
-            if (page * kPageSize + t >= t_end) v[t] = make_uint2(0u, 0u);   // tail slots of the last page: weight 0, but 0 x NaN
-        // acc[0],acc[1]: token row g, heads 2*tig, 2*tig+1 ; acc[2],acc[3]: token row g+8.  Mask the tail of the last page.
-        const int t0 = page * kPageSize;
-        const bool ok0 = t0 + g < t_end, ok1 = t0 + g + 8 < t_end;
-        float s0 = ok0 ? acc[0] * p.scale_log2 : -INFINITY, s1 = ok0 ? acc[1] * p.scale_log2 : -INFINITY;
-        float s2 = ok1 ? acc[2] * p.scale_log2 : -INFINITY, s3 = ok1 ? acc[3] * p.scale_log2 : -INFINITY;
-        // page maximum per head: over this lane's two rows, then over the 8 row groups (lanes with equal tig)
-        float mx0 = fmaxf(s0, s2), mx1 = fmaxf(s1, s3);
-#pragma unroll
-        for (int off = 4; off < 32; off <<= 1) {
-            mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, off));
-            mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, off));
+        // the fragments are consumed: put the next page of this warp in flight
+        if (page + kRepWarps < page_end) {
+            issue_page(page + kRepWarps, phys_next, st ^ 1);
+            if (page + 2 * kRepWarps < page_end) phys_next = __ldg(pt + page + 2 * kRepWarps);
         }
-        // every lane needs the maxima of all 8 head slots: lane tig' holds heads 2tig', 2tig'+1
-        float m_new[8], alpha[8];
+        cp_async_commit();
+        // sa[0], sa[1]: head g, tokens 2tig, 2tig+1 ; sb[0], sb[1]: tokens 8+2tig, 9+2tig.  Mask the tail of the last page.
+        const int t0 = page * kPageSize + 2 * tig;
+        const bool ok0 = t0 < t_end, ok1 = t0 + 1 < t_end, ok2 = t0 + 8 < t_end, ok3 = t0 + 9 < t_end;
+        const float s0 = ok0 ? sa[0] * p.scale_log2 : -INFINITY, s1 = ok1 ? sa[1] * p.scale_log2 : -INFINITY;
+        const float s2 = ok2 ? sb[0] * p.scale_log2 : -INFINITY, s3 = ok3 ? sb[1] * p.scale_log2 : -INFINITY;
+        float mx = fmaxf(fmaxf(s0, s1), fmaxf(s2, s3));     // page maximum of head g: 4 values here, 4 lanes per head
+        mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 1));
+        mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 2));
+        const float m_new = fmaxf(m_run, mx);               // finite: token 0 of the page is valid
+        const float alpha = (m_run == -INFINITY) ? 0.f : fast_exp2(m_run - m_new);
+        m_run = m_new;
+        const float p0 = ok0 ? fast_exp2(s0 - m_new) : 0.f, p1 = ok1 ? fast_exp2(s1 - m_new) : 0.f;
+        const float p2 = ok2 ? fast_exp2(s2 - m_new) : 0.f, p3 = ok3 ? fast_exp2(s3 - m_new) : 0.f;
+        l_run = l_run * alpha + ((p0 + p1) + (p2 + p3));
+        const uint32_t h01 = pack_bf16(p0, p1), h23 = pack_bf16(p2, p3);
+        const uint32_t l01 = pack_bf16(p0 - __uint_as_float(h01 << 16), p1 - __uint_as_float(h01 & 0xffff0000u));
+        const uint32_t l23 = pack_bf16(p2 - __uint_as_float(h23 << 16), p3 - __uint_as_float(h23 & 0xffff0000u));
+        if (__any_sync(0xffffffffu, alpha != 1.f)) {        // a maximum moved: rescale (heads 2tig, 2tig+1 live in lanes 8tig, 8tig+4)
+            const float a0 = __shfl_sync(0xffffffffu, alpha, 8 * tig), a1 = __shfl_sync(0xffffffffu, alpha, 8 * tig + 4);
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const float e0 = __shfl_sync(0xffffffffu, mx0, q), e1 = __shfl_sync(0xffffffffu, mx1, q);
-            m_new[2 * q] = fmaxf(m_run[2 * q], e0);
-            m_new[2 * q + 1] = fmaxf(m_run[2 * q + 1], e1);
-        }
-#pragma unroll
-        for (int q = 0; q < 8; ++q) {
-            alpha[q] = (m_run[q] == -INFINITY) ? 0.f : fast_exp2(m_run[q] - m_new[q]);
-            m_run[q] = m_new[q];
-        }
-        // weights of this lane's four (token, head) pairs -> shared memory (the page has a valid token, so m_new of a
-        // real head is finite; head slots >= G carry zeros throughout)
-        const float mh0 = m_new[2 * tig], mh1 = m_new[2 * tig + 1];
-        __syncwarp();
-        s_p[warp][g][2 * tig] = (2 * tig < G && ok0) ? fast_exp2(s0 - mh0) : 0.f;
-        s_p[warp][g][2 * tig + 1] = (2 * tig + 1 < G && ok0) ? fast_exp2(s1 - mh1) : 0.f;
-        s_p[warp][g + 8][2 * tig] = (2 * tig < G && ok1) ? fast_exp2(s2 - mh0) : 0.f;
-        s_p[warp][g + 8][2 * tig + 1] = (2 * tig + 1 < G && ok1) ? fast_exp2(s3 - mh1) : 0.f;
-        __syncwarp();
-#pragma unroll
-        for (int q = 0; q < 8; ++q) {
-            l_run[q] *= alpha[q];
-#pragma unroll
-            for (int cc = 0; cc < 4; ++cc) o[q][cc] *= alpha[q];
-        }
-#pragma unroll
-        for (int t = 0; t < 16; ++t) {
-            const float4 pa = *reinterpret_cast<const float4*>(&s_p[warp][t][0]);
-            const float4 pb = *reinterpret_cast<const float4*>(&s_p[warp][t][4]);
-            const float pw[8] = {pa.x, pa.y, pa.z, pa.w, pb.x, pb.y, pb.z, pb.w};
-            const float vf[4] = {__uint_as_float(v[t].x << 16), __uint_as_float(v[t].x & 0xffff0000u),
-                                 __uint_as_float(v[t].y << 16), __uint_as_float(v[t].y & 0xffff0000u)};
-#pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                l_run[q] += pw[q];
-#pragma unroll
-                for (int cc = 0; cc < 4; ++cc) o[q][cc] = fmaf(pw[q], vf[cc], o[q][cc]);
+            for (int cc = 0; cc < 8; ++cc) {
+                o[cc][0] *= a0;
+                o[cc][1] *= a1;
+                o[cc][2] *= a0;
+                o[cc][3] *= a1;
             }
         }
+        cp_async_wait<1>();       // this page's V rows (every group but the one just committed)
+        __syncwarp();
+        const uint32_t lm_base = v_stage + st * kRepVStageBytes + lm_tok * (kHeadDim * 2);
+#pragma unroll
+        for (int cc = 0; cc < 8; ++cc) {                    // channels [16cc, 16cc+16)
+            uint32_t v0, v1, v2, v3;
+            ldmatrix_x4_trans(lm_base + (((2 * cc + lm_col) ^ (lane & 7)) << 4), v0, v1, v2, v3);
+            mma_bf16_16816(o[cc], v0, v1, v2, v3, h01, h23);
+            mma_bf16_16816(o[cc], v0, v1, v2, v3, l01, l23);
+        }
+        __syncwarp();             // the stage is refilled two pages from now
     }
+    cp_async_wait<0>();
+    __syncthreads();              // s_o lies over the V stages of every warp
 
     // ---- merge the warps of the CTA, write the chunk's partial ----
+    l_run += __shfl_xor_sync(0xffffffffu, l_run, 1);
+    l_run += __shfl_xor_sync(0xffffffffu, l_run, 2);
+    if (tig == 0) {
+        s_o[warp][g][kHeadDim] = m_run;
+        s_o[warp][g][kHeadDim + 1] = l_run;
+    }
 #pragma unroll
-    for (int q = 0; q < 8; ++q) {
-        *reinterpret_cast<float4*>(&s_o[warp][q][4 * lane]) = make_float4(o[q][0], o[q][1], o[q][2], o[q][3]);
-        if (lane == 0) {
-            s_o[warp][q][kHeadDim] = m_run[q];
-            s_o[warp][q][kHeadDim + 1] = l_run[q];
-        }
+    for (int cc = 0; cc < 8; ++cc) {
+        s_o[warp][2 * tig][16 * cc + g] = o[cc][0];
+        s_o[warp][2 * tig + 1][16 * cc + g] = o[cc][1];
+        s_o[warp][2 * tig][16 * cc + g + 8] = o[cc][2];
+        s_o[warp][2 * tig + 1][16 * cc + g + 8] = o[cc][3];
     }
     __syncthreads();
     for (int idx = threadIdx.x; idx < 8 * kHeadDim; idx += kRepThreads) {
         const int q = idx >> 7, ch = idx & (kHeadDim - 1);
         float ms = -INFINITY;
+#pragma unroll
         for (int wv = 0; wv < kRepWarps; ++wv) ms = fmaxf(ms, s_o[wv][q][kHeadDim]);
         float num = 0.f, den = 0.f;
+#pragma unroll
         for (int wv = 0; wv < kRepWarps; ++wv) {
             const float mw = s_o[wv][q][kHeadDim];
-            if (mw == -INFINITY) continue;
-            const float wgt = fast_exp2(mw - ms);
+            const float wgt = (mw == -INFINITY) ? 0.f : fast_exp2(mw - ms);
             num += wgt * s_o[wv][q][ch];
             den += wgt * s_o[wv][q][kHeadDim + 1];
         }
@@ -179,27 +218,32 @@ __global__ void __launch_bounds__(kRepThreads, 2) rep_attn_kernel(const RepAttnP
     }
 }
 
-// out[b, hq, :] = sum_c 2^(m_c - m*) o_c / sum_c 2^(m_c - m*) l_c over the chunks of the unit; one block per unit.
-__global__ void __launch_bounds__(kHeadDim) rep_attn_merge_kernel(const RepAttnParams p) {
-    const int unit = blockIdx.x, ch = threadIdx.x;
+// out[b, hq, :] = sum_c 2^(m_c - m*) o_c / sum_c 2^(m_c - m*) l_c over the chunks of the unit; one block per unit,
+// blockDim = (128 channels, G heads).  The chunk loops carry no dependent loads (the kernel is a latency chain otherwise).
+__global__ void __launch_bounds__(kHeadDim * 8) rep_attn_merge_kernel(const RepAttnParams p) {
+    const int unit = blockIdx.x, ch = threadIdx.x, q = threadIdx.y;
     const int b = unit / p.n_kv_heads, h = unit % p.n_kv_heads;
     const int G = p.n_q_heads / p.n_kv_heads;
-    const float* part = p.part + (int64_t)unit * p.n_chunks * kRepPartFloats;
-    for (int q = 0; q < G; ++q) {
-        float ms = -INFINITY;
-        for (int c = 0; c < p.n_chunks; ++c) ms = fmaxf(ms, part[c * kRepPartFloats + q * (kHeadDim + 2) + kHeadDim]);
-        float num = 0.f, den = 0.f;
+    const float* part = p.part + (int64_t)unit * p.n_chunks * kRepPartFloats + q * (kHeadDim + 2);
+    float ms = -INFINITY;
+#pragma unroll 8
+    for (int c = 0; c < p.n_chunks; ++c) ms = fmaxf(ms, __ldg(part + c * kRepPartFloats + kHeadDim));
+    float num = 0.f, den = 0.f;
+    if (ms != -INFINITY) {
+#pragma unroll 8
         for (int c = 0; c < p.n_chunks; ++c) {
-            const float* pc = part + c * kRepPartFloats + q * (kHeadDim + 2);
-            if (pc[kHeadDim] == -INFINITY) continue;
-            const float wgt = fast_exp2(pc[kHeadDim] - ms);
-            num += wgt * pc[ch];
-            den += wgt * pc[kHeadDim + 1];
+            const float* pc = part + c * kRepPartFloats;
+            const float mc = __ldg(pc + kHeadDim);
+            const bool live = mc != -INFINITY;              // an empty chunk wrote only its m
+            const float wgt = live ? fast_exp2(mc - ms) : 0.f;
+            const float oc = live ? __ldg(pc + ch) : 0.f, lc = live ? __ldg(pc + kHeadDim + 1) : 0.f;
+            num += wgt * oc;
+            den += wgt * lc;
         }
-        const int64_t row = (int64_t)b * p.n_q_heads + h * G + q;
-        p.out[row * kHeadDim + ch] = den > 0.f ? num / den : 0.f;                       // no cached token: zeros
-        if (p.lse && ch == 0) p.lse[row] = den > 0.f ? (ms + log2f(den)) * 0.6931471805599453f : -INFINITY;
     }
+    const int64_t row = (int64_t)b * p.n_q_heads + h * G + q;
+    p.out[row * kHeadDim + ch] = den > 0.f ? num / den : 0.f;                           // no cached token: zeros
+    if (p.lse && ch == 0) p.lse[row] = den > 0.f ? (ms + log2f(den)) * 0.6931471805599453f : -INFINITY;
 }
 
 }  // namespace herald
