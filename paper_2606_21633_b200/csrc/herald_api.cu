@@ -642,15 +642,17 @@ int herald_pool_append_block(const herald_shape_t* shape, void* pool_k, void* po
     return HERALD_OK;
 }
 
-static int rep_chunks(const herald_shape_t* s) {
-    const int c = (s->max_seq_len + kRepChunkTokens - 1) / kRepChunkTokens;
-    return c > 0 ? c : 1;
+// herald_rep_attn takes hg KV heads of a page together: the largest of 8, 4, 2, 1 that divides H_kv
+static int rep_head_group(const herald_shape_t* s) {
+    for (int hg = 8; hg > 1; hg >>= 1)
+        if (s->n_kv_heads % hg == 0) return hg;
+    return 1;
 }
 
 size_t herald_rep_attn_workspace_bytes(const herald_shape_t* shape) {
     if (check_shape(shape) != HERALD_OK) return 0;
-    const size_t units = (size_t)shape->batch * shape->n_kv_heads;
-    return align_up((units > 0 ? units : 1) * rep_chunks(shape) * kRepPartFloats * sizeof(float), 256);
+    const size_t hg = rep_head_group(shape), groups = (size_t)shape->batch * (shape->n_kv_heads / hg);
+    return align_up((kRepMaxCtas + groups) * hg * kRepPartFloats * sizeof(float), 256);   // slot = cta + group, hg head partials each
 }
 
 int herald_rep_attn(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep, float* out, float* lse,
@@ -677,23 +679,24 @@ int herald_rep_attn(const herald_shape_t* shape, const herald_cache_t* cache, co
     rp.page_table = cache->page_table;
     rp.seq_lens = cache->seq_lens;
     rp.q_rep = static_cast<const __nv_bfloat16*>(q_rep);
+    rp.hg = rep_head_group(shape);
     rp.part = static_cast<float*>(ws);
+    rp.batch = shape->batch;
     rp.out = out;
     rp.lse = lse;
     rp.n_q_heads = shape->n_q_heads;
     rp.n_kv_heads = shape->n_kv_heads;
     rp.max_seq_len = shape->max_seq_len;
     rp.max_pages = shape->max_pages_per_seq;
-    rp.n_chunks = rep_chunks(shape);
     rp.scale_log2 = shape->sm_scale * 1.4426950408889634f;
-    const dim3 rgrid(rp.n_chunks, units);
+    const int n_ctas = std::min(2 * sm_count(), kRepMaxCtas);   // persistent: two CTAs per SM
     static thread_local bool rep_attr_set = false;   // over the 48 KB default: opt in once
     if (!rep_attr_set) {
         cudaFuncSetAttribute(rep_attn_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kRepSmemBytes);
         rep_attr_set = true;
     }
-    rep_attn_kernel<<<rgrid, kRepThreads, kRepSmemBytes, stream>>>(rp);
-    rep_attn_merge_kernel<<<units, dim3(kHeadDim, shape->n_q_heads / shape->n_kv_heads), 0, stream>>>(rp);
+    rep_attn_kernel<<<n_ctas, kRepThreads, kRepSmemBytes, stream>>>(rp);
+    rep_attn_merge_kernel<<<shape->batch * shape->n_q_heads, dim3(kHeadDim, kRepMergeSlices), 0, stream>>>(rp, n_ctas);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "rep_attn launch");
     return HERALD_OK;
