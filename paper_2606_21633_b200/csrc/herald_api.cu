@@ -696,8 +696,20 @@ int herald_rep_attn(const herald_shape_t* shape, const herald_cache_t* cache, co
         rep_attr_set = true;
     }
     rep_attn_kernel<<<n_ctas, kRepThreads, kRepSmemBytes, stream>>>(rp);
-    rep_attn_merge_kernel<<<shape->batch * shape->n_q_heads, dim3(kHeadDim, kRepMergeSlices), 0, stream>>>(rp, n_ctas);
     cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "rep_attn launch");
+    // the merge is launched programmatically behind the main grid: its blocks are scheduled as the main CTAs retire,
+    // find their partial list (inputs only) and wait (griddepcontrol.wait) for the grid to complete
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(shape->batch * shape->n_q_heads);
+    cfg.blockDim = dim3(kHeadDim, kRepMergeSlices);
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    e = cudaLaunchKernelEx(&cfg, rep_attn_merge_kernel, rp, n_ctas);
     if (e != cudaSuccess) return cuda_fail(e, "rep_attn launch");
     return HERALD_OK;
 }

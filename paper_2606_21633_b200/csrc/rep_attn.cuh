@@ -78,6 +78,7 @@ __global__ void __launch_bounds__(kRepThreads, 2) rep_attn_kernel(const RepAttnP
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = lane >> 2, tig = lane & 3;
     const int n_ctas = gridDim.x, cta = blockIdx.x;
+    asm volatile("griddepcontrol.launch_dependents;");       // the merge grid may be scheduled as this grid's CTAs retire
     const int hg = p.hg, n_groups = p.n_kv_heads / hg, n_slots = kRepWarps / hg;
     const int w_head = warp % hg, w_slot = warp / hg;         // this warp: head inside the group, first page slot
     if (threadIdx.x == 0) {
@@ -241,15 +242,17 @@ __global__ void __launch_bounds__(kRepThreads, 2) rep_attn_kernel(const RepAttnP
     }
 }
 
-constexpr int kRepMergeSlices = 8;
+constexpr int kRepMergeSlices = 4;
 
 // out[b, hq, :] = sum_c 2^(m_c - m*) o_c / sum_c 2^(m_c - m*) l_c over the partials c of the row's group; one block per
-// output row, blockDim = (128 channels, 8 slices of the partial list).  No load depends on another load except through
+// output row, blockDim = (128 channels, 4 slices of the partial list).  No load depends on another load except through
 // the row maximum, so the kernel is three short latency steps rather than a chain over the partials.
 __global__ void __launch_bounds__(kHeadDim * kRepMergeSlices) rep_attn_merge_kernel(const RepAttnParams p, int n_ctas) {
     __shared__ float s_w[kRepMaxCtas];
     __shared__ float s_red[kRepMergeSlices][kHeadDim + 1];
     __shared__ float s_max[32];
+    __shared__ int s_first, s_nparts;
+    __shared__ int64_t s_total;
     const int row = blockIdx.x, ch = threadIdx.x, slice = threadIdx.y, tid = slice * kHeadDim + ch;
     const int G = p.n_q_heads / p.n_kv_heads, hg = p.hg, n_groups = p.n_kv_heads / hg;
     const int b = row / p.n_q_heads, hq = row % p.n_q_heads, h = hq / G, q = hq % G, hgrp = h / hg, hh = h % hg;
@@ -259,15 +262,23 @@ __global__ void __launch_bounds__(kHeadDim * kRepMergeSlices) rep_attn_merge_ker
         if (p.lse && tid == 0) p.lse[row] = -INFINITY;
         return;
     }
-    int64_t total = 0, unit_begin = 0;
-    for (int bb = 0; bb < p.batch; ++bb) {
-        const int64_t np = (int64_t)((min(p.seq_lens[bb], p.max_seq_len) + kPageSize - 1) / kPageSize) * n_groups;
-        if (bb < b) unit_begin += np;
-        total += np;
+    if (tid == 0) {           // the row's partial list: one thread does the 64-bit divisions
+        int64_t total = 0, unit_begin = 0;
+        for (int bb = 0; bb < p.batch; ++bb) {
+            const int64_t np = (int64_t)((min(p.seq_lens[bb], p.max_seq_len) + kPageSize - 1) / kPageSize) * n_groups;
+            if (bb < b) unit_begin += np;
+            total += np;
+        }
+        unit_begin += (int64_t)hgrp * n_pages;
+        const int c_first = rep_cta_of(unit_begin, total, n_ctas);
+        s_first = c_first;
+        s_nparts = rep_cta_of(unit_begin + n_pages - 1, total, n_ctas) - c_first + 1;
+        s_total = total;
     }
-    unit_begin += (int64_t)hgrp * n_pages;
-    const int c_first = rep_cta_of(unit_begin, total, n_ctas), c_last = rep_cta_of(unit_begin + n_pages - 1, total, n_ctas);
-    const int n_parts = c_last - c_first + 1;
+    __syncthreads();
+    const int c_first = s_first, n_parts = s_nparts;
+    const int64_t total = s_total;
+    asm volatile("griddepcontrol.wait;" ::: "memory");        // launched programmatically: the partials are complete from here on
     const int group = b * n_groups + hgrp;
     const float* pq = p.part + ((int64_t)(c_first + group) * hg + hh) * kRepPartFloats + q * (kHeadDim + 2);
     const int64_t cstride = (int64_t)hg * kRepPartFloats;
@@ -275,7 +286,7 @@ __global__ void __launch_bounds__(kHeadDim * kRepMergeSlices) rep_attn_merge_ker
     float mx = -INFINITY;
     for (int c = tid; c < n_parts; c += kHeadDim * kRepMergeSlices) {
         const int cc = c_first + c;
-        const bool live = total * cc / n_ctas < total * (cc + 1) / n_ctas;
+        const bool live = total >= n_ctas || total * cc / n_ctas < total * (cc + 1) / n_ctas;   // with fewer pages than CTAs some ranges are empty
         const float m = live ? __ldcg(pq + c * cstride + kHeadDim) : -INFINITY;
         s_w[c] = m;
         mx = fmaxf(mx, m);
@@ -284,18 +295,19 @@ __global__ void __launch_bounds__(kHeadDim * kRepMergeSlices) rep_attn_merge_ker
     for (int off = 16; off; off >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, off));
     if ((tid & 31) == 0) s_max[tid >> 5] = mx;
     __syncthreads();
-    float ms = -INFINITY;
+    float ms = (tid & 31) < kHeadDim * kRepMergeSlices / 32 ? s_max[tid & 31] : -INFINITY;
 #pragma unroll
-    for (int i = 0; i < 32; ++i) ms = fmaxf(ms, s_max[i]);
+    for (int off = 16; off; off >>= 1) ms = fmaxf(ms, __shfl_xor_sync(0xffffffffu, ms, off));
     // 2. this thread's slice of the weighted sums
     float num = 0.f, den = 0.f;
-#pragma unroll 4
-    for (int c = slice; c < n_parts; c += kRepMergeSlices) {
+#pragma unroll 8
+    for (int c = slice; c < n_parts; c += kRepMergeSlices) {   // branch-free: the loads of all iterations go out together
         const float m = s_w[c];
-        if (m == -INFINITY) continue;
-        const float wgt = fast_exp2(m - ms);
-        num += wgt * __ldcg(pq + c * cstride + ch);
-        den += wgt * __ldcg(pq + c * cstride + kHeadDim + 1);
+        const bool live = m != -INFINITY;                    // an empty range's slot is unwritten memory
+        const float wgt = live ? fast_exp2(m - ms) : 0.f;
+        const float oc = live ? __ldcg(pq + c * cstride + ch) : 0.f, lc = live ? __ldcg(pq + c * cstride + kHeadDim + 1) : 0.f;
+        num += wgt * oc;
+        den += wgt * lc;
     }
     s_red[slice][ch] = num;
     if (ch == 0) s_red[slice][kHeadDim] = den;
