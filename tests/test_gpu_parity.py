@@ -470,6 +470,9 @@ REP_CASES = {
     "ragged_g7": (synth.Workload("rg7", 4, (5000, 2049, 16, 0), 28, 4, 32, 2, 50, "planted", 8), 2, True),
     "g8_h8": (synth.Workload("rg8", 2, (4096, 33), 64, 8, 16, 2, 50, "zipf"), 0, True),
     "g1": (synth.Workload("rg1", 2, (1, 700), 2, 2, 16, 2, 50, "plain"), 1, True),
+    # head groups of herald_rep_attn: H_kv = 6 -> two heads of a page per CTA, H_kv = 3 -> one; ranges that cross sequences
+    "h6_g2": (synth.Workload("rh6", 3, (3000, 0, 7001), 12, 6, 16, 2, 50, "zipf"), 1, True),
+    "h3_g5": (synth.Workload("rh3", 5, (17, 1500, 640, 31, 9000), 15, 3, 16, 2, 50, "planted", 8), 3, True),
 }
 
 
