@@ -25,8 +25,13 @@ Data conventions (same as include/herald.h, but HOST NumPy arrays):
 
 Pin status (see tests/test_oracle_pins.py, all ``-m "not gpu"``; ``rep_attn``, ``cache_write_block`` and ``pool_append_block`` included): every function
 below is pinned against something other than itself -- closed forms, brute
-force pure-Python loops, library SDPA / softmax, invariants.  No function is
-"parity unpinned".
+force pure-Python loops, library SDPA / softmax, invariants.  ``select_xq`` is
+"parity unpinned" AGAINST THE PAPER: PAPER.md:137 (Fig. 8) and :161 sweep the
+query count x of the selection kernel but never say how the x queries' scores
+combine into one ranking, so the function follows DESIGN.md reading 25 (the
+maximum over the x queries, as mode 0 takes it over the G heads); its
+arithmetic under that reading is pinned like the rest (x = 1 reduces to
+``select``, brute force loops, permutation and monotonicity invariants).
 """
 from __future__ import annotations
 
@@ -317,3 +322,32 @@ def pool_append_block(pool_k_u16, pool_v_u16, pool_len, k_new_u16, v_new_u16):
             pv[b, h, n:n + B] = v_new_u16[b, :, h]
             pl[b, h] = n + B
     return pk, pv, pl
+
+
+# ----------------------------------------------------------------------------
+# NEXT-4: selection with x queries  (PAPER.md:137 Fig. 8, :143, :161 -- parity unpinned against the paper, see header)
+# ----------------------------------------------------------------------------
+def select_xq(q_x_u16, k_pages_u16, page_table, seq_lens, k_per_seq, n_kv_heads, sm_scale):
+    """Selection scored by x queries per sequence instead of one ("B queries perform attention in GEMM
+    form"; :161: the cost "shrink[s] in proportion to the query count"; Fig. 8 sweeps x from B = 32 down to 1).
+
+    q_x_u16: [batch, x, H_q, d] bf16 bits.  DESIGN.md reading 25 (the paper does not define the combination):
+        a[t] = max over the x queries j and the G heads g of the group of  sm_scale * q_x[b, j, h*G+g] . K[b, t, h]
+    i.e. mode 0 of ``aggregate`` taken over all x*G score rows; then the same top-k.  Returns (sel, scores) like ``select``.
+    """
+    batch, x, H_q, d = q_x_u16.shape
+    G = H_q // n_kv_heads
+    assert G * n_kv_heads == H_q and x >= 1
+    sel, scores = [], []
+    for b in range(batch):
+        L = int(seq_lens[b])
+        sel_b, sc_b = [], []
+        for h in range(n_kv_heads):
+            k_rows = cached_rows(k_pages_u16, page_table, b, L, h)
+            rows = [raw_scores(q_x_u16[b, j, h * G:(h + 1) * G, :], k_rows, sm_scale) for j in range(x)]   # x arrays [G, L]
+            a = aggregate(np.concatenate(rows, axis=0), AGG_MAX_LOGIT)
+            sel_b.append(topk_positions(a, int(k_per_seq[b])))
+            sc_b.append(a)
+        sel.append(sel_b)
+        scores.append(sc_b)
+    return sel, scores

@@ -488,3 +488,85 @@ def test_pool_append_block_then_attention_sees_the_rows():
         logits = 0.2 * O.bf16_bits_to_f64(q[0, :, hq]) @ K.T
         p = np.exp(logits - logits.max(axis=1, keepdims=True)); p /= p.sum(axis=1, keepdims=True)
         assert np.allclose(ref[0, :, hq], p @ V, atol=1e-6)
+
+
+# ---------------------------------------------------------------- NEXT-4: x-query selection (reading 25)
+def _xq_inputs(seed, x, batch=2, Hq=4, Hkv=2, seq_lens=(53, 16), d=128, P=16):
+    rng = np.random.default_rng(seed)
+    n_pages = sum((L + P - 1) // P for L in seq_lens)
+    K = rng.standard_normal((n_pages, P, Hkv, d)).astype(np.float32)
+    q = rng.standard_normal((batch, x, Hq, d)).astype(np.float32)
+    pt = np.zeros((batch, max((L + P - 1) // P for L in seq_lens)), np.int32)
+    perm, nxt = rng.permutation(n_pages), 0
+    for b, L in enumerate(seq_lens):
+        for j in range((L + P - 1) // P):
+            pt[b, j] = perm[nxt]
+            nxt += 1
+    return bf16_bits(q), bf16_bits(K), pt, np.array(seq_lens)
+
+
+def test_select_xq_with_one_query_is_select():
+    q, K, pt, L = _xq_inputs(31, 1)
+    sa, sca = O.select_xq(q, K, pt, L, [7, 3], 2, 128 ** -0.5)
+    sb, scb = O.select(q[:, 0], K, pt, L, [7, 3], 2, 128 ** -0.5, O.AGG_MAX_LOGIT)
+    for b in range(2):
+        for h in range(2):
+            assert sa[b][h].tolist() == sb[b][h].tolist() and np.array_equal(sca[b][h], scb[b][h])
+
+
+def test_select_xq_brute_force_loops():
+    # a[t] = max_j max_g scale * q[j, h*G+g] . K[t, h], written as scalar loops over widened values
+    x, G, d = 3, 2, 128
+    q, K, pt, L = _xq_inputs(32, x, seq_lens=(21, 5))
+    qf, Kf = O.bf16_bits_to_f64(q), O.bf16_bits_to_f64(K)
+    sel, sc = O.select_xq(q, K, pt, L, [4, 5], 2, 0.25)
+    for b in range(2):
+        for h in range(2):
+            ref = []
+            for t in range(int(L[b])):
+                krow = Kf[pt[b, t // 16], t % 16, h]
+                best = -math.inf
+                for j in range(x):
+                    for g in range(G):
+                        acc = 0.0
+                        for c in range(d):
+                            acc += qf[b, j, h * G + g, c] * krow[c]
+                        best = max(best, 0.25 * acc)
+                ref.append(best)
+            assert np.allclose(sc[b][h], ref, rtol=1e-12, atol=1e-12)
+            k = min([4, 5][b], int(L[b]))
+            want = sorted(sorted(range(int(L[b])), key=lambda t: (-ref[t], t))[:k])
+            assert sel[b][h].tolist() == want
+
+
+def test_select_xq_invariants():
+    x = 4
+    q, K, pt, L = _xq_inputs(33, x)
+    _, sc = O.select_xq(q, K, pt, L, [5, 5], 2, 1.0)
+    # the order of the x queries does not matter
+    _, sc_perm = O.select_xq(q[:, ::-1].copy(), K, pt, L, [5, 5], 2, 1.0)
+    # a duplicated query changes nothing; one more query never lowers a score; a subset never raises one
+    _, sc_dup = O.select_xq(np.concatenate([q, q[:, :1]], axis=1), K, pt, L, [5, 5], 2, 1.0)
+    _, sc_sub = O.select_xq(q[:, :2].copy(), K, pt, L, [5, 5], 2, 1.0)
+    singles = [O.select(q[:, j].copy(), K, pt, L, [5, 5], 2, 1.0)[1] for j in range(x)]
+    for b in range(2):
+        for h in range(2):
+            assert np.array_equal(sc[b][h], sc_perm[b][h]) and np.array_equal(sc[b][h], sc_dup[b][h])
+            assert np.all(sc_sub[b][h] <= sc[b][h])
+            # and it is exactly the pointwise maximum of the x single-query score planes
+            assert np.array_equal(sc[b][h], np.max([singles[j][b][h] for j in range(x)], axis=0))
+
+
+def test_select_xq_planted_key_found_by_the_one_query_that_matches():
+    # keys are 0 except one row equal to query j=2's head 1; every other query is orthogonal noise on other channels
+    d, L, P, x = 128, 32, 16, 4
+    q = np.zeros((1, x, 2, d), np.float32)
+    for j in range(x):
+        q[0, j, :, 8 * j:8 * j + 8] = -1.0          # negative everywhere it is non-zero: only the planted row scores > 0 ...
+    q[0, 2, 1, 100:108] = 2.0
+    K = np.zeros((L, 1, d), np.float32)
+    K[19, 0, 100:108] = 2.0                          # ... and only through query 2, head 1
+    k_pages = bf16_bits(K).reshape(L // P, P, 1, d)
+    pt = np.arange(L // P, dtype=np.int32)[None]
+    sel, sc = O.select_xq(bf16_bits(q), k_pages, pt, np.array([L]), [1], 1, 1.0)
+    assert sel[0][0].tolist() == [19] and sc[0][0][19] == 32.0 and np.all(np.delete(sc[0][0], 19) == 0.0)
