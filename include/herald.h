@@ -115,6 +115,18 @@ int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, cons
                   const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, float* scores_out,
                   void* ws, size_t ws_bytes, herald_stream_t stream);
 
+/* Selection scored by x queries per sequence instead of one (PAPER.md:137 Fig. 8, :143, :161: the selection kernel as
+ * the query count goes from B = 32 down to 1).  The paper does not say how the x
+ * queries' scores combine into one ranking (reading 25): this entry takes the maximum,
+ *   a[t] = sm_scale * max over j < x, g < G of  q_x[b, j, h*G+g, :] . K[b, t, h, :]
+ * i.e. herald_select's max-logit aggregation over all x*G score rows; x = 1 is herald_select with agg_mode 0.  K is
+ * read once whatever x is; FLOPs grow with x.
+ *   q_x   bf16 [batch][x][H_q][128], device;  1 <= x, x*G <= 256;  shape->agg_mode must be HERALD_AGG_MAX_LOGIT.
+ * Every other argument, the output layout, the workspace size and the error behaviour are herald_select's. */
+int herald_select_xq(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_x, int32_t x,
+                     const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, float* scores_out,
+                     void* ws, size_t ws_bytes, herald_stream_t stream);
+
 /* Gather of the selected entries into a sparse KV pool (pools PAPER.md:175):
  *   pool_k[b][h][j][:] = K[b, sel_idx[b][h][j], h, :]   for j < sel_cnt[b][h]   (bit copies; same for V)
  *   pool_k, pool_v  bf16 [batch][H_kv][pool_capacity][128] -- the IDLE buffer; rows j >= sel_cnt untouched. */

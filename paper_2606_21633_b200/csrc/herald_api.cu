@@ -12,6 +12,7 @@
 #include "cache_ops.cuh"
 #include "gather.cuh"
 #include "rep_attn.cuh"
+#include "scan_xq.cuh"
 #include "scan.cuh"
 #include "topk.cuh"
 
@@ -335,6 +336,40 @@ int32_t herald_attn_grid_ctas(const herald_shape_t* shape) {
     return a.n_splits * a.m_tiles * shape->batch * shape->n_kv_heads;
 }
 
+// Top-k of every unit from the score plane and its level-1 histogram (shared by herald_select and herald_select_xq).
+static int launch_topk(const herald_shape_t* shape, const herald_cache_t* cache, const float* scores, const uint32_t* hist1,
+                       const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t stream) {
+    const int units = shape->batch * shape->n_kv_heads;
+    cudaError_t e;
+    TopkParams tp{};
+    tp.scores = scores;
+    tp.hist1 = hist1;
+    tp.seq_lens = cache->seq_lens;
+    tp.k_per_seq = k_per_seq;
+    tp.sel_idx = sel_idx;
+    tp.sel_cnt = sel_cnt;
+    tp.n_kv_heads = shape->n_kv_heads;
+    tp.max_seq_len = shape->max_seq_len;
+    tp.cap = shape->pool_capacity;
+    static bool topk_attr_set = false;
+    if (!topk_attr_set) {
+        e = cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTopkMaxSmemBytes);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(topk)");
+        topk_attr_set = true;
+    }
+    // shared memory of the one-pass path: a bit per position and room for 1/8 of the positions in the threshold bin
+    // (N(0,1)-like scores put 1-5 % of them there); what does not fit takes the multi-pass path
+    tp.bitmap_words = (shape->max_seq_len + 31) / 32;
+    if (tp.bitmap_words > kTopkMaxBitmapWords) tp.bitmap_words = kTopkMaxBitmapWords;
+    tp.cand_cap = shape->max_seq_len / 8;
+    if (tp.cand_cap < 2048) tp.cand_cap = 2048;
+    if (tp.cand_cap > kTopkMaxCandCap) tp.cand_cap = kTopkMaxCandCap;
+    topk_kernel<<<units, kTopkThreads, (size_t)tp.cand_cap * 8 + 2 * (size_t)tp.bitmap_words * 4, stream>>>(tp);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "topk launch");
+    return HERALD_OK;
+}
+
 int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep,
                   const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, float* scores_out, void* ws,
                   size_t ws_bytes, herald_stream_t stream_) {
@@ -417,34 +452,69 @@ int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, cons
     }
 
     if (prof && prof->scan_end) cudaEventRecord(static_cast<cudaEvent_t>(prof->scan_end), stream);
-    TopkParams tp{};
-    tp.scores = scores;
-    tp.hist1 = hist1;
-    tp.seq_lens = cache->seq_lens;
-    tp.k_per_seq = k_per_seq;
-    tp.sel_idx = sel_idx;
-    tp.sel_cnt = sel_cnt;
-    tp.n_kv_heads = shape->n_kv_heads;
-    tp.max_seq_len = shape->max_seq_len;
-    tp.cap = shape->pool_capacity;
-    static bool topk_attr_set = false;
-    if (!topk_attr_set) {
-        e = cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTopkMaxSmemBytes);
-        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(topk)");
-        topk_attr_set = true;
-    }
-    // shared memory of the one-pass path: a bit per position and room for 1/8 of the positions in the threshold bin
-    // (N(0,1)-like scores put 1-5 % of them there); what does not fit takes the multi-pass path
-    tp.bitmap_words = (shape->max_seq_len + 31) / 32;
-    if (tp.bitmap_words > kTopkMaxBitmapWords) tp.bitmap_words = kTopkMaxBitmapWords;
-    tp.cand_cap = shape->max_seq_len / 8;
-    if (tp.cand_cap < 2048) tp.cand_cap = 2048;
-    if (tp.cand_cap > kTopkMaxCandCap) tp.cand_cap = kTopkMaxCandCap;
-    topk_kernel<<<units, kTopkThreads, (size_t)tp.cand_cap * 8 + 2 * (size_t)tp.bitmap_words * 4, stream>>>(tp);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "topk launch");
+    rc = launch_topk(shape, cache, scores, hist1, k_per_seq, sel_idx, sel_cnt, stream);
+    if (rc) return rc;
     if (prof && prof->topk_end) cudaEventRecord(static_cast<cudaEvent_t>(prof->topk_end), stream);
     return HERALD_OK;
+}
+
+int herald_select_xq(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_x, int32_t x,
+                     const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, float* scores_out, void* ws,
+                     size_t ws_bytes, herald_stream_t stream_) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    rc = check_cache(cache, false);
+    if (rc) return rc;
+    if (!q_x || !k_per_seq || !sel_idx || !sel_cnt || !ws) return fail(HERALD_ERR_INVALID_ARG, "herald_select_xq: NULL pointer");
+    if (!aligned16(q_x) || !aligned16(sel_idx) || !aligned16(scores_out) || (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return fail(HERALD_ERR_INVALID_ARG, "herald_select_xq: misaligned pointer (16 B; workspace 256 B)");
+    const int G = shape->n_q_heads / shape->n_kv_heads;
+    if (x < 1 || (int64_t)x * G > 8 * kXqMaxTiles)
+        return fail(HERALD_ERR_INVALID_ARG, "herald_select_xq: x = %d queries x G = %d heads must give 1..%d score rows per KV head", x, G, 8 * kXqMaxTiles);
+    if (shape->agg_mode != HERALD_AGG_MAX_LOGIT)
+        return fail(HERALD_ERR_INVALID_ARG, "herald_select_xq: only agg_mode HERALD_AGG_MAX_LOGIT is defined for x queries");
+    const SelectWs w = select_ws_layout(shape);
+    if (ws_bytes < w.total) return fail(HERALD_ERR_WORKSPACE_TOO_SMALL, "herald_select_xq: workspace %zu < %zu", ws_bytes, w.total);
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const int units = shape->batch * shape->n_kv_heads;
+    if (units == 0) return HERALD_OK;
+    g_err[0] = 0;
+
+    uint8_t* wsb = static_cast<uint8_t*>(ws);
+    uint32_t* hist1 = reinterpret_cast<uint32_t*>(wsb + w.hist1);
+    float* scores = scores_out ? scores_out : reinterpret_cast<float*>(wsb + w.scores);
+    cudaError_t e = cudaMemsetAsync(hist1, 0, (size_t)units * kBins1 * sizeof(uint32_t), stream);
+    if (e != cudaSuccess) return cuda_fail(e, "memset hist1");
+    if (shape->max_seq_len > 0) {
+        ScanXqParams sp{};
+        sp.k_pages = static_cast<const __nv_bfloat16*>(cache->k_pages);
+        sp.page_stride = cache->page_stride;
+        sp.token_stride = cache->token_stride;
+        sp.head_stride = cache->head_stride;
+        sp.page_table = cache->page_table;
+        sp.seq_lens = cache->seq_lens;
+        sp.q_x = static_cast<const __nv_bfloat16*>(q_x);
+        sp.scores = scores;
+        sp.hist1 = hist1;
+        sp.batch = shape->batch;
+        sp.n_q_heads = shape->n_q_heads;
+        sp.n_kv_heads = shape->n_kv_heads;
+        sp.max_seq_len = shape->max_seq_len;
+        sp.max_pages = shape->max_pages_per_seq;
+        sp.x = x;
+        sp.sm_scale = shape->sm_scale;
+        static bool xq_attr_set = false;
+        if (!xq_attr_set) {
+            e = cudaFuncSetAttribute(scan_xq_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kXqMaxSmemBytes);
+            if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(scan_xq)");
+            xq_attr_set = true;
+        }
+        const int n_tiles = (x * G + 7) / 8;
+        scan_xq_kernel<<<scan_ctas_for(shape), kScanThreads, (size_t)n_tiles * kXqTileBytes, stream>>>(sp);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e, "scan_xq launch");
+    }
+    return launch_topk(shape, cache, scores, hist1, k_per_seq, sel_idx, sel_cnt, stream);
 }
 
 int herald_gather(const herald_shape_t* shape, const herald_cache_t* cache, const int32_t* sel_idx,

@@ -24,7 +24,7 @@ OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE_TOO_SMALL, ERR_CUDA = 0, -1,
 AGG_MAX_LOGIT, AGG_SOFTMAX_SUM = 0, 1
 
 EXPORTS = ("herald_last_error", "herald_budget_rows", "herald_select_workspace_bytes",
-           "herald_attn_workspace_bytes", "herald_attn_grid_ctas", "herald_select", "herald_gather", "herald_sparse_attn",
+           "herald_attn_workspace_bytes", "herald_attn_grid_ctas", "herald_select", "herald_select_xq", "herald_gather", "herald_sparse_attn",
            "herald_dense_attn", "herald_rep_attn_workspace_bytes", "herald_rep_attn",
            "herald_cache_write_block", "herald_pool_append_block",
            "herald_pipeline_step", "herald_pipeline_step_host", "herald_pipeline_set_profile")
@@ -89,6 +89,9 @@ _lib.herald_attn_grid_ctas.argtypes = [C.POINTER(Shape)]
 _lib.herald_select.restype = C.c_int
 _lib.herald_select.argtypes = [C.POINTER(Shape), C.POINTER(Cache), C.c_void_p, C.c_void_p, C.c_void_p,
                                C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+_lib.herald_select_xq.restype = C.c_int
+_lib.herald_select_xq.argtypes = [C.POINTER(Shape), C.POINTER(Cache), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p,
+                                  C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
 _lib.herald_gather.restype = C.c_int
 _lib.herald_gather.argtypes = [C.POINTER(Shape), C.POINTER(Cache), C.c_void_p, C.c_void_p, C.c_void_p,
                                C.c_void_p, C.c_void_p]
@@ -180,6 +183,12 @@ def herald_select(shape, cache, q_rep, k_per_seq, sel_idx, sel_cnt, scores_out, 
     ws_ptr, ws_bytes = _ws(ws)
     _check(_lib.herald_select(C.byref(shape), C.byref(cache), _ptr(q_rep), _ptr(k_per_seq), _ptr(sel_idx),
                               _ptr(sel_cnt), _ptr(scores_out), ws_ptr, ws_bytes, _stream(stream)))
+
+
+def herald_select_xq(shape, cache, q_x, x, k_per_seq, sel_idx, sel_cnt, scores_out, ws, stream=None):
+    ws_ptr, ws_bytes = _ws(ws)
+    _check(_lib.herald_select_xq(C.byref(shape), C.byref(cache), _ptr(q_x), int(x), _ptr(k_per_seq), _ptr(sel_idx),
+                                 _ptr(sel_cnt), _ptr(scores_out), ws_ptr, ws_bytes, _stream(stream)))
 
 
 def herald_gather(shape, cache, sel_idx, sel_cnt, pool_k, pool_v, stream=None):

@@ -178,3 +178,16 @@ def to_u16(t: torch.Tensor):
     """bf16 tensor -> host uint16 NumPy array of its bit patterns (what the oracle takes)."""
     import numpy as np
     return t.detach().to("cpu").contiguous().view(torch.int16).numpy().view(np.uint16)
+
+
+def make_q_x(q_rep: torch.Tensor, x: int, seed: int) -> torch.Tensor:
+    """x queries per sequence for the x-query selection sweep (Fig. 8): bf16 [batch, x, H_q, d].
+    PAPER.md:145-149: the B queries of a block share one [MASK] embedding and differ only by their position, so
+    query 0 is q_rep itself and query j > 0 is q_rep plus a seeded N(0, 1/4) perturbation (the stand-in for the
+    RoPE offset of position j; no RoPE is applied anywhere in the synthetic inputs)."""
+    batch, Hq, d = q_rep.shape
+    gen = torch.Generator(device=q_rep.device)
+    gen.manual_seed(int(seed) + 104729)
+    noise = torch.randn((batch, x, Hq, d), generator=gen, device=q_rep.device, dtype=torch.float32) * 0.5
+    noise[:, 0] = 0.0
+    return (q_rep.to(torch.float32)[:, None] + noise).to(torch.bfloat16).contiguous()

@@ -74,6 +74,62 @@ def test_select_matches_oracle(H, cuda, case, agg_mode):
                     assert len(planted - set(sel_g[b, h, :ks[b]].tolist())) <= max(1, len(planted) // 8)
 
 
+XQ_CASES = [("tiny_ragged", 1), ("tiny_ragged", 3), ("one_token", 2), ("g7_ragged", 4), ("g7_ragged", 32), ("g8_h8", 32), ("g1", 5)]
+
+
+@pytest.mark.parametrize("case,x", XQ_CASES)
+def test_select_xq_matches_oracle(H, cuda, case, x):
+    """herald_select_xq (NEXT-4, Fig. 8): x queries per sequence, maximum over the x*G score rows
+    (reading 25).  Same bar as herald_select: scores within 1e-4, index sets exact outside the band."""
+    c = SELECT_CASES[case]
+    w = c["w"]
+    inp = synth.make_inputs(w, seed=100 + len(case), device=cuda, spare_pages=c["spare"], hostile_tails=c["hostile"])
+    q_x = synth.make_q_x(inp["q_rep"], x, seed=900 + x)
+    ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
+    cap = max(max(ks), 1) + w.block_size
+    max_seq = (w.max_seq_len + 15) // 16 * 16
+    shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, max_seq, inp["page_table"].shape[1], cap, 0)
+    cache = H.make_cache(inp["k_pages"], inp["v_pages"], inp["page_table"], inp["seq_lens"])
+    k_per_seq = torch.tensor(ks, dtype=torch.int32, device=cuda)
+    sel_idx = torch.full((w.batch, w.n_kv_heads, cap), -7, dtype=torch.int32, device=cuda)
+    sel_cnt = torch.full((w.batch, w.n_kv_heads), -7, dtype=torch.int32, device=cuda)
+    scores = torch.full((w.batch, w.n_kv_heads, max(max_seq, 16)), float("nan"), dtype=torch.float32, device=cuda)
+    ws = H.alloc_workspace(H.herald_select_workspace_bytes(shape), cuda)
+    H.herald_select_xq(shape, cache, q_x, x, k_per_seq, sel_idx, sel_cnt, scores, ws)
+    torch.cuda.synchronize()
+    oi = oracle_inputs(inp)
+    sel_o, sc_o = O.select_xq(synth.to_u16(q_x), oi["k_pages"], oi["page_table"], oi["seq_lens"], ks, w.n_kv_heads, 128 ** -0.5)
+    sel_g, cnt_g, sc_g = sel_idx.cpu().numpy(), sel_cnt.cpu().numpy(), scores.cpu().numpy()
+    differing = 0
+    for b, L in enumerate(w.seq_lens):
+        for h in range(w.n_kv_heads):
+            ref = sc_o[b][h]
+            assert np.abs(sc_g[b, h, :L] - ref).max() <= 1e-4, (case, x, b, h, np.abs(sc_g[b, h, :L] - ref).max())
+            differing += check_selection(sel_g[b, h], int(cnt_g[b, h]), ref, ks[b], L, f"{case} x{x} b{b} h{h}")
+            assert np.all(sel_g[b, h, int(cnt_g[b, h]):] == -7), "entries past sel_cnt must stay untouched"
+    units = w.batch * w.n_kv_heads
+    assert differing <= max(1, units // 4), f"{differing} in-band swaps over {units} units is more than rounding explains"
+    if x == 1:      # one query: bit-identical to herald_select's mode-0 plane
+        _, _, _, sel1, cnt1, sc1 = run_select(H, w, inp, ks, 0)
+        assert torch.equal(sc1[:, :, :max_seq].nan_to_num(0.0), scores[:, :, :max_seq].nan_to_num(0.0))
+        assert torch.equal(sel1, sel_idx) and torch.equal(cnt1, sel_cnt)
+
+
+def test_select_xq_rejects_bad_arguments(H, cuda):
+    w = synth.tiny(seq_lens=(40, 7), permille=100)
+    inp = synth.make_inputs(w, seed=5, device=cuda)
+    q_x = synth.make_q_x(inp["q_rep"], 2, seed=1)
+    args = lambda shape: (shape, H.make_cache(inp["k_pages"], inp["v_pages"], inp["page_table"], inp["seq_lens"]), q_x)
+    k_per_seq = torch.tensor([4, 1], dtype=torch.int32, device=cuda)
+    sel_idx = torch.zeros((2, w.n_kv_heads, 32), dtype=torch.int32, device=cuda)
+    sel_cnt = torch.zeros((2, w.n_kv_heads), dtype=torch.int32, device=cuda)
+    for mode, x in ((0, 0), (0, 256 // w.group + 1), (1, 2)):    # no query, too many score rows, undefined aggregation
+        shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, 48, inp["page_table"].shape[1], 32, mode)
+        ws = H.alloc_workspace(H.herald_select_workspace_bytes(shape), cuda)
+        with pytest.raises(H.HeraldError):
+            H.herald_select_xq(*args(shape), x, k_per_seq, sel_idx, sel_cnt, None, ws)
+
+
 def test_select_edge_cases(H, cuda):
     # empty sequence, k = 0, k >= L (identity), k > pool capacity (clamped)
     w = synth.Workload("edge", 4, (0, 40, 33, 64), 4, 2, 16, 3, 100, "plain")
