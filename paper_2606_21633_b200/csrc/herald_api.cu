@@ -13,6 +13,7 @@
 #include "gather.cuh"
 #include "rep_attn.cuh"
 #include "scan_xq.cuh"
+#include "scan_xq_tc.cuh"
 #include "scan.cuh"
 #include "topk.cuh"
 
@@ -306,6 +307,25 @@ static int make_q_map(CUtensorMap* out, const void* q_blk, const herald_shape_t*
     return HERALD_OK;
 }
 
+// q_x [batch][x][H_q][128]: box = (64 channels, G heads, x queries, 1 sequence): the x*G score rows of one KV head
+static int make_qx_map(CUtensorMap* out, const void* q_x, const herald_shape_t* s, int x) {
+    const MapKey key{q_x, {s->batch, x, s->n_q_heads, 7 | (s->n_kv_heads << 16)}};
+    if (cached_map(key, out)) return HERALD_OK;
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
+    const int G = s->n_q_heads / s->n_kv_heads;
+    const cuuint64_t dims[4] = {(cuuint64_t)kHeadDim, (cuuint64_t)s->n_q_heads, (cuuint64_t)x, (cuuint64_t)s->batch};
+    const cuuint64_t strides[3] = {(cuuint64_t)kRowBytes, (cuuint64_t)s->n_q_heads * kRowBytes, (cuuint64_t)x * s->n_q_heads * kRowBytes};
+    const cuuint32_t box[4] = {64u, (cuuint32_t)G, (cuuint32_t)x, 1u};
+    const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    const CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(q_x), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(HERALD_ERR_CUDA, "cuTensorMapEncodeTiled(q_x) failed with CUresult %d", (int)r);
+    store_map(key, *out);
+    return HERALD_OK;
+}
+
 }  // namespace herald
 
 using namespace herald;
@@ -486,31 +506,62 @@ int herald_select_xq(const herald_shape_t* shape, const herald_cache_t* cache, c
     cudaError_t e = cudaMemsetAsync(hist1, 0, (size_t)units * kBins1 * sizeof(uint32_t), stream);
     if (e != cudaSuccess) return cuda_fail(e, "memset hist1");
     if (shape->max_seq_len > 0) {
-        ScanXqParams sp{};
-        sp.k_pages = static_cast<const __nv_bfloat16*>(cache->k_pages);
-        sp.page_stride = cache->page_stride;
-        sp.token_stride = cache->token_stride;
-        sp.head_stride = cache->head_stride;
-        sp.page_table = cache->page_table;
-        sp.seq_lens = cache->seq_lens;
-        sp.q_x = static_cast<const __nv_bfloat16*>(q_x);
-        sp.scores = scores;
-        sp.hist1 = hist1;
-        sp.batch = shape->batch;
-        sp.n_q_heads = shape->n_q_heads;
-        sp.n_kv_heads = shape->n_kv_heads;
-        sp.max_seq_len = shape->max_seq_len;
-        sp.max_pages = shape->max_pages_per_seq;
-        sp.x = x;
-        sp.sm_scale = shape->sm_scale;
-        static bool xq_attr_set = false;
-        if (!xq_attr_set) {
-            e = cudaFuncSetAttribute(scan_xq_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kXqMaxSmemBytes);
-            if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(scan_xq)");
-            xq_attr_set = true;
+        // a dense contraction from ~32 score rows per KV head on: tcgen05 (scan_xq_tc.cuh); below that the rows fit a few
+        // mma.sync tiles and the kernel is an HBM stream either way (scan_xq.cuh).  HERALD_XQ_TC = 0 / 1 forces one.
+        const int rows = x * G;
+        const int want_tc = env_int("HERALD_XQ_TC", -1);
+        if (want_tc == 1 || (want_tc != 0 && rows >= 32)) {
+            CUtensorMap tm_k, tm_q;
+            rc = make_paged_map(&tm_k, cache->k_pages, cache, shape->n_kv_heads);
+            if (rc) return rc;
+            rc = make_qx_map(&tm_q, q_x, shape, x);
+            if (rc) return rc;
+            ScanXqTcParams tp{};
+            tp.page_table = cache->page_table;
+            tp.seq_lens = cache->seq_lens;
+            tp.scores = scores;
+            tp.hist1 = hist1;
+            tp.batch = shape->batch;
+            tp.n_q_heads = shape->n_q_heads;
+            tp.n_kv_heads = shape->n_kv_heads;
+            tp.max_seq_len = shape->max_seq_len;
+            tp.max_pages = shape->max_pages_per_seq;
+            tp.x = x;
+            tp.sm_scale = shape->sm_scale;
+            static bool xt_attr_set = false;
+            if (!xt_attr_set) {
+                e = cudaFuncSetAttribute(scan_xq_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kXtSmemBytes + 1024);
+                if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(scan_xq_tc)");
+                xt_attr_set = true;
+            }
+            scan_xq_tc_kernel<<<scan_ctas_for(shape), kXtThreads, kXtSmemBytes + 1024, stream>>>(tm_k, tm_q, tp);
+        } else {
+            ScanXqParams sp{};
+            sp.k_pages = static_cast<const __nv_bfloat16*>(cache->k_pages);
+            sp.page_stride = cache->page_stride;
+            sp.token_stride = cache->token_stride;
+            sp.head_stride = cache->head_stride;
+            sp.page_table = cache->page_table;
+            sp.seq_lens = cache->seq_lens;
+            sp.q_x = static_cast<const __nv_bfloat16*>(q_x);
+            sp.scores = scores;
+            sp.hist1 = hist1;
+            sp.batch = shape->batch;
+            sp.n_q_heads = shape->n_q_heads;
+            sp.n_kv_heads = shape->n_kv_heads;
+            sp.max_seq_len = shape->max_seq_len;
+            sp.max_pages = shape->max_pages_per_seq;
+            sp.x = x;
+            sp.sm_scale = shape->sm_scale;
+            static bool xq_attr_set = false;
+            if (!xq_attr_set) {
+                e = cudaFuncSetAttribute(scan_xq_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kXqMaxSmemBytes);
+                if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(scan_xq)");
+                xq_attr_set = true;
+            }
+            const int n_tiles = (x * G + 7) / 8;
+            scan_xq_kernel<<<scan_ctas_for(shape), kScanThreads, (size_t)n_tiles * kXqTileBytes, stream>>>(sp);
         }
-        const int n_tiles = (x * G + 7) / 8;
-        scan_xq_kernel<<<scan_ctas_for(shape), kScanThreads, (size_t)n_tiles * kXqTileBytes, stream>>>(sp);
         e = cudaGetLastError();
         if (e != cudaSuccess) return cuda_fail(e, "scan_xq launch");
     }
