@@ -528,13 +528,15 @@ int herald_select_xq(const herald_shape_t* shape, const herald_cache_t* cache, c
             tp.max_pages = shape->max_pages_per_seq;
             tp.x = x;
             tp.sm_scale = shape->sm_scale;
+            const int xt_ctas = scan_ctas_for(shape);
+            tp.set_size = (xt_ctas >= shape->n_kv_heads && !env_int("HERALD_SCAN_HEAD_MAJOR", 0)) ? shape->n_kv_heads : 1;
             static bool xt_attr_set = false;
             if (!xt_attr_set) {
                 e = cudaFuncSetAttribute(scan_xq_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kXtSmemBytes + 1024);
                 if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(scan_xq_tc)");
                 xt_attr_set = true;
             }
-            scan_xq_tc_kernel<<<scan_ctas_for(shape), kXtThreads, kXtSmemBytes + 1024, stream>>>(tm_k, tm_q, tp);
+            scan_xq_tc_kernel<<<xt_ctas, kXtThreads, kXtSmemBytes + 1024, stream>>>(tm_k, tm_q, tp);
         } else {
             ScanXqParams sp{};
             sp.k_pages = static_cast<const __nv_bfloat16*>(cache->k_pages);

@@ -11,9 +11,12 @@
 // K 1400 cycles at the chip's HBM rate: the kernel stays on the HBM roofline at every x, which the mma.sync form
 // (scan_xq.cuh) leaves at x*G ~ 32.
 //   warps 0-7: read-out (TMEM lane quarter = warp % 4, column chunks of 32 alternate between warp / 4 = 0, 1), score
-//   plane + level-1 histogram; warp 8: TMA producer; warp 9: MMA issuer.  One persistent CTA per SM; the (unit, tile)
-//   space is cut into gridDim.x equal ranges (head-major like scan_kernel<0>: the query rows of one KV head fill the
-//   shared memory left beside the K ring).
+//   plane + level-1 histogram; warp 8: TMA producer; warp 9: MMA issuer.  One persistent CTA per SM.  The query rows of
+//   one KV head fill the shared memory left beside the K ring, so a CTA works on one head at a time; to keep DRAM on
+//   whole pages all the same (a page holds the rows of all H_kv heads side by side) the CTAs form sets of H_kv: a set
+//   shares a range of the (sequence, tile) space and CTA i of the set takes head i of it, so the H_kv head slices of a
+//   page are requested at about the same time (p.set_size = H_kv).  Grids smaller than H_kv fall back to ranges of the
+//   (unit, tile) space (p.set_size = 1).
 #pragma once
 #include "attn_tc.cuh"
 #include "scan.cuh"
@@ -40,21 +43,24 @@ struct ScanXqTcParams {
     float* scores;                // [units][max_seq_len]
     uint32_t* hist1;              // [units][kBins1]
     int32_t batch, n_q_heads, n_kv_heads, max_seq_len, max_pages, x;
+    int32_t set_size;             // H_kv: CTA sets share (sequence, tile) ranges, one head each; 1: ranges of the (unit, tile) space
     float sm_scale;
 };
 
-// Walk the (unit, 128-token tile) segments of the range [g0, g1): f(b, h, L, tile_lo, tile_hi, seg)
+// Walk the segments of this CTA: f(b, h, L, tile_lo, tile_hi, seg).  With sets, [g0, g1) is a range of the (sequence,
+// tile) space and the CTA's head is fixed; without, a range of the (unit, tile) space.
 template <typename F>
-__device__ __forceinline__ void xt_for_each_segment(const ScanXqTcParams& p, int64_t g0, int64_t g1, F&& f) {
-    int64_t unit_begin = 0;
+__device__ __forceinline__ void xt_for_each_segment(const ScanXqTcParams& p, int64_t g0, int64_t g1, int my_h, F&& f) {
+    int64_t begin = 0;
     int seg = 0;
-    for (int b = 0; b < p.batch && unit_begin < g1; ++b) {
+    for (int b = 0; b < p.batch && begin < g1; ++b) {
         const int L = min(p.seq_lens[b], p.max_seq_len);
         const int n_t = (L + kTcBN - 1) / kTcBN;
-        for (int h = 0; h < p.n_kv_heads; ++h, unit_begin += n_t) {
-            const int64_t lo = max(g0, unit_begin), hi = min(g1, unit_begin + n_t);
+        const int h_lo = my_h >= 0 ? my_h : 0, h_hi = my_h >= 0 ? my_h + 1 : p.n_kv_heads;
+        for (int h = h_lo; h < h_hi; ++h, begin += n_t) {
+            const int64_t lo = max(g0, begin), hi = min(g1, begin + n_t);
             if (lo >= hi) continue;
-            f(b, h, L, (int)(lo - unit_begin), (int)(hi - unit_begin), seg);
+            f(b, h, L, (int)(lo - begin), (int)(hi - begin), seg);
             ++seg;
         }
     }
@@ -101,29 +107,44 @@ scan_xq_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constan
     const uint32_t tmem = *tmem_ptr_gen;
 
     // the range of this CTA (every role computes it from the inputs alone)
+    const bool sets = p.set_size > 1;
+    const int my_h = sets ? (int)(blockIdx.x % p.set_size) : -1;
+    const int n_ranges = sets ? (int)(gridDim.x / p.set_size) : (int)gridDim.x, range = sets ? (int)(blockIdx.x / p.set_size) : (int)blockIdx.x;
     int64_t total = 0;
-    for (int b = 0; b < p.batch; ++b) total += (int64_t)((min(p.seq_lens[b], p.max_seq_len) + kTcBN - 1) / kTcBN) * p.n_kv_heads;
-    const int64_t g0 = cta_range_begin(total, blockIdx.x, gridDim.x), g1 = cta_range_begin(total, blockIdx.x + 1, gridDim.x);
+    for (int b = 0; b < p.batch; ++b) total += (int64_t)((min(p.seq_lens[b], p.max_seq_len) + kTcBN - 1) / kTcBN) * (sets ? 1 : p.n_kv_heads);
+    // (CTAs past the last whole set have no range)
+    const int64_t g0 = range < n_ranges ? cta_range_begin(total, range, n_ranges) : 0, g1 = range < n_ranges ? cta_range_begin(total, range + 1, n_ranges) : 0;
 
     if (warp == kXtTmaWarp) {
         // =========================== producer: the unit's query rows, then its K tiles ===========================
         int kt = 0;
-        xt_for_each_segment(p, g0, g1, [&](int b, int h, int L, int tile_lo, int tile_hi, int seg) {
-            if (seg > 0) mbar_wait(bar(kXtBarQFree), (seg - 1) & 1);        // the MMAs of the previous unit are done with Q
-            if (elect_one()) {
-                // q_x [batch][x][H_q][128]: box = (64 channels, G heads, x queries) per half -> rows rho = j*G + g
-                mbar_arrive_expect_tx(bar(kXtBarQFull), (uint32_t)rows * 256u);
-                tma_load_4d(sbase + kXtSmemQ, &tm_q, 0, h * G, 0, b, bar(kXtBarQFull));
-                tma_load_4d(sbase + kXtSmemQ + kXtQHalfBytes, &tm_q, 64, h * G, 0, b, bar(kXtBarQFull));
-            }
-            __syncwarp();
+        xt_for_each_segment(p, g0, g1, my_h, [&](int b, int h, int L, int tile_lo, int tile_hi, int seg) {
+            auto load_q = [&]() {
+                if (seg > 0) mbar_wait(bar(kXtBarQFree), (seg - 1) & 1);    // the MMAs of the previous unit are done with Q
+                if (elect_one()) {
+                    // q_x [batch][x][H_q][128]: box = (64 channels, G heads, x queries) per half -> rows rho = j*G + g
+                    mbar_arrive_expect_tx(bar(kXtBarQFull), (uint32_t)rows * 256u);
+                    tma_load_4d(sbase + kXtSmemQ, &tm_q, 0, h * G, 0, b, bar(kXtBarQFull));
+                    tma_load_4d(sbase + kXtSmemQ + kXtQHalfBytes, &tm_q, 64, h * G, 0, b, bar(kXtBarQFull));
+                }
+                __syncwarp();
+            };
+            // At a unit boundary the K ring keeps filling with the new unit's tiles while the MMAs finish the old one;
+            // only the query rows wait for them (after up to kXtStages - 1 tiles are on their way).
+            const int q_after = seg == 0 ? -1 : min(kXtStages - 1, tile_hi - tile_lo) - 1;
+            if (q_after < 0) load_q();
+            // the 128 tokens of a tile are 8 pages of the cache; page i lands on tile rows [16i, 16i+16) (2 KB per half: whole
+            // 1 KB swizzle atoms).  Pages past the sequence are not requested: their rows are never read out.  The page
+            // ids of the next tile are fetched before waiting for its ring slot.
+            const int32_t* pt = p.page_table + (int64_t)b * p.max_pages;
+            auto tile_pages = [&](int t) { return (min(kTcBN, L - t * kTcBN) + kPageSize - 1) / kPageSize; };
+            int n_pg = tile_pages(tile_lo);
+            int my_phys = lane < n_pg ? __ldg(pt + tile_lo * (kTcBN / kPageSize) + lane) : 0;
             for (int t = tile_lo; t < tile_hi; ++t, ++kt) {
                 const int stage = kt % kXtStages;
+                const int n_pg_next = t + 1 < tile_hi ? tile_pages(t + 1) : 0;
+                const int phys_next = lane < n_pg_next ? __ldg(pt + (t + 1) * (kTcBN / kPageSize) + lane) : 0;
                 if (kt >= kXtStages) mbar_wait(bar(kXtBarKEmpty + stage), ((kt / kXtStages) - 1) & 1);
-                // the 128 tokens of the tile are 8 pages of the cache; page i lands on tile rows [16i, 16i+16) (2 KB per
-                // half: whole 1 KB swizzle atoms).  Pages past the sequence are not requested: their rows are never read out.
-                const int valid = min(kTcBN, L - t * kTcBN), n_pg = (valid + kPageSize - 1) / kPageSize;
-                const int my_phys = lane < n_pg ? __ldg(p.page_table + (int64_t)b * p.max_pages + t * (kTcBN / kPageSize) + lane) : 0;
                 const uint32_t dst = sbase + kXtSmemK + stage * kTcTileBytes, full = bar(kXtBarKFull + stage);
                 if (lane == 0) mbar_arrive_expect_tx(full, (uint32_t)n_pg * kPageSize * 256u);
                 __syncwarp();
@@ -132,6 +153,9 @@ scan_xq_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constan
                     tma_load_4d(dst + kTcHalfBytes + lane * (kPageSize * 128), &tm_k, 64, h, 0, my_phys, full);
                 }
                 __syncwarp();
+                if (t - tile_lo == q_after) load_q();
+                n_pg = n_pg_next;
+                my_phys = phys_next;
             }
         });
     } else if (warp == kXtMmaWarp) {
@@ -140,7 +164,7 @@ scan_xq_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constan
         const uint32_t q_lo = umma_desc_lo(sbase + kXtSmemQ, 16);
         const uint32_t idesc = umma_idesc(/*A bf16*/ 1, /*B bf16*/ 1, /*K-major*/ 0, 0, kTcBM, n_pad);
         int kt = 0;
-        xt_for_each_segment(p, g0, g1, [&](int, int, int, int tile_lo, int tile_hi, int seg) {
+        xt_for_each_segment(p, g0, g1, my_h, [&](int, int, int, int tile_lo, int tile_hi, int seg) {
             mbar_wait(bar(kXtBarQFull), seg & 1);
             for (int t = tile_lo; t < tile_hi; ++t, ++kt) {
                 const int stage = kt % kXtStages, buf = kt & 1;
@@ -172,7 +196,7 @@ scan_xq_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constan
         const uint32_t lane_base = tmem + ((uint32_t)(quarter * 32) << 16);
         const int n_chunks = (rows + 31) >> 5;
         int dt = 0;
-        xt_for_each_segment(p, g0, g1, [&](int b, int h, int L, int tile_lo, int tile_hi, int) {
+        xt_for_each_segment(p, g0, g1, my_h, [&](int b, int h, int L, int tile_lo, int tile_hi, int) {
             const int unit = b * p.n_kv_heads + h;
             float* score_row = p.scores + (int64_t)unit * p.max_seq_len;
             for (int t = tile_lo; t < tile_hi; ++t, ++dt) {
