@@ -396,6 +396,19 @@ def main():
     rep_out = torch.empty((w.batch, w.n_q_heads, 128), dtype=torch.float32, device=dev)
     ws_rep = H.alloc_workspace(H.herald_rep_attn_workspace_bytes(shape), dev)
     rep_attn_ms = time_isolated(lambda: H.herald_rep_attn(shape, cache, inp["q_rep"], rep_out, None, ws_rep, side), reps=4, warm=2, timed=3)
+    # NEXT-4: the selection kernel against the number of queries x (Fig. 8: 32 -> 1 gives 8x on the CPU)
+    xq_sweep = {}
+    for x in (1, 2, 4, 8, 16, 32):
+        if x * w.group > 256:
+            break
+        q_x = synth.make_q_x(inp["q_rep"], x, seed=7000 + x)
+        xq_ms = time_isolated(lambda: H.herald_select_xq(shape, cache, q_x, x, k_per_seq, sel_idx, sel_cnt, None, ws_sel, side), reps=4, warm=2, timed=3)
+        xq_sweep[str(x)] = {"select_ms": xq_ms, "score_tflops": 2 * 128 * x * w.n_q_heads * tokens / (xq_ms * 1e-3) / 1e12}
+        del q_x
+    if xq_sweep:
+        x_max = max(xq_sweep, key=int)
+        for v in xq_sweep.values():
+            v["throughput_vs_x%s" % x_max] = xq_sweep[x_max]["select_ms"] / v["select_ms"]
     dense_flops = sum(4 * M * (L + w.block_size) * 128 for L in w.seq_lens) * w.n_kv_heads
     denoise_alone_ms = attn_alone_ms * n_steps * n_layers        # stage timings are per layer (layer 0), the block has n_layers
     select_alone_ms, select_mode1_alone_ms = select_alone_ms * n_layers, select_mode1_alone_ms * n_layers
@@ -483,6 +496,7 @@ def main():
             "overlap_efficiency": (denoise_alone_ms + select_alone_ms + gather_alone_ms_block - ms_step) / (select_alone_ms + gather_alone_ms_block),
             "n_layers": n_layers,
             "rep_attn_ms": rep_attn_ms, "rep_attn_gbs": tokens * w.n_kv_heads * 512 / (rep_attn_ms * 1e-3) / 1e9,
+            "select_xq_sweep": xq_sweep,
             "dense_attn_full_cache_ms": dense_attn_ms, "dense_attn_tflops": dense_flops / (dense_attn_ms * 1e-3) / 1e12,
             "attn_time_share_alone": attn_share,
             "algorithmic": {"scan_bytes": scan_bytes, "gather_bytes": gather_bytes, "attn_flops_per_step": attn_flops,
