@@ -8,6 +8,7 @@
 #include <cstring>
 
 #include "attn_tc.cuh"
+#include <functional>
 #include "common.cuh"
 #include "cache_ops.cuh"
 #include "gather.cuh"
@@ -358,7 +359,7 @@ int32_t herald_attn_grid_ctas(const herald_shape_t* shape) {
 
 // Top-k of every unit from the score plane and its level-1 histogram (shared by herald_select and herald_select_xq).
 static int launch_topk(const herald_shape_t* shape, const herald_cache_t* cache, const float* scores, const uint32_t* hist1,
-                       const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t stream) {
+                       const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, cudaStream_t stream, bool programmatic = false) {
     const int units = shape->batch * shape->n_kv_heads;
     cudaError_t e;
     TopkParams tp{};
@@ -384,8 +385,17 @@ static int launch_topk(const herald_shape_t* shape, const herald_cache_t* cache,
     tp.cand_cap = shape->max_seq_len / 8;
     if (tp.cand_cap < 2048) tp.cand_cap = 2048;
     if (tp.cand_cap > kTopkMaxCandCap) tp.cand_cap = kTopkMaxCandCap;
-    topk_kernel<<<units, kTopkThreads, (size_t)tp.cand_cap * 8 + 2 * (size_t)tp.bitmap_words * 4, stream>>>(tp);
-    e = cudaGetLastError();
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(units);
+    cfg.blockDim = dim3(kTopkThreads);
+    cfg.dynamicSmemBytes = (size_t)tp.cand_cap * 8 + 2 * (size_t)tp.bitmap_words * 4;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = programmatic ? 1 : 0;
+    e = cudaLaunchKernelEx(&cfg, topk_kernel, tp);
     if (e != cudaSuccess) return cuda_fail(e, "topk launch");
     return HERALD_OK;
 }
@@ -778,22 +788,17 @@ size_t herald_rep_attn_workspace_bytes(const herald_shape_t* shape) {
     return align_up((kRepMaxCtas + groups) * hg * kRepPartFloats * sizeof(float), 256);   // slot = cta + group, hg head partials each
 }
 
-int herald_rep_attn(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep, float* out, float* lse,
-                    void* ws, size_t ws_bytes, herald_stream_t stream_) {
-    int rc = check_shape(shape);
-    if (rc) return rc;
-    rc = check_cache(cache, true);
-    if (rc) return rc;
-    if (!q_rep || !out || !ws) return fail(HERALD_ERR_INVALID_ARG, "herald_rep_attn: NULL pointer");
-    if (!aligned16(q_rep) || !aligned16(out) || (reinterpret_cast<uintptr_t>(ws) & 255u))
-        return fail(HERALD_ERR_INVALID_ARG, "herald_rep_attn: misaligned pointer (16 B; workspace 256 B)");
-    const size_t need = herald_rep_attn_workspace_bytes(shape);
-    if (ws_bytes < need) return fail(HERALD_ERR_WORKSPACE_TOO_SMALL, "herald_rep_attn: workspace %zu < %zu", ws_bytes, need);
-    const int units = shape->batch * shape->n_kv_heads;
-    if (units == 0) return HERALD_OK;
-    g_err[0] = 0;
-    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+// The K+V pass of herald_rep_attn; with `scores` it also writes the max-logit selection scores (herald_select_rep).
+// `between` (herald_select_rep: the top-k, launched programmatically) runs after the pass and before the merge is enqueued;
+// the merge then starts beside it and does not wait for it.
+static int rep_attn_launch(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep, float* out, float* lse,
+                           void* ws, float* scores, uint32_t* hist1, cudaStream_t stream, const std::function<int()>& between,
+                           bool has_between) {
     RepAttnParams rp{};
+    rp.scores = scores;
+    rp.hist1 = hist1;
+    rp.sm_scale = shape->sm_scale;
+    rp.merge_waits = has_between ? 0 : 1;
     rp.k_pages = static_cast<const __nv_bfloat16*>(cache->k_pages);
     rp.v_pages = static_cast<const __nv_bfloat16*>(cache->v_pages);
     rp.page_stride = cache->page_stride;
@@ -821,6 +826,10 @@ int herald_rep_attn(const herald_shape_t* shape, const herald_cache_t* cache, co
     rep_attn_kernel<<<n_ctas, kRepThreads, kRepSmemBytes, stream>>>(rp);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "rep_attn launch");
+    if (has_between) {
+        const int rc = between();
+        if (rc) return rc;
+    }
     // the merge is launched programmatically behind the main grid: its blocks are scheduled as the main CTAs retire,
     // find their partial list (inputs only) and wait (griddepcontrol.wait) for the grid to complete
     cudaLaunchConfig_t cfg{};
@@ -835,6 +844,56 @@ int herald_rep_attn(const herald_shape_t* shape, const herald_cache_t* cache, co
     e = cudaLaunchKernelEx(&cfg, rep_attn_merge_kernel, rp, n_ctas);
     if (e != cudaSuccess) return cuda_fail(e, "rep_attn launch");
     return HERALD_OK;
+}
+
+int herald_rep_attn(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep, float* out, float* lse,
+                    void* ws, size_t ws_bytes, herald_stream_t stream_) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    rc = check_cache(cache, true);
+    if (rc) return rc;
+    if (!q_rep || !out || !ws) return fail(HERALD_ERR_INVALID_ARG, "herald_rep_attn: NULL pointer");
+    if (!aligned16(q_rep) || !aligned16(out) || (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return fail(HERALD_ERR_INVALID_ARG, "herald_rep_attn: misaligned pointer (16 B; workspace 256 B)");
+    const size_t need = herald_rep_attn_workspace_bytes(shape);
+    if (ws_bytes < need) return fail(HERALD_ERR_WORKSPACE_TOO_SMALL, "herald_rep_attn: workspace %zu < %zu", ws_bytes, need);
+    if (shape->batch * shape->n_kv_heads == 0) return HERALD_OK;
+    g_err[0] = 0;
+    return rep_attn_launch(shape, cache, q_rep, out, lse, ws, nullptr, nullptr, static_cast<cudaStream_t>(stream_), [] { return 0; }, false);
+}
+
+size_t herald_select_rep_workspace_bytes(const herald_shape_t* shape) {
+    if (check_shape(shape) != HERALD_OK) return 0;
+    return align_up(select_ws_layout(shape).total, 256) + herald_rep_attn_workspace_bytes(shape);
+}
+
+int herald_select_rep(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep, const int32_t* k_per_seq,
+                      int32_t* sel_idx, int32_t* sel_cnt, float* scores_out, float* rep_out, float* rep_lse, void* ws,
+                      size_t ws_bytes, herald_stream_t stream_) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    rc = check_cache(cache, true);
+    if (rc) return rc;
+    if (!q_rep || !k_per_seq || !sel_idx || !sel_cnt || !rep_out || !ws) return fail(HERALD_ERR_INVALID_ARG, "herald_select_rep: NULL pointer");
+    if (!aligned16(q_rep) || !aligned16(sel_idx) || !aligned16(scores_out) || !aligned16(rep_out) || (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return fail(HERALD_ERR_INVALID_ARG, "herald_select_rep: misaligned pointer (16 B; workspace 256 B)");
+    if (shape->agg_mode != HERALD_AGG_MAX_LOGIT)
+        return fail(HERALD_ERR_UNSUPPORTED, "herald_select_rep: the fused pass aggregates by max-logit (agg_mode 0) only");
+    const size_t need = herald_select_rep_workspace_bytes(shape);
+    if (ws_bytes < need) return fail(HERALD_ERR_WORKSPACE_TOO_SMALL, "herald_select_rep: workspace %zu < %zu", ws_bytes, need);
+    const int units = shape->batch * shape->n_kv_heads;
+    if (units == 0) return HERALD_OK;
+    g_err[0] = 0;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const SelectWs w = select_ws_layout(shape);
+    uint8_t* wsb = static_cast<uint8_t*>(ws);
+    uint32_t* hist1 = reinterpret_cast<uint32_t*>(wsb + w.hist1);
+    float* scores = scores_out ? scores_out : reinterpret_cast<float*>(wsb + w.scores);
+    cudaError_t e = cudaMemsetAsync(hist1, 0, (size_t)units * kBins1 * sizeof(uint32_t), stream);
+    if (e != cudaSuccess) return cuda_fail(e, "memset hist1");
+    // pass (scores + histogram + partials) -> top-k, launched programmatically behind the pass -> merge, beside the top-k
+    return rep_attn_launch(shape, cache, q_rep, rep_out, rep_lse, wsb + align_up(w.total, 256), scores, hist1, stream,
+                           [&] { return launch_topk(shape, cache, scores, hist1, k_per_seq, sel_idx, sel_cnt, stream, true); }, true);
 }
 
 // Longest-pool-first unit order of one layer into `order` (device, [units]); enqueued on `stream`.

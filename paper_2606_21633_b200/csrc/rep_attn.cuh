@@ -51,6 +51,10 @@ struct RepAttnParams {
     float* part;          // [gridDim.x + groups][hg][8][130], slot = cta + group
     float* out;           // [batch][H_q][128]
     float* lse;           // optional [batch][H_q]
+    float* scores;        // optional [units][max_seq_len]: the selection scores of the same pass (herald_select_rep), mode 0
+    uint32_t* hist1;      // with scores: [units][kBins1] level-1 histogram of the top-k (zeroed before the launch)
+    float sm_scale;
+    int32_t merge_waits;  // the merge grid waits for its predecessor (0: it is launched behind a grid that already did)
     int32_t batch, n_q_heads, n_kv_heads, max_seq_len, max_pages, hg;
     float scale_log2;     // sm_scale * log2(e): the softmax runs in base 2
 };
@@ -155,7 +159,7 @@ __global__ void __launch_bounds__(kRepThreads, 2) rep_attn_kernel(const RepAttnP
                 mma_bf16_16816(sb, qf[i].x, 0u, qf[i].y, 0u, c[i].x, c[i].y);
                 mma_bf16_16816(sb, qf[i].z, 0u, qf[i].w, 0u, c[i].z, c[i].w);
             }
-            // the fragments are consumed: put the next page of this warp in flight
+            // the K fragments are consumed: put the next page of this warp in flight
             if (page + n_slots < page_end) {
                 issue_page(page + n_slots, phys_next, st ^ 1);
                 if (page + 2 * n_slots < page_end) phys_next = __ldg(pt + page + 2 * n_slots);
@@ -164,6 +168,30 @@ __global__ void __launch_bounds__(kRepThreads, 2) rep_attn_kernel(const RepAttnP
             // sa[0], sa[1]: head g, tokens 2tig, 2tig+1 ; sb[0], sb[1]: tokens 8+2tig, 9+2tig.  Mask the tail of the last page.
             const int t0 = page * kPageSize + 2 * tig;
             const bool ok0 = t0 < t_end, ok1 = t0 + 1 < t_end, ok2 = t0 + 8 < t_end, ok3 = t0 + 9 < t_end;
+            if (p.scores) {
+                // the fused retrieval kernel: the raw scores of this pass are the selection scores too;
+                // max-logit aggregation = maximum over the G heads = over the lanes with equal tig
+                float r0 = g < G ? sa[0] : -INFINITY, r1 = g < G ? sa[1] : -INFINITY;
+                float r2 = g < G ? sb[0] : -INFINITY, r3 = g < G ? sb[1] : -INFINITY;
+#pragma unroll
+                for (int off = 4; off < 32; off <<= 1) {
+                    r0 = fmaxf(r0, __shfl_xor_sync(0xffffffffu, r0, off));
+                    r1 = fmaxf(r1, __shfl_xor_sync(0xffffffffu, r1, off));
+                    r2 = fmaxf(r2, __shfl_xor_sync(0xffffffffu, r2, off));
+                    r3 = fmaxf(r3, __shfl_xor_sync(0xffffffffu, r3, off));
+                }
+                if (g == 0) {
+                    // score plane + level-1 histogram (fire-and-forget reductions in L2: 64 KB of shared histograms per
+                    // CTA would cost the second CTA of the SM)
+                    float* sr = p.scores + (int64_t)(b * p.n_kv_heads + h) * p.max_seq_len + t0;
+                    uint32_t* hh = p.hist1 + (int64_t)(b * p.n_kv_heads + h) * kBins1;
+                    const float v0 = r0 * p.sm_scale, v1 = r1 * p.sm_scale, v2 = r2 * p.sm_scale, v3 = r3 * p.sm_scale;
+                    if (ok0) { sr[0] = v0; atomicAdd(hh + (score_key(v0) >> (32 - kBits1)), 1u); }
+                    if (ok1) { sr[1] = v1; atomicAdd(hh + (score_key(v1) >> (32 - kBits1)), 1u); }
+                    if (ok2) { sr[8] = v2; atomicAdd(hh + (score_key(v2) >> (32 - kBits1)), 1u); }
+                    if (ok3) { sr[9] = v3; atomicAdd(hh + (score_key(v3) >> (32 - kBits1)), 1u); }
+                }
+            }
             const float s0 = ok0 ? sa[0] * p.scale_log2 : -INFINITY, s1 = ok1 ? sa[1] * p.scale_log2 : -INFINITY;
             const float s2 = ok2 ? sb[0] * p.scale_log2 : -INFINITY, s3 = ok3 ? sb[1] * p.scale_log2 : -INFINITY;
             float mx = fmaxf(fmaxf(s0, s1), fmaxf(s2, s3));     // page maximum of head g: 4 values here, 4 lanes per head
@@ -278,7 +306,7 @@ __global__ void __launch_bounds__(kHeadDim * kRepMergeSlices) rep_attn_merge_ker
     __syncthreads();
     const int c_first = s_first, n_parts = s_nparts;
     const int64_t total = s_total;
-    asm volatile("griddepcontrol.wait;" ::: "memory");        // launched programmatically: the partials are complete from here on
+    if (p.merge_waits) asm volatile("griddepcontrol.wait;" ::: "memory");   // launched programmatically: the partials are complete from here on
     const int group = b * n_groups + hgrp;
     const float* pq = p.part + ((int64_t)(c_first + group) * hg + hh) * kRepPartFloats + q * (kHeadDim + 2);
     const int64_t cstride = (int64_t)hg * kRepPartFloats;

@@ -66,6 +66,10 @@ __global__ void __launch_bounds__(kTopkThreads, 2) topk_kernel(const TopkParams 
     __shared__ uint32_t s_res[2];
     __shared__ uint32_t s_ncand;
 
+    // herald_select_rep launches this grid programmatically behind the K+V pass and the partial merge behind this one:
+    // wait for the pass (scores, histogram), then let the merge start beside us.  No-ops in an ordinary launch.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;");
     const int unit = blockIdx.x;
     const int b = unit / p.n_kv_heads;
     const int L = min(p.seq_lens[b], p.max_seq_len);

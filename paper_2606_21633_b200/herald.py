@@ -26,6 +26,7 @@ AGG_MAX_LOGIT, AGG_SOFTMAX_SUM = 0, 1
 EXPORTS = ("herald_last_error", "herald_budget_rows", "herald_select_workspace_bytes",
            "herald_attn_workspace_bytes", "herald_attn_grid_ctas", "herald_select", "herald_select_xq", "herald_gather", "herald_sparse_attn",
            "herald_dense_attn", "herald_rep_attn_workspace_bytes", "herald_rep_attn",
+           "herald_select_rep_workspace_bytes", "herald_select_rep",
            "herald_cache_write_block", "herald_pool_append_block",
            "herald_pipeline_step", "herald_pipeline_step_host", "herald_pipeline_set_profile")
 
@@ -104,6 +105,10 @@ _lib.herald_rep_attn_workspace_bytes.argtypes = [C.POINTER(Shape)]
 _lib.herald_rep_attn.restype = C.c_int
 _lib.herald_rep_attn.argtypes = [C.POINTER(Shape), C.POINTER(Cache), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t,
                                  C.c_void_p]
+_lib.herald_select_rep_workspace_bytes.restype = C.c_size_t
+_lib.herald_select_rep_workspace_bytes.argtypes = [C.POINTER(Shape)]
+_lib.herald_select_rep.restype = C.c_int
+_lib.herald_select_rep.argtypes = [C.POINTER(Shape), C.POINTER(Cache)] + [C.c_void_p] * 8 + [C.c_size_t, C.c_void_p]
 _lib.herald_cache_write_block.restype = C.c_int
 _lib.herald_cache_write_block.argtypes = [C.POINTER(Shape), C.POINTER(Cache), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.herald_pool_append_block.restype = C.c_int
@@ -207,6 +212,16 @@ def herald_dense_attn(shape, cache, q_blk, k_blk, v_blk, out, lse, ws, stream=No
     ws_ptr, ws_bytes = _ws(ws)
     _check(_lib.herald_dense_attn(C.byref(shape), C.byref(cache), _ptr(q_blk), _ptr(k_blk), _ptr(v_blk), _ptr(out),
                                   _ptr(lse), ws_ptr, ws_bytes, _stream(stream)))
+
+
+def herald_select_rep_workspace_bytes(shape: Shape) -> int:
+    return int(_lib.herald_select_rep_workspace_bytes(C.byref(shape)))
+
+
+def herald_select_rep(shape, cache, q_rep, k_per_seq, sel_idx, sel_cnt, scores_out, rep_out, rep_lse, ws, stream=None):
+    ws_ptr, ws_bytes = _ws(ws)
+    _check(_lib.herald_select_rep(C.byref(shape), C.byref(cache), _ptr(q_rep), _ptr(k_per_seq), _ptr(sel_idx), _ptr(sel_cnt),
+                                  _ptr(scores_out), _ptr(rep_out), _ptr(rep_lse), ws_ptr, ws_bytes, _stream(stream)))
 
 
 def herald_rep_attn_workspace_bytes(shape: Shape) -> int:

@@ -136,6 +136,53 @@ def test_select_xq_rejects_bad_arguments(H, cuda):
             H.herald_select_xq(*args(shape), x, k_per_seq, sel_idx, sel_cnt, None, ws)
 
 
+@pytest.mark.parametrize("case", ["tiny_ragged", "one_token", "g7_ragged", "g8_h8", "g1"])
+def test_select_rep_fused_matches_oracle(H, cuda, case):
+    """herald_select_rep: the paper's fused retrieval kernel -- one pass over K and V gives the
+    selection (same bar as herald_select, mode 0) AND the representative query's attention output (bar of herald_rep_attn)."""
+    c = SELECT_CASES[case]
+    w = c["w"]
+    inp = synth.make_inputs(w, seed=100 + len(case), device=cuda, spare_pages=c["spare"], hostile_tails=False)
+    pt = inp["page_table"].cpu().numpy()
+    for b, L in enumerate(w.seq_lens):      # hostile tails on both planes: huge K (must not be selected), NaN V (0 x NaN)
+        if L % 16:
+            inp["k_pages"][int(pt[b, L // 16]), L % 16:] = 16384.0
+            inp["v_pages"][int(pt[b, L // 16]), L % 16:] = float("nan")
+    ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
+    cap = max(max(ks), 1) + w.block_size
+    max_seq = (w.max_seq_len + 15) // 16 * 16
+    shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, max_seq, inp["page_table"].shape[1], cap, 0)
+    cache = H.make_cache(inp["k_pages"], inp["v_pages"], inp["page_table"], inp["seq_lens"])
+    k_per_seq = torch.tensor(ks, dtype=torch.int32, device=cuda)
+    sel_idx = torch.full((w.batch, w.n_kv_heads, cap), -7, dtype=torch.int32, device=cuda)
+    sel_cnt = torch.full((w.batch, w.n_kv_heads), -7, dtype=torch.int32, device=cuda)
+    scores = torch.full((w.batch, w.n_kv_heads, max(max_seq, 16)), float("nan"), dtype=torch.float32, device=cuda)
+    out = torch.full((w.batch, w.n_q_heads, 128), float("nan"), dtype=torch.float32, device=cuda)
+    lse = torch.full((w.batch, w.n_q_heads), float("nan"), dtype=torch.float32, device=cuda)
+    ws = H.alloc_workspace(H.herald_select_rep_workspace_bytes(shape), cuda)
+    H.herald_select_rep(shape, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, scores, out, lse, ws)
+    torch.cuda.synchronize()
+    oi = oracle_inputs(inp)
+    sel_o, sc_o = O.select(oi["q_rep"], oi["k_pages"], oi["page_table"], oi["seq_lens"], ks, w.n_kv_heads, 128 ** -0.5, 0)
+    ref, lse_ref = O.rep_attn(oi["q_rep"], oi["k_pages"], oi["v_pages"], oi["page_table"], oi["seq_lens"], w.n_kv_heads, 128 ** -0.5)
+    sel_g, cnt_g, sc_g = sel_idx.cpu().numpy(), sel_cnt.cpu().numpy(), scores.cpu().numpy()
+    differing = 0
+    for b, L in enumerate(w.seq_lens):
+        for h in range(w.n_kv_heads):
+            assert np.abs(sc_g[b, h, :L] - sc_o[b][h]).max() <= 1e-4, (case, b, h)
+            differing += check_selection(sel_g[b, h], int(cnt_g[b, h]), sc_o[b][h], ks[b], L, f"{case} b{b} h{h}")
+            assert np.all(sel_g[b, h, int(cnt_g[b, h]):] == -7)
+    assert differing <= max(1, w.batch * w.n_kv_heads // 4)
+    got, got_lse = out.cpu().numpy().astype(np.float64), lse.cpu().numpy().astype(np.float64)
+    assert np.isfinite(got).all() and np.abs(got - ref).max() <= 1e-4, (case, np.abs(got - ref).max())
+    fin = np.isfinite(lse_ref)
+    assert np.array_equal(np.isneginf(got_lse), ~fin) and np.abs(got_lse[fin] - lse_ref[fin]).max() <= 1e-3
+    # mode 1 is not defined for the fused pass
+    shape1 = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, max_seq, inp["page_table"].shape[1], cap, 1)
+    with pytest.raises(H.HeraldError):
+        H.herald_select_rep(shape1, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, scores, out, lse, ws)
+
+
 def test_select_edge_cases(H, cuda):
     # empty sequence, k = 0, k >= L (identity), k > pool capacity (clamped)
     w = synth.Workload("edge", 4, (0, 40, 33, 64), 4, 2, 16, 3, 100, "plain")
