@@ -139,6 +139,8 @@ static AttnGeom attn_geom(const herald_shape_t* s, bool dense = false) {
     // an M tile is `ipt` whole block rows x G heads (<= 128 rows), balanced over the tiles
     const int rows_cap = kTcBM / G;
     a.m_tiles = (s->block_size + rows_cap - 1) / rows_cap;
+    const int forced_mt = env_int("HERALD_ATTN_MTILES", 0);
+    if (forced_mt > a.m_tiles && forced_mt <= s->block_size) a.m_tiles = forced_mt;
     a.ipt = (s->block_size + a.m_tiles - 1) / a.m_tiles;
     // one CTA per SM: split the keys of a unit over a cluster until the grid covers the 148 SMs once
     const int max_keys = dense ? s->max_seq_len : s->pool_capacity;
