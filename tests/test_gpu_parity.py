@@ -183,6 +183,56 @@ def test_select_rep_fused_matches_oracle(H, cuda, case):
         H.herald_select_rep(shape1, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, scores, out, lse, ws)
 
 
+@pytest.mark.parametrize("name,seqs", [("C2", (0, 5)), ("C3", (3,))])
+def test_full_size_fused_retrieval_and_xq_sampled(H, cuda, name, seqs):
+    """BASELINE.json sizes, the launch configuration bench.py times: herald_select_rep (fused pass), herald_rep_attn and
+    herald_select_xq at x = 32 (tcgen05 scan) on the whole batch; the oracle recomputes sampled sequences from exactly
+    their bytes (pages re-indexed 0..n-1)."""
+    w = synth.config(name)
+    inp = synth.make_inputs(w, seed=21633 + 77, device=cuda, with_block_inputs=False)
+    ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
+    cap = max(ks) + w.block_size
+    max_seq = (w.max_seq_len + 15) // 16 * 16
+    shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, max_seq, inp["page_table"].shape[1], cap, 0)
+    cache = H.make_cache(inp["k_pages"], inp["v_pages"], inp["page_table"], inp["seq_lens"])
+    k_per_seq = torch.tensor(ks, dtype=torch.int32, device=cuda)
+    mk = lambda: (torch.full((w.batch, w.n_kv_heads, cap), -7, dtype=torch.int32, device=cuda),
+                  torch.full((w.batch, w.n_kv_heads), -7, dtype=torch.int32, device=cuda),
+                  torch.full((w.batch, w.n_kv_heads, max_seq), float("nan"), dtype=torch.float32, device=cuda))
+    sel_f, cnt_f, sc_f = mk()
+    out_f = torch.full((w.batch, w.n_q_heads, 128), float("nan"), dtype=torch.float32, device=cuda)
+    lse_f = torch.full((w.batch, w.n_q_heads), float("nan"), dtype=torch.float32, device=cuda)
+    ws = H.alloc_workspace(H.herald_select_rep_workspace_bytes(shape), cuda)
+    H.herald_select_rep(shape, cache, inp["q_rep"], k_per_seq, sel_f, cnt_f, sc_f, out_f, lse_f, ws)
+    out_r = torch.full_like(out_f, float("nan"))
+    H.herald_rep_attn(shape, cache, inp["q_rep"], out_r, None, ws)
+    x = 32 if 32 * w.group <= 256 else 256 // w.group
+    q_x = synth.make_q_x(inp["q_rep"], x, seed=5)
+    sel_x, cnt_x, sc_x = mk()
+    H.herald_select_xq(shape, cache, q_x, x, k_per_seq, sel_x, cnt_x, sc_x, ws)
+    torch.cuda.synchronize()
+    assert torch.equal(out_f, out_r)          # the fused pass and the plain one run the same arithmetic on the V side
+    pt = inp["page_table"].cpu().numpy()
+    differing = 0
+    for b in seqs:
+        L = w.seq_lens[b]
+        n_pages = (L + 15) // 16
+        phys = torch.from_numpy(pt[b, :n_pages].astype(np.int64)).to(cuda)
+        kp, vp = synth.to_u16(inp["k_pages"][phys]), synth.to_u16(inp["v_pages"][phys])
+        ident = np.arange(n_pages, dtype=np.int32)[None, :]
+        q1 = synth.to_u16(inp["q_rep"][b:b + 1])
+        _, sc_o = O.select(q1, kp, ident, np.array([L]), [ks[b]], w.n_kv_heads, 128 ** -0.5, 0)
+        ref, lse_ref = O.rep_attn(q1, kp, vp, ident, np.array([L]), w.n_kv_heads, 128 ** -0.5)
+        _, scx_o = O.select_xq(synth.to_u16(q_x[b:b + 1]), kp, ident, np.array([L]), [ks[b]], w.n_kv_heads, 128 ** -0.5)
+        assert np.abs(out_f[b].cpu().numpy().astype(np.float64) - ref[0]).max() <= 1e-4
+        assert np.abs(lse_f[b].cpu().numpy().astype(np.float64) - lse_ref[0]).max() <= 1e-3
+        for h in range(w.n_kv_heads):
+            for sc_g, sel_g, cnt_g, sc_ref, tag in ((sc_f, sel_f, cnt_f, sc_o[0][h], "fused"), (sc_x, sel_x, cnt_x, scx_o[0][h], "xq")):
+                assert np.abs(sc_g[b, h, :L].cpu().numpy() - sc_ref).max() <= 1e-4, (name, tag, b, h)
+                differing += check_selection(sel_g[b, h].cpu().numpy(), int(cnt_g[b, h]), sc_ref, ks[b], L, f"{name} {tag} b{b} h{h}")
+    assert differing <= max(1, len(seqs) * w.n_kv_heads // 2)
+
+
 def test_select_edge_cases(H, cuda):
     # empty sequence, k = 0, k >= L (identity), k > pool capacity (clamped)
     w = synth.Workload("edge", 4, (0, 40, 33, 64), 4, 2, 16, 3, 100, "plain")
