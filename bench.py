@@ -400,7 +400,10 @@ def main():
     ws_fused = H.alloc_workspace(H.herald_select_rep_workspace_bytes(shape), dev)
     select_rep_fused_ms = time_isolated(lambda: H.herald_select_rep(shape, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, None, rep_out, None,
                                                                     ws_fused, side), reps=4, warm=2, timed=3)
-    del ws_fused
+    ws_fused_m1 = H.alloc_workspace(H.herald_select_rep_workspace_bytes(shape_m1), dev)
+    select_rep_fused_m1_ms = time_isolated(lambda: H.herald_select_rep(shape_m1, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, None, rep_out, None,
+                                                                       ws_fused_m1, side), reps=4, warm=2, timed=3)
+    del ws_fused, ws_fused_m1
     # NEXT-4: the selection kernel against the number of queries x (Fig. 8: 32 -> 1 gives 8x on the CPU)
     xq_sweep = {}
     for x in (1, 2, 4, 8, 16, 32):
@@ -501,7 +504,7 @@ def main():
             "overlap_efficiency": (denoise_alone_ms + select_alone_ms + gather_alone_ms_block - ms_step) / (select_alone_ms + gather_alone_ms_block),
             "n_layers": n_layers,
             "rep_attn_ms": rep_attn_ms, "rep_attn_gbs": tokens * w.n_kv_heads * 512 / (rep_attn_ms * 1e-3) / 1e9,
-            "select_rep_fused_ms": select_rep_fused_ms, "select_plus_rep_separate_ms": select_alone_ms / n_layers + rep_attn_ms,
+            "select_rep_fused_ms": select_rep_fused_ms, "select_rep_fused_softmax_sum_mode_ms": select_rep_fused_m1_ms, "select_plus_rep_separate_ms": select_alone_ms / n_layers + rep_attn_ms,
             "select_xq_sweep": xq_sweep,
             "dense_attn_full_cache_ms": dense_attn_ms, "dense_attn_tflops": dense_flops / (dense_attn_ms * 1e-3) / 1e12,
             "attn_time_share_alone": attn_share,

@@ -167,9 +167,9 @@ int herald_rep_attn(const herald_shape_t* shape, const herald_cache_t* cache, co
 
 /* The fused retrieval kernel (section IV-B4: the selection kernel "maintains the FlashAttention
  * statistics (m_g, l_g, o_g)" next to the raw scores): ONE pass over K and V gives both what herald_select gives
- * (scores, sel_idx, sel_cnt; max-logit aggregation only: shape->agg_mode must be HERALD_AGG_MAX_LOGIT, else UNSUPPORTED)
- * and what herald_rep_attn gives (rep_out [batch][H_q][128] fp32, optional rep_lse [batch][H_q]).  K is read once
- * instead of twice.  Arguments as in those two entries; ws >= herald_select_rep_workspace_bytes(shape), 256-byte aligned. */
+ * (scores, sel_idx, sel_cnt, either aggregation) and what herald_rep_attn gives (rep_out [batch][H_q][128] fp32,
+ * optional rep_lse [batch][H_q]).  K is read once instead of twice.  With HERALD_AGG_SOFTMAX_SUM the pass keeps the
+ * per-head logits in the workspace and one more kernel, after the statistics are final, forms sum_g exp(s - lse_g).  Arguments as in those two entries; ws >= herald_select_rep_workspace_bytes(shape), 256-byte aligned. */
 size_t herald_select_rep_workspace_bytes(const herald_shape_t* shape);
 int herald_select_rep(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep, const int32_t* k_per_seq,
                       int32_t* sel_idx, int32_t* sel_cnt, float* scores_out, float* rep_out, float* rep_lse,

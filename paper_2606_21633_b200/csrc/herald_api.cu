@@ -794,11 +794,12 @@ size_t herald_rep_attn_workspace_bytes(const herald_shape_t* shape) {
 // `between` (herald_select_rep: the top-k, launched programmatically) runs after the pass and before the merge is enqueued;
 // the merge then starts beside it and does not wait for it.
 static int rep_attn_launch(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep, float* out, float* lse,
-                           void* ws, float* scores, uint32_t* hist1, cudaStream_t stream, const std::function<int()>& between,
-                           bool has_between) {
+                           void* ws, float* scores, uint32_t* hist1, float* raw, cudaStream_t stream,
+                           const std::function<int()>& between, bool has_between) {
     RepAttnParams rp{};
     rp.scores = scores;
     rp.hist1 = hist1;
+    rp.raw = raw;
     rp.sm_scale = shape->sm_scale;
     rp.merge_waits = has_between ? 0 : 1;
     rp.k_pages = static_cast<const __nv_bfloat16*>(cache->k_pages);
@@ -861,12 +862,14 @@ int herald_rep_attn(const herald_shape_t* shape, const herald_cache_t* cache, co
     if (ws_bytes < need) return fail(HERALD_ERR_WORKSPACE_TOO_SMALL, "herald_rep_attn: workspace %zu < %zu", ws_bytes, need);
     if (shape->batch * shape->n_kv_heads == 0) return HERALD_OK;
     g_err[0] = 0;
-    return rep_attn_launch(shape, cache, q_rep, out, lse, ws, nullptr, nullptr, static_cast<cudaStream_t>(stream_), [] { return 0; }, false);
+    return rep_attn_launch(shape, cache, q_rep, out, lse, ws, nullptr, nullptr, nullptr, static_cast<cudaStream_t>(stream_), [] { return 0; }, false);
 }
 
 size_t herald_select_rep_workspace_bytes(const herald_shape_t* shape) {
     if (check_shape(shape) != HERALD_OK) return 0;
-    return align_up(select_ws_layout(shape).total, 256) + herald_rep_attn_workspace_bytes(shape);
+    // select workspace, rep_attn partials, and a log-sum-exp per query head (mode 1 needs it even when the caller does not)
+    return align_up(select_ws_layout(shape).total, 256) + herald_rep_attn_workspace_bytes(shape) +
+           align_up((size_t)(shape->batch > 0 ? shape->batch : 1) * shape->n_q_heads * sizeof(float), 256);
 }
 
 int herald_select_rep(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep, const int32_t* k_per_seq,
@@ -879,8 +882,6 @@ int herald_select_rep(const herald_shape_t* shape, const herald_cache_t* cache, 
     if (!q_rep || !k_per_seq || !sel_idx || !sel_cnt || !rep_out || !ws) return fail(HERALD_ERR_INVALID_ARG, "herald_select_rep: NULL pointer");
     if (!aligned16(q_rep) || !aligned16(sel_idx) || !aligned16(scores_out) || !aligned16(rep_out) || (reinterpret_cast<uintptr_t>(ws) & 255u))
         return fail(HERALD_ERR_INVALID_ARG, "herald_select_rep: misaligned pointer (16 B; workspace 256 B)");
-    if (shape->agg_mode != HERALD_AGG_MAX_LOGIT)
-        return fail(HERALD_ERR_UNSUPPORTED, "herald_select_rep: the fused pass aggregates by max-logit (agg_mode 0) only");
     const size_t need = herald_select_rep_workspace_bytes(shape);
     if (ws_bytes < need) return fail(HERALD_ERR_WORKSPACE_TOO_SMALL, "herald_select_rep: workspace %zu < %zu", ws_bytes, need);
     const int units = shape->batch * shape->n_kv_heads;
@@ -893,9 +894,37 @@ int herald_select_rep(const herald_shape_t* shape, const herald_cache_t* cache, 
     float* scores = scores_out ? scores_out : reinterpret_cast<float*>(wsb + w.scores);
     cudaError_t e = cudaMemsetAsync(hist1, 0, (size_t)units * kBins1 * sizeof(uint32_t), stream);
     if (e != cudaSuccess) return cuda_fail(e, "memset hist1");
-    // pass (scores + histogram + partials) -> top-k, launched programmatically behind the pass -> merge, beside the top-k
-    return rep_attn_launch(shape, cache, q_rep, rep_out, rep_lse, wsb + align_up(w.total, 256), scores, hist1, stream,
-                           [&] { return launch_topk(shape, cache, scores, hist1, k_per_seq, sel_idx, sel_cnt, stream, true); }, true);
+    uint8_t* ws_rep = wsb + align_up(w.total, 256);
+    if (shape->agg_mode == HERALD_AGG_MAX_LOGIT) {
+        // pass (scores + histogram + partials) -> top-k, launched programmatically behind the pass -> merge, beside the top-k
+        return rep_attn_launch(shape, cache, q_rep, rep_out, rep_lse, ws_rep, scores, hist1, nullptr, stream,
+                               [&] { return launch_topk(shape, cache, scores, hist1, k_per_seq, sel_idx, sel_cnt, stream, true); }, true);
+    }
+    // softmax-sum aggregation: a[t] = sum_g exp(s[g,t] - m_g) / l_g needs the finished (m_g, l_g), i.e. the
+    // log-sum-exp the merge produces.  The pass keeps the per-head logits; after the merge one more kernel turns them into
+    // the score plane and its histogram; then the top-k.
+    float* lse_buf = rep_lse ? rep_lse : reinterpret_cast<float*>(ws_rep + herald_rep_attn_workspace_bytes(shape));
+    float* raw = reinterpret_cast<float*>(wsb + w.raw);
+    rc = rep_attn_launch(shape, cache, q_rep, rep_out, lse_buf, ws_rep, nullptr, nullptr, raw, stream, [] { return 0; }, false);
+    if (rc) return rc;
+    if (shape->max_seq_len > 0) {
+        AggParams ap{};
+        ap.raw = raw;
+        ap.lse = lse_buf;
+        ap.batch = shape->batch;
+        ap.seq_lens = cache->seq_lens;
+        ap.scores = scores;
+        ap.hist1 = hist1;
+        ap.n_q_heads = shape->n_q_heads;
+        ap.n_kv_heads = shape->n_kv_heads;
+        ap.max_seq_len = shape->max_seq_len;
+        int chunks = (shape->max_seq_len + 256 * 8 - 1) / (256 * 8);
+        if (chunks < 1) chunks = 1;
+        aggregate_softmax_kernel<<<dim3(chunks, shape->n_kv_heads, shape->batch), 256, 0, stream>>>(ap);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(e, "aggregate launch");
+    }
+    return launch_topk(shape, cache, scores, hist1, k_per_seq, sel_idx, sel_cnt, stream);
 }
 
 // Longest-pool-first unit order of one layer into `order` (device, [units]); enqueued on `stream`.

@@ -53,6 +53,7 @@ struct RepAttnParams {
     float* lse;           // optional [batch][H_q]
     float* scores;        // optional [units][max_seq_len]: the selection scores of the same pass (herald_select_rep), mode 0
     uint32_t* hist1;      // with scores: [units][kBins1] level-1 histogram of the top-k (zeroed before the launch)
+    float* raw;           // optional [units][G][max_seq_len]: the per-head scaled logits, for the softmax-sum aggregation (mode 1)
     float sm_scale;
     int32_t merge_waits;  // the merge grid waits for its predecessor (0: it is launched behind a grid that already did)
     int32_t batch, n_q_heads, n_kv_heads, max_seq_len, max_pages, hg;
@@ -168,6 +169,14 @@ __global__ void __launch_bounds__(kRepThreads, 2) rep_attn_kernel(const RepAttnP
             // sa[0], sa[1]: head g, tokens 2tig, 2tig+1 ; sb[0], sb[1]: tokens 8+2tig, 9+2tig.  Mask the tail of the last page.
             const int t0 = page * kPageSize + 2 * tig;
             const bool ok0 = t0 < t_end, ok1 = t0 + 1 < t_end, ok2 = t0 + 8 < t_end, ok3 = t0 + 9 < t_end;
+            if (p.raw && g < G) {
+                // mode 1: a[t] = sum_g exp(s[g,t] - lse_g) needs the finished statistics; keep the logits
+                float* rr = p.raw + ((int64_t)(b * p.n_kv_heads + h) * G + g) * p.max_seq_len + t0;
+                if (ok0) rr[0] = sa[0] * p.sm_scale;
+                if (ok1) rr[1] = sa[1] * p.sm_scale;
+                if (ok2) rr[8] = sb[0] * p.sm_scale;
+                if (ok3) rr[9] = sb[1] * p.sm_scale;
+            }
             if (p.scores) {
                 // the fused retrieval kernel: the raw scores of this pass are the selection scores too;
                 // max-logit aggregation = maximum over the G heads = over the lanes with equal tig

@@ -289,6 +289,7 @@ struct AggParams {
     const float* raw;
     const float2* stats_part;
     int32_t n_parts;      // grid size of the scan that wrote stats_part
+    const float* lse;     // optional [batch][H_q]: finished log-sum-exp per head (herald_select_rep); replaces stats_part
     const int32_t* seq_lens;
     float* scores;
     uint32_t* hist1;
@@ -303,7 +304,12 @@ __global__ void __launch_bounds__(256) aggregate_softmax_kernel(const AggParams 
     const int G = p.n_q_heads / p.n_kv_heads;
     const int L = min(p.seq_lens[b], p.max_seq_len);
     for (int i = threadIdx.x; i < kBins1; i += blockDim.x) s_hist[i] = 0;
-    if (threadIdx.x < G) {
+    if (p.lse) {
+        if (threadIdx.x < G) {   // exp(s - m) / l with m = lse, l = 1
+            s_m[threadIdx.x] = p.lse[(int64_t)b * p.n_q_heads + h * G + threadIdx.x];
+            s_inv_l[threadIdx.x] = 1.f;
+        }
+    } else if (threadIdx.x < G) {
         // the scan CTAs whose tile range intersects this unit wrote a partial (same range arithmetic as scan_kernel)
         int64_t total = 0, unit_begin = 0;
         for (int bb = 0; bb < p.batch; ++bb) {
