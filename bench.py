@@ -396,6 +396,15 @@ def main():
     rep_out = torch.empty((w.batch, w.n_q_heads, 128), dtype=torch.float32, device=dev)
     ws_rep = H.alloc_workspace(H.herald_rep_attn_workspace_bytes(shape), dev)
     rep_attn_ms = time_isolated(lambda: H.herald_rep_attn(shape, cache, inp["q_rep"], rep_out, None, ws_rep, side), reps=4, warm=2, timed=3)
+    # the 2B-token step: denoising group + draft group over the same pools, one launch against two
+    q2 = torch.stack([inp["q_blk"][0], inp["q_blk"][1 % n_steps]]).contiguous()
+    kb2 = torch.stack([inp["k_blk"][0], inp["k_blk"][1 % n_steps]]).contiguous()
+    vb2 = torch.stack([inp["v_blk"][0], inp["v_blk"][1 % n_steps]]).contiguous()
+    out2 = torch.empty((2,) + tuple(out1.shape), dtype=torch.float32, device=dev)
+    ws_att2 = H.alloc_workspace(2 * H.herald_attn_workspace_bytes(shape), dev)
+    attn_2b_ms = time_isolated(lambda: H.herald_sparse_attn_groups(shape, 2, pipe.pools_k[0][pipe.active], pipe.pools_v[0][pipe.active],
+                                                                   pipe.pool_lens[0][pipe.active], q2, kb2, vb2, out2, None, ws_att2, side))
+    del q2, kb2, vb2, out2, ws_att2
     # the paper's fused retrieval kernel: selection and the representative query's output from ONE pass over K and V
     ws_fused = H.alloc_workspace(H.herald_select_rep_workspace_bytes(shape), dev)
     select_rep_fused_ms = time_isolated(lambda: H.herald_select_rep(shape, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, None, rep_out, None,
@@ -504,6 +513,7 @@ def main():
             "overlap_efficiency": (denoise_alone_ms + select_alone_ms + gather_alone_ms_block - ms_step) / (select_alone_ms + gather_alone_ms_block),
             "n_layers": n_layers,
             "rep_attn_ms": rep_attn_ms, "rep_attn_gbs": tokens * w.n_kv_heads * 512 / (rep_attn_ms * 1e-3) / 1e9,
+            "attn_2b_step_one_launch_ms": attn_2b_ms,
             "select_rep_fused_ms": select_rep_fused_ms, "select_rep_fused_softmax_sum_mode_ms": select_rep_fused_m1_ms, "select_plus_rep_separate_ms": select_alone_ms / n_layers + rep_attn_ms,
             "select_xq_sweep": xq_sweep,
             "dense_attn_full_cache_ms": dense_attn_ms, "dense_attn_tflops": dense_flops / (dense_attn_ms * 1e-3) / 1e12,

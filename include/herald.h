@@ -145,6 +145,19 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
                        const int32_t* pool_len, const void* q_blk, const void* k_blk, const void* v_blk,
                        float* out, float* lse, void* ws, size_t ws_bytes, herald_stream_t stream);
 
+/* The same attention for n_groups query groups that share the prefix (the step after the draft is formed
+ * runs "as a 2B-token forward pass ... the denoising group and the draft group use different custom attention masks: both
+ * groups attend to the KV cache of the completed prefix but not to each other"): ONE launch in which group g, sequence b
+ * attends over the pools of sequence b and over its OWN in-block rows,
+ *   out[g][b][i][hq][:] = softmax_j( sm_scale * q_blk[g][b][i][hq][:] . K'_j ) . V'_j,
+ *   K' = pool_k[b][h][0 .. pool_len[b][h]) followed by k_blk[g][b][0..B)[h].
+ *   q_blk bf16 [n_groups][batch][B][H_q][128]; k_blk, v_blk bf16 [n_groups][batch][B][H_kv][128]
+ *   out fp32 [n_groups][batch][B][H_q][128]; lse optional fp32 [n_groups][batch][B][H_q]; pools and pool_len as above.
+ *   ws >= n_groups * herald_attn_workspace_bytes(shape), 256-byte aligned.  n_groups = 1 is herald_sparse_attn. */
+int herald_sparse_attn_groups(const herald_shape_t* shape, int32_t n_groups, const void* pool_k, const void* pool_v,
+                              const int32_t* pool_len, const void* q_blk, const void* k_blk, const void* v_blk,
+                              float* out, float* lse, void* ws, size_t ws_bytes, herald_stream_t stream);
+
 /* Dense attention of the block queries over the FULL paged cache + in-block KV, for layers that keep their whole KV
  * ("the first two layers ... retain the full KV cache"; = herald_sparse_attn at a 100 % budget without
  * the gather):

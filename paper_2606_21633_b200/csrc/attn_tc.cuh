@@ -101,6 +101,8 @@ struct AttnParams {
     float* out;
     float* lse;
     int32_t n_q_heads, n_kv_heads, block_size, cap, n_splits;
+    int32_t pool_batch; // sequences that own pools / cache pages: query sequence b reads those of b % pool_batch (query groups
+                        // that share the prefix; == batch otherwise)
     int32_t ipt;        // block rows per M tile (ipt * G <= 128)
     int32_t pool_box;   // rows of the pool tensor-map box: min(cap, 128)
     float scale_log2;   // sm_scale * log2(e)
@@ -368,8 +370,9 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     // pool, so that the long units start first and the short ones fill the tail of a multi-wave grid
     const int unit = p.unit_order ? p.unit_order[blockIdx.z] : (int)blockIdx.z;
     const int b = unit / p.n_kv_heads, h = unit % p.n_kv_heads;
+    const int b_pool = b % p.pool_batch, unit_pool = b_pool * p.n_kv_heads + h;   // whose keys: the group's prefix owner
     const bool paged = p.page_table != nullptr;
-    const int n_pool = paged ? max(0, min(p.seq_lens[b], p.max_seq_len)) : max(0, min(p.pool_len[unit], p.cap));
+    const int n_pool = paged ? max(0, min(p.seq_lens[b_pool], p.max_seq_len)) : max(0, min(p.pool_len[unit_pool], p.cap));
     const int n_tiles = 1 + (n_pool + kTcBN - 1) / kTcBN;    // key tile 0 = the in-block rows, tile t >= 1 = pool rows [128(t-1), 128t)
     const int per = (n_tiles + S - 1) / S;
     const int t0 = split * per, t1 = min(n_tiles, t0 + per);
@@ -423,8 +426,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                         tma_load_4d(dst + kTcHalfBytes, map_blk, 64, h, 0, b, land);
                     } else if (!paged) {   // pool rows: box = (64 channels, pool_box rows, 1 unit) per half; rows past cap are zero-filled
                         mbar_arrive_expect_tx(land, (uint32_t)p.pool_box * 256u);
-                        tma_load_3d(dst, map, 0, (t - 1) * kTcBN, unit, land);
-                        tma_load_3d(dst + kTcHalfBytes, map, 64, (t - 1) * kTcBN, unit, land);
+                        tma_load_3d(dst, map, 0, (t - 1) * kTcBN, unit_pool, land);
+                        tma_load_3d(dst + kTcHalfBytes, map, 64, (t - 1) * kTcBN, unit_pool, land);
                     }
                 }
                 __syncwarp();
@@ -432,7 +435,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                     // dense mode: the 128 tokens of the tile are 8 pages of the cache; page i lands on tile rows [16i, 16i+16)
                     // (2 KB per half: a whole number of 1 KB swizzle atoms).  Pages past the sequence are not requested.
                     const int page0 = (t - 1) * (kTcBN / kPageSize), n_pg = (valid + kPageSize - 1) / kPageSize;
-                    const int my_phys = lane < n_pg ? __ldg(p.page_table + (int64_t)b * p.max_pages + page0 + lane) : 0;
+                    const int my_phys = lane < n_pg ? __ldg(p.page_table + (int64_t)b_pool * p.max_pages + page0 + lane) : 0;
                     if (lane == 0) mbar_arrive_expect_tx(land, (uint32_t)n_pg * kPageSize * 256u);
                     __syncwarp();
                     if (lane < n_pg) {

@@ -621,8 +621,10 @@ int herald_gather(const herald_shape_t* shape, const herald_cache_t* cache, cons
 static int sparse_attn_impl(const herald_shape_t* shape, const void* pool_k, const void* pool_v, const int32_t* pool_len,
                             const void* q_blk, const void* k_blk, const void* v_blk, float* out, float* lse, void* ws,
                             size_t ws_bytes, herald_stream_t stream_, const int32_t* unit_order,
-                            const herald_cache_t* dense_cache = nullptr) {
+                            const herald_cache_t* dense_cache = nullptr, int pool_batch = 0) {
     const bool dense = dense_cache != nullptr;
+    if (pool_batch <= 0) pool_batch = shape->batch;           // every query sequence has its own pools / pages
+    const int units_pool = pool_batch * shape->n_kv_heads;
     int rc = check_shape(shape);
     if (rc) return rc;
     if (!pool_k || !pool_v || (!dense && !pool_len) || !q_blk || !k_blk || !v_blk || !out || !ws)
@@ -644,9 +646,9 @@ static int sparse_attn_impl(const herald_shape_t* shape, const void* pool_k, con
         attr_set = true;
     }
     CUtensorMap tm_k, tm_v, tm_q, tm_kb, tm_vb;
-    rc = dense ? make_paged_map(&tm_k, pool_k, dense_cache, shape->n_kv_heads) : make_pool_map(&tm_k, pool_k, units, shape->pool_capacity);
+    rc = dense ? make_paged_map(&tm_k, pool_k, dense_cache, shape->n_kv_heads) : make_pool_map(&tm_k, pool_k, units_pool, shape->pool_capacity);
     if (rc) return rc;
-    rc = dense ? make_paged_map(&tm_v, pool_v, dense_cache, shape->n_kv_heads) : make_pool_map(&tm_v, pool_v, units, shape->pool_capacity);
+    rc = dense ? make_paged_map(&tm_v, pool_v, dense_cache, shape->n_kv_heads) : make_pool_map(&tm_v, pool_v, units_pool, shape->pool_capacity);
     if (rc) return rc;
     rc = make_q_map(&tm_q, q_blk, shape, a.ipt);
     if (rc) return rc;
@@ -668,6 +670,7 @@ static int sparse_attn_impl(const herald_shape_t* shape, const void* pool_k, con
     ap.block_size = shape->block_size;
     ap.cap = shape->pool_capacity;
     ap.n_splits = a.n_splits;
+    ap.pool_batch = pool_batch;
     ap.ipt = a.ipt;
     ap.pool_box = shape->pool_capacity < kTcBN ? (shape->pool_capacity > 0 ? shape->pool_capacity : 1) : kTcBN;
     ap.scale_log2 = shape->sm_scale * 1.4426950408889634f;
@@ -707,6 +710,19 @@ int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const vo
                        const void* q_blk, const void* k_blk, const void* v_blk, float* out, float* lse, void* ws,
                        size_t ws_bytes, herald_stream_t stream_) {
     return sparse_attn_impl(shape, pool_k, pool_v, pool_len, q_blk, k_blk, v_blk, out, lse, ws, ws_bytes, stream_, nullptr);
+}
+
+int herald_sparse_attn_groups(const herald_shape_t* shape, int32_t n_groups, const void* pool_k, const void* pool_v,
+                              const int32_t* pool_len, const void* q_blk, const void* k_blk, const void* v_blk, float* out,
+                              float* lse, void* ws, size_t ws_bytes, herald_stream_t stream) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    if (n_groups < 1 || (int64_t)n_groups * shape->batch > (1 << 20))
+        return fail(HERALD_ERR_INVALID_ARG, "herald_sparse_attn_groups: n_groups = %d", n_groups);
+    herald_shape_t grouped = *shape;                          // the query side sees n_groups * batch sequences,
+    grouped.batch = shape->batch * n_groups;                  // sequence b of group g reads the pools of sequence b
+    return sparse_attn_impl(&grouped, pool_k, pool_v, pool_len, q_blk, k_blk, v_blk, out, lse, ws, ws_bytes, stream, nullptr,
+                            nullptr, shape->batch);
 }
 
 int herald_dense_attn(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_blk, const void* k_blk,

@@ -24,7 +24,7 @@ OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE_TOO_SMALL, ERR_CUDA = 0, -1,
 AGG_MAX_LOGIT, AGG_SOFTMAX_SUM = 0, 1
 
 EXPORTS = ("herald_last_error", "herald_budget_rows", "herald_select_workspace_bytes",
-           "herald_attn_workspace_bytes", "herald_attn_grid_ctas", "herald_select", "herald_select_xq", "herald_gather", "herald_sparse_attn",
+           "herald_attn_workspace_bytes", "herald_attn_grid_ctas", "herald_select", "herald_select_xq", "herald_gather", "herald_sparse_attn", "herald_sparse_attn_groups",
            "herald_dense_attn", "herald_rep_attn_workspace_bytes", "herald_rep_attn",
            "herald_select_rep_workspace_bytes", "herald_select_rep",
            "herald_cache_write_block", "herald_pool_append_block",
@@ -98,6 +98,8 @@ _lib.herald_gather.argtypes = [C.POINTER(Shape), C.POINTER(Cache), C.c_void_p, C
                                C.c_void_p, C.c_void_p]
 _lib.herald_sparse_attn.restype = C.c_int
 _lib.herald_sparse_attn.argtypes = [C.POINTER(Shape)] + [C.c_void_p] * 9 + [C.c_size_t, C.c_void_p]
+_lib.herald_sparse_attn_groups.restype = C.c_int
+_lib.herald_sparse_attn_groups.argtypes = [C.POINTER(Shape), C.c_int32] + [C.c_void_p] * 9 + [C.c_size_t, C.c_void_p]
 _lib.herald_dense_attn.restype = C.c_int
 _lib.herald_dense_attn.argtypes = [C.POINTER(Shape), C.POINTER(Cache)] + [C.c_void_p] * 6 + [C.c_size_t, C.c_void_p]
 _lib.herald_rep_attn_workspace_bytes.restype = C.c_size_t
@@ -199,6 +201,12 @@ def herald_select_xq(shape, cache, q_x, x, k_per_seq, sel_idx, sel_cnt, scores_o
 def herald_gather(shape, cache, sel_idx, sel_cnt, pool_k, pool_v, stream=None):
     _check(_lib.herald_gather(C.byref(shape), C.byref(cache), _ptr(sel_idx), _ptr(sel_cnt), _ptr(pool_k),
                               _ptr(pool_v), _stream(stream)))
+
+
+def herald_sparse_attn_groups(shape, n_groups, pool_k, pool_v, pool_len, q_blk, k_blk, v_blk, out, lse, ws, stream=None):
+    ws_ptr, ws_bytes = _ws(ws)
+    _check(_lib.herald_sparse_attn_groups(C.byref(shape), int(n_groups), _ptr(pool_k), _ptr(pool_v), _ptr(pool_len), _ptr(q_blk),
+                                          _ptr(k_blk), _ptr(v_blk), _ptr(out), _ptr(lse), ws_ptr, ws_bytes, _stream(stream)))
 
 
 def herald_sparse_attn(shape, pool_k, pool_v, pool_len, q_blk, k_blk, v_blk, out, lse, ws, stream=None):

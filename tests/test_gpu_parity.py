@@ -366,6 +366,38 @@ def test_sparse_attn_split_kv_is_consistent(H, cuda, splits, monkeypatch):
     assert np.abs(out.cpu().numpy() - ref).max() <= ATTN_TOL
 
 
+@pytest.mark.parametrize("n_groups", [1, 2, 3])
+def test_sparse_attn_groups_share_the_pools(H, cuda, n_groups):
+    """herald_sparse_attn_groups: the denoising group and the draft group of the 2B-token step attend over the
+    same prefix pools and over their own in-block rows, not over each other -- one launch equals one oracle call per group."""
+    batch, B, Hq, Hkv, cap = 2, 32, 28, 4, 700
+    q, kb, vb, pk, pv, pl = _attn_case(cuda, batch, B, Hq, Hkv, cap, [[700, 1, 333, 64], [63, 65, 0, 512]], seed=91)
+    gen = torch.Generator(device=cuda)
+    gen.manual_seed(92)
+    rn = lambda *sh: torch.randn(*sh, generator=gen, device=cuda, dtype=torch.float32).to(torch.bfloat16)
+    qg, kbg, vbg = rn(n_groups, batch, B, Hq, 128), rn(n_groups, batch, B, Hkv, 128), rn(n_groups, batch, B, Hkv, 128)
+    qg[0], kbg[0], vbg[0] = q, kb, vb
+    shape = H.make_shape(batch, Hq, Hkv, B, 16, 1, cap)
+    out = torch.full((n_groups, batch, B, Hq, 128), float("nan"), dtype=torch.float32, device=cuda)
+    lse = torch.full((n_groups, batch, B, Hq), float("nan"), dtype=torch.float32, device=cuda)
+    ws = H.alloc_workspace(n_groups * H.herald_attn_workspace_bytes(shape), cuda)
+    H.herald_sparse_attn_groups(shape, n_groups, pk, pv, pl, qg, kbg, vbg, out, lse, ws)
+    torch.cuda.synchronize()
+    pv_clean = pv.clone()
+    pv_clean[torch.isnan(pv_clean)] = 0
+    for g in range(n_groups):
+        ref, lse_ref = O.sparse_attn(synth.to_u16(qg[g]), synth.to_u16(kbg[g]), synth.to_u16(vbg[g]), synth.to_u16(pk),
+                                     synth.to_u16(pv_clean), pl.cpu().numpy(), 128 ** -0.5)
+        err = np.abs(out[g].cpu().numpy().astype(np.float64) - ref).max()
+        assert np.isfinite(err) and err <= ATTN_TOL, (g, err)
+        assert np.abs(lse[g].cpu().numpy() - lse_ref).max() <= 2e-3
+    if n_groups == 1:     # one group is herald_sparse_attn, bit for bit
+        out1 = torch.empty((batch, B, Hq, 128), dtype=torch.float32, device=cuda)
+        H.herald_sparse_attn(shape, pk, pv, pl, q, kb, vb, out1, None, ws)
+        torch.cuda.synchronize()
+        assert torch.equal(out1, out[0])
+
+
 @pytest.mark.parametrize("splits", [7, 8])
 def test_sparse_attn_more_splits_than_tile_rows(H, cuda, splits, monkeypatch):
     """G = 1, B = 8: the M tile has 8 real rows, so with 7 or 8 KV splits some CTAs of the cluster own no row at all;
