@@ -121,6 +121,39 @@ def test_select_xq_matches_oracle(H, cuda, case, x, path, monkeypatch):
         assert torch.equal(sel1, sel_idx) and torch.equal(cnt1, sel_cnt)
 
 
+@pytest.mark.parametrize("ctas", [1, 5, 37])
+def test_select_xq_small_grids(H, cuda, ctas, monkeypatch):
+    """Grids smaller than H_kv (no CTA sets), not a multiple of it (idle CTAs past the last set), and a single CTA."""
+    monkeypatch.setenv("HERALD_SCAN_CTAS", str(ctas))
+    for path in ("0", "1"):
+        monkeypatch.setenv("HERALD_XQ_TC", path)
+        c = SELECT_CASES["g8_h8"]
+        w = c["w"]
+        inp = synth.make_inputs(w, seed=321, device=cuda, spare_pages=1, hostile_tails=True)
+        x = 6
+        q_x = synth.make_q_x(inp["q_rep"], x, seed=12)
+        ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
+        cap = max(ks) + w.block_size
+        max_seq = (w.max_seq_len + 15) // 16 * 16
+        shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, max_seq, inp["page_table"].shape[1], cap, 0)
+        cache = H.make_cache(inp["k_pages"], inp["v_pages"], inp["page_table"], inp["seq_lens"])
+        k_per_seq = torch.tensor(ks, dtype=torch.int32, device=cuda)
+        sel_idx = torch.full((w.batch, w.n_kv_heads, cap), -7, dtype=torch.int32, device=cuda)
+        sel_cnt = torch.full((w.batch, w.n_kv_heads), -7, dtype=torch.int32, device=cuda)
+        scores = torch.full((w.batch, w.n_kv_heads, max_seq), float("nan"), dtype=torch.float32, device=cuda)
+        ws = H.alloc_workspace(H.herald_select_workspace_bytes(shape), cuda)
+        H.herald_select_xq(shape, cache, q_x, x, k_per_seq, sel_idx, sel_cnt, scores, ws)
+        torch.cuda.synchronize()
+        oi = oracle_inputs(inp)
+        _, sc_o = O.select_xq(synth.to_u16(q_x), oi["k_pages"], oi["page_table"], oi["seq_lens"], ks, w.n_kv_heads, 128 ** -0.5)
+        differing = 0
+        for b, L in enumerate(w.seq_lens):
+            for h in range(w.n_kv_heads):
+                assert np.abs(scores[b, h, :L].cpu().numpy() - sc_o[b][h]).max() <= 1e-4, (ctas, path, b, h)
+                differing += check_selection(sel_idx[b, h].cpu().numpy(), int(sel_cnt[b, h]), sc_o[b][h], ks[b], L, f"ctas{ctas} tc{path} b{b} h{h}")
+        assert differing <= 4
+
+
 def test_select_xq_rejects_bad_arguments(H, cuda):
     w = synth.tiny(seq_lens=(40, 7), permille=100)
     inp = synth.make_inputs(w, seed=5, device=cuda)
