@@ -277,6 +277,19 @@ __device__ __forceinline__ void split_bf16(float x, float y, uint32_t& hi, uint3
     const float hx = __uint_as_float(hi << 16), hy = __uint_as_float(hi & 0xffff0000u);
     lo = pack_bf16(x - hx, y - hy);
 }
+// packed fp32 pairs (sm_100: one FMA-pipe instruction for two lanes' worth of elements)
+__device__ __forceinline__ void ffma2(float& d0, float& d1, float a0, float a1, float b, float c) {   // d = a * b + c
+    asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %4};\n\tmov.b64 rc, {%5, %5};\n\t"
+        "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}" : "=f"(d0), "=f"(d1) : "f"(a0), "f"(a1), "f"(b), "f"(c));
+}
+__device__ __forceinline__ void ffma2v(float& d0, float& d1, float a0, float a1, float b, float c0, float c1) {   // d = a * b + c
+    asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %4};\n\tmov.b64 rc, {%5, %6};\n\t"
+        "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}" : "=f"(d0), "=f"(d1) : "f"(a0), "f"(a1), "f"(b), "f"(c0), "f"(c1));
+}
+__device__ __forceinline__ void fadd2(float& d0, float& d1, float a0, float a1, float b0, float b1) {   // d = a + b
+    asm("{\n\t.reg .b64 ra, rb, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\t"
+        "add.rn.f32x2 rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}" : "=f"(d0), "=f"(d1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
+}
 __device__ __forceinline__ float fmax3(float a, float b, float c) {
     float r;
     asm("max.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
@@ -561,11 +574,14 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 uint32_t hi[16], lo[16];
 #pragma unroll
                 for (int i = 0; i < 16; ++i) {
-                    const float e0 = fast_exp2(fmaf(s[2 * i], p.scale_log2, -m_used));
-                    const float e1 = fast_exp2(fmaf(s[2 * i + 1], p.scale_log2, -m_used));
-                    sum0 += e0;
-                    sum1 += e1;
-                    split_bf16(e0, e1, hi[i], lo[i]);
+                    float x0, x1;
+                    ffma2(x0, x1, s[2 * i], s[2 * i + 1], p.scale_log2, -m_used);
+                    const float e0 = fast_exp2(x0), e1 = fast_exp2(x1);
+                    fadd2(sum0, sum1, sum0, sum1, e0, e1);
+                    hi[i] = pack_bf16(e0, e1);
+                    float r0, r1;
+                    ffma2v(r0, r1, __uint_as_float(hi[i] << 16), __uint_as_float(hi[i] & 0xffff0000u), -1.f, e0, e1);   // e - hi, exact
+                    lo[i] = pack_bf16(r0, r1);
                 }
                 l_run = l_run * alpha + (sum0 + sum1);
                 if (any) {   // rare: the running maximum of some row grew past the threshold -> rescale O in place
