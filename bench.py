@@ -225,6 +225,9 @@ def main():
     ap.add_argument("--layers", type=int, default=None, help="layers of the stack (default: the workload's; C5 has 28)")
     ap.add_argument("--start-after-step", type=int, default=None,
                     help="denoising steps before the retrieval stream starts (default: 0 or T-1, calibrated)")
+    ap.add_argument("--dense-layers", type=int, default=0,
+                    help="layers of the stack that keep their full KV and attend over the cache itself (PAPER.md:181: two in "
+                         "the paper's models); 0 = every layer sparse, the configuration BASELINE.json quotes")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--scan-ctas", type=int, default=None,
                     help="grid of the overlapped score scan (default: calibrated before the timed region)")
@@ -265,6 +268,9 @@ def main():
     k_per_seq = torch.tensor(ks, dtype=torch.int32, device=dev)
     layers = [dict(k_pages=x["k_pages"], v_pages=x["v_pages"], page_table=x["page_table"], seq_lens=x["seq_lens"],
                    q_rep=x["q_rep"], k_per_seq=k_per_seq, q_blk=x["q_blk"], k_blk=x["k_blk"], v_blk=x["v_blk"]) for x in inps]
+    n_dense = max(0, min(args.dense_layers, n_layers - 1))
+    for ly in layers[n_layers - n_dense:]:     # (which layers are dense does not matter to the step; layer 0 stays sparse for the stage timings)
+        ly["dense"] = True
     pipe = H.BlockPipeline(shape, layers, n_steps, args.start_after_step or 0, dev, scan_ctas=args.scan_ctas)
     units = w.batch * w.n_kv_heads
     G, M = w.group, w.block_size * w.group
@@ -511,7 +517,7 @@ def main():
             "attn_tflops_in_pipeline": attn_tflops_live, "denoise_alone_ms": denoise_alone_ms,
             "block_latency_ms": ms_step, "exposed_selection_ms": ms_step - denoise_alone_ms,
             "overlap_efficiency": (denoise_alone_ms + select_alone_ms + gather_alone_ms_block - ms_step) / (select_alone_ms + gather_alone_ms_block),
-            "n_layers": n_layers,
+            "n_layers": n_layers, "n_dense_layers": n_dense,
             "rep_attn_ms": rep_attn_ms, "rep_attn_gbs": tokens * w.n_kv_heads * 512 / (rep_attn_ms * 1e-3) / 1e9,
             "attn_2b_step_one_launch_ms": attn_2b_ms,
             "select_rep_fused_ms": select_rep_fused_ms, "select_rep_fused_softmax_sum_mode_ms": select_rep_fused_m1_ms, "select_plus_rep_separate_ms": select_alone_ms / n_layers + rep_attn_ms,
@@ -523,7 +529,7 @@ def main():
         "roofline": roofline, "roofline_scan": roofline_scan,
         "cpu_baseline": cpu_baseline,
         "e2e": {"value": e2e_tokens, "unit": "tokens/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-        "gpu_launches": args.steps * n_layers * (3 + n_steps),   # per block step: scan, top-k, gather, T-1 x attention (timed region only)
+        "gpu_launches": args.steps * ((n_layers - n_dense) * (3 + n_steps) + n_dense * n_steps),   # per block step: scan, top-k, gather, T-1 x attention (timed region only)
         "clocks": clock_info,
     }
     print(json.dumps(line))

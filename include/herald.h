@@ -213,10 +213,14 @@ typedef struct herald_layer {
     void* pool_k[2];           /* double-buffered sparse KV pools, each [batch][H_kv][cap][128] */
     void* pool_v[2];
     int32_t* pool_len[2];      /* int32 [batch][H_kv] per buffer                                              */
+    int32_t dense;             /* non-zero: the layer keeps its full KV and attends over the cache itself (PAPER.md:181:
+                                  "the first two layers always perform exact attention"): no selection, no gather,
+                                  q_rep / k_per_seq / pool_* unused (may be NULL)                               */
 } herald_layer_t;
 
 /* One block step of the dual-stream pipeline (Fig. 11):
  *   main stream     : for s in [0, n_steps): for each layer: herald_sparse_attn on pools[active]
+ *                     (herald_dense_attn on the cache for a layer with `dense` set; the retrieval stream skips it)
  *   retrieval stream: starts once `start_after_step` main-stream steps have been enqueued-and-finished
  *                     (0 = immediately, the north-star default; 2 = the paper's "waits only for the
  *                     first two steps"); for each layer: herald_select -> herald_gather into

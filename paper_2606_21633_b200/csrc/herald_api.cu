@@ -986,9 +986,13 @@ int herald_pipeline_step(herald_pipeline_t* p) {
         if (e != cudaSuccess) return cuda_fail(e, "record fork");
         e = cudaStreamWaitEvent(s_ret, ev_fork, 0);
         if (e != cudaSuccess) return cuda_fail(e, "wait fork");
+        int last_sparse = -1;
+        for (int l = 0; l < p->n_layers; ++l)
+            if (!p->layers[l].dense) last_sparse = l;
         for (int l = 0; l < p->n_layers; ++l) {
             herald_layer_t* ly = &p->layers[l];
-            g_prof_armed = (l == p->n_layers - 1);
+            if (ly->dense) continue;                      // keeps its full KV: nothing to select
+            g_prof_armed = (l == last_sparse);
             g_scan_ctas = p->scan_ctas;
             int r = herald_select(sh, &ly->cache, ly->q_rep, ly->k_per_seq, p->sel_idx, ly->pool_len[idle], nullptr,
                                   p->ws_select, p->ws_select_bytes, s_ret);
@@ -997,7 +1001,7 @@ int herald_pipeline_step(herald_pipeline_t* p) {
             if (r) return r;
             r = herald_gather(sh, &ly->cache, p->sel_idx, ly->pool_len[idle], ly->pool_k[idle], ly->pool_v[idle], s_ret);
             if (r) return r;
-            if (l == p->n_layers - 1 && g_prof && g_prof->gather_end)
+            if (l == last_sparse && g_prof && g_prof->gather_end)
                 cudaEventRecord(static_cast<cudaEvent_t>(g_prof->gather_end), s_ret);
         }
         e = cudaEventRecord(ev_join, s_ret);
@@ -1011,6 +1015,7 @@ int herald_pipeline_step(herald_pipeline_t* p) {
     const bool planned = herald_attn_grid_ctas(sh) > sm_count() && p->ws_attn_bytes >= ws_layer * (size_t)p->n_layers && p->n_steps > 0;
     if (planned) {
         for (int l = 0; l < p->n_layers; ++l) {
+            if (p->layers[l].dense) continue;
             rc = attn_plan(sh, p->layers[l].pool_len[act], reinterpret_cast<int32_t*>(static_cast<uint8_t*>(p->ws_attn) + ws_layer * l), s_main);
             if (rc) return rc;
         }
@@ -1025,6 +1030,15 @@ int herald_pipeline_step(herald_pipeline_t* p) {
         if (s == p->n_steps) break;
         for (int l = 0; l < p->n_layers; ++l) {
             herald_layer_t* ly = &p->layers[l];
+            if (ly->dense) {      // exact attention over the whole paged cache
+                rc = sparse_attn_impl(sh, ly->cache.k_pages, ly->cache.v_pages, nullptr,
+                                      static_cast<const __nv_bfloat16*>(ly->q_blk) + s * q_step,
+                                      static_cast<const __nv_bfloat16*>(ly->k_blk) + s * kv_step,
+                                      static_cast<const __nv_bfloat16*>(ly->v_blk) + s * kv_step,
+                                      ly->out + s * q_step, nullptr, p->ws_attn, p->ws_attn_bytes, s_main, nullptr, &ly->cache);
+                if (rc) return rc;
+                continue;
+            }
             rc = sparse_attn_impl(sh, ly->pool_k[act], ly->pool_v[act], ly->pool_len[act],
                                   static_cast<const __nv_bfloat16*>(ly->q_blk) + s * q_step,
                                   static_cast<const __nv_bfloat16*>(ly->k_blk) + s * kv_step,

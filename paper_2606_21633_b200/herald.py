@@ -53,7 +53,7 @@ class Cache(C.Structure):
 class Layer(C.Structure):
     _fields_ = [("cache", Cache), ("q_rep", C.c_void_p), ("k_per_seq", C.c_void_p),
                 ("q_blk", C.c_void_p), ("k_blk", C.c_void_p), ("v_blk", C.c_void_p), ("out", C.c_void_p),
-                ("pool_k", C.c_void_p * 2), ("pool_v", C.c_void_p * 2), ("pool_len", C.c_void_p * 2)]
+                ("pool_k", C.c_void_p * 2), ("pool_v", C.c_void_p * 2), ("pool_len", C.c_void_p * 2), ("dense", C.c_int32)]
 
 
 class Pipeline(C.Structure):
@@ -279,7 +279,7 @@ class BlockPipeline:
 
     def __init__(self, shape: Shape, layers, n_steps: int, start_after_step: int = 0, device="cuda", scan_ctas=None):
         """layers: list of dicts with torch tensors k_pages, v_pages, page_table, seq_lens, q_rep, k_per_seq,
-        q_blk, k_blk, v_blk ([n_steps, ...])."""
+        q_blk, k_blk, v_blk ([n_steps, ...]); optional "dense": True for a layer that keeps its full KV."""
         dev = torch.device(device)
         self.shape, self.n_steps, self.device = shape, n_steps, dev
         units, cap = shape.batch * shape.n_kv_heads, shape.pool_capacity
@@ -288,13 +288,15 @@ class BlockPipeline:
         self.outs, self.pools_k, self.pools_v, self.pool_lens = [], [], [], []
         for i, ly in enumerate(layers):
             out = torch.empty((n_steps, shape.batch, shape.block_size, shape.n_q_heads, 128), dtype=torch.float32, device=dev)
-            pk = [torch.zeros((shape.batch, shape.n_kv_heads, cap, 128), dtype=torch.bfloat16, device=dev) for _ in range(2)]
-            pv = [torch.zeros((shape.batch, shape.n_kv_heads, cap, 128), dtype=torch.bfloat16, device=dev) for _ in range(2)]
+            rows = 1 if ly.get("dense") else cap          # a dense layer has no pools: placeholders
+            pk = [torch.zeros((shape.batch, shape.n_kv_heads, rows, 128), dtype=torch.bfloat16, device=dev) for _ in range(2)]
+            pv = [torch.zeros((shape.batch, shape.n_kv_heads, rows, 128), dtype=torch.bfloat16, device=dev) for _ in range(2)]
             pl = [torch.zeros((shape.batch, shape.n_kv_heads), dtype=torch.int32, device=dev) for _ in range(2)]
             L = self.layer_arr[i]
             L.cache = make_cache(ly["k_pages"], ly["v_pages"], ly["page_table"], ly["seq_lens"])
             L.q_rep, L.k_per_seq = _ptr(ly["q_rep"]), _ptr(ly["k_per_seq"])
             L.q_blk, L.k_blk, L.v_blk, L.out = _ptr(ly["q_blk"]), _ptr(ly["k_blk"]), _ptr(ly["v_blk"]), _ptr(out)
+            L.dense = 1 if ly.get("dense") else 0
             for j in range(2):
                 L.pool_k[j], L.pool_v[j], L.pool_len[j] = _ptr(pk[j]), _ptr(pv[j]), _ptr(pl[j])
             self.outs.append(out)

@@ -518,6 +518,38 @@ def test_pipeline_step_matches_sequential_oracle(H, cuda, start_after):
         assert np.abs(pipe.outs[l][0].cpu().numpy() - ref).max() <= ATTN_TOL
 
 
+def test_pipeline_with_a_dense_layer(H, cuda):
+    """A layer flagged dense keeps its full KV (the first two layers): the main stream attends over its
+    paged cache, the retrieval stream skips it; the sparse layer beside it behaves as before."""
+    w = synth.Workload("mix", 2, (700, 333), 8, 2, 16, 4, 100, "planted", 8)
+    inps = [synth.make_inputs(w, seed=4242 + l, device=cuda, spare_pages=1, hostile_tails=True) for l in range(2)]
+    ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
+    cap = max(ks) + w.block_size
+    shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, (w.max_seq_len + 15) // 16 * 16, inps[0]["page_table"].shape[1], cap)
+    layers = [_layer_inputs(w, x, ks, cuda) for x in inps]
+    layers[0]["dense"] = True
+    pipe = H.BlockPipeline(shape, layers, w.n_attn_steps, 0, cuda)
+    pipe.step()
+    pipe.step()
+    torch.cuda.synchronize()
+    # layer 0: exact attention over the whole prefix, every step, both blocks
+    oi = oracle_inputs(inps[0])
+    sel_all = [[np.arange(L, dtype=np.int32) for _ in range(w.n_kv_heads)] for L in w.seq_lens]
+    pk, pv, pl = O.gather(oi["k_pages"], oi["v_pages"], oi["page_table"], sel_all, w.max_seq_len)
+    for s in range(w.n_attn_steps):
+        ref, _ = O.sparse_attn(synth.to_u16(inps[0]["q_blk"][s]), synth.to_u16(inps[0]["k_blk"][s]), synth.to_u16(inps[0]["v_blk"][s]), pk, pv, pl, 128 ** -0.5)
+        assert np.abs(pipe.outs[0][s].cpu().numpy().astype(np.float64) - ref).max() <= ATTN_TOL
+    assert int(pipe.pool_lens[0][0].abs().sum()) == 0 and int(pipe.pool_lens[0][1].abs().sum()) == 0   # untouched
+    # layer 1: the sparse path (block 1 attends over the pool selected during block 0)
+    oi = oracle_inputs(inps[1])
+    sel, _ = O.select(oi["q_rep"], oi["k_pages"], oi["page_table"], oi["seq_lens"], ks, w.n_kv_heads, 128 ** -0.5)
+    pk, pv, pl = O.gather(oi["k_pages"], oi["v_pages"], oi["page_table"], sel, cap)
+    assert np.array_equal(pipe.pool_lens[1][1].cpu().numpy(), pl)
+    for s in range(w.n_attn_steps):
+        ref, _ = O.sparse_attn(synth.to_u16(inps[1]["q_blk"][s]), synth.to_u16(inps[1]["k_blk"][s]), synth.to_u16(inps[1]["v_blk"][s]), pk, pv, pl, 128 ** -0.5)
+        assert np.abs(pipe.outs[1][s].cpu().numpy().astype(np.float64) - ref).max() <= ATTN_TOL
+
+
 def test_pipeline_host_io_roundtrip(H, cuda):
     w = synth.Workload("pipeh", 1, (1024,), 8, 2, 16, 3, 100, "plain")
     inp = synth.make_inputs(w, seed=9, device=cuda)
