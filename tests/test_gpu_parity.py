@@ -399,6 +399,36 @@ def test_sparse_attn_split_kv_is_consistent(H, cuda, splits, monkeypatch):
     assert np.abs(out.cpu().numpy() - ref).max() <= ATTN_TOL
 
 
+@pytest.mark.parametrize("splits", [1, 2])
+def test_sparse_attn_late_peaks_rescale_the_accumulator(H, cuda, splits, monkeypatch):
+    """The running row maximum is lazy (it moves only when a tile exceeds it by 2^40): keys planted deep in the pool that
+    match one query row each make the logit of that row jump by hundreds of log2 units in a late tile, so the in-place
+    rescale of the accumulator in TMEM runs -- in some rows of a tile and not in others, more than once per row."""
+    monkeypatch.setenv("HERALD_ATTN_SPLITS", str(splits))
+    batch, B, Hq, Hkv, cap = 1, 32, 14, 2, 900
+    q, kb, vb, pk, pv, pl = _attn_case(cuda, batch, B, Hq, Hkv, cap, [[900, 520]], seed=311)
+    G = Hq // Hkv
+    for n, (i, hq, pos, gain) in enumerate([(0, 0, 300, 6.0), (0, 0, 700, 12.0), (5, 3, 450, 9.0), (17, 9, 333, 8.0), (31, 13, 519, 10.0),
+                                              (31, 13, 140, 5.0), (8, 7, 899, 7.0)]):
+        h = hq // G
+        if pos < int(pl[0, h]):
+            pk[0, h, pos] = (gain * q[0, i, hq].to(torch.float32)).to(torch.bfloat16)
+    shape = H.make_shape(batch, Hq, Hkv, B, 16, 1, cap)
+    out = torch.full((batch, B, Hq, 128), float("nan"), dtype=torch.float32, device=cuda)
+    lse = torch.full((batch, B, Hq), float("nan"), dtype=torch.float32, device=cuda)
+    ws = H.alloc_workspace(H.herald_attn_workspace_bytes(shape), cuda)
+    H.herald_sparse_attn(shape, pk, pv, pl, q, kb, vb, out, lse, ws)
+    torch.cuda.synchronize()
+    pv_clean = pv.clone()
+    pv_clean[torch.isnan(pv_clean)] = 0
+    ref, lse_ref = O.sparse_attn(synth.to_u16(q), synth.to_u16(kb), synth.to_u16(vb), synth.to_u16(pk), synth.to_u16(pv_clean),
+                                 pl.cpu().numpy(), 128 ** -0.5)
+    assert lse_ref.max() > 60.0                       # the planted logits are far above everything else
+    err = np.abs(out.cpu().numpy().astype(np.float64) - ref).max()
+    assert np.isfinite(err) and err <= ATTN_TOL, err
+    assert np.abs(lse.cpu().numpy() - lse_ref).max() <= 2e-3 * max(1.0, np.abs(lse_ref).max() / 10)
+
+
 @pytest.mark.parametrize("n_groups", [1, 2, 3])
 def test_sparse_attn_groups_share_the_pools(H, cuda, n_groups):
     """herald_sparse_attn_groups: the denoising group and the draft group of the 2B-token step attend over the
