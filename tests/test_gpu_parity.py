@@ -40,6 +40,9 @@ SELECT_CASES = {
     "g7_ragged": dict(w=synth.Workload("g7", 3, (5000, 3333, 16), 28, 4, 32, 4, 50, "planted", 20), spare=2, hostile=True),
     "g8_h8": dict(w=synth.Workload("g8", 2, (2049, 4096), 64, 8, 16, 3, 25, "zipf"), spare=0, hostile=False),
     "g1": dict(w=synth.Workload("g1", 2, (1000, 999), 2, 2, 16, 3, 100, "plain"), spare=0, hostile=True),
+    # KV head counts that do not divide a 32-warp CTA: the head-major scan (scan_kernel<0>) instead of the page-major one
+    "h3_g5": dict(w=synth.Workload("h3", 3, (2500, 17, 900), 15, 3, 16, 3, 50, "planted", 6), spare=2, hostile=True),
+    "h6_g2": dict(w=synth.Workload("h6", 2, (1200, 4097), 12, 6, 16, 3, 30, "zipf"), spare=0, hostile=True),
 }
 
 
@@ -74,7 +77,8 @@ def test_select_matches_oracle(H, cuda, case, agg_mode):
                     assert len(planted - set(sel_g[b, h, :ks[b]].tolist())) <= max(1, len(planted) // 8)
 
 
-XQ_CASES = [("tiny_ragged", 1), ("tiny_ragged", 3), ("one_token", 2), ("g7_ragged", 4), ("g7_ragged", 32), ("g8_h8", 32), ("g1", 5)]
+XQ_CASES = [("tiny_ragged", 1), ("tiny_ragged", 3), ("one_token", 2), ("g7_ragged", 4), ("g7_ragged", 32), ("g8_h8", 32), ("g1", 5),
+            ("h3_g5", 7), ("h6_g2", 20)]
 
 
 @pytest.mark.parametrize("path", ["auto", "mma_sync", "tcgen05"])
