@@ -274,6 +274,60 @@ def test_full_size_fused_retrieval_and_xq_sampled(H, cuda, name, seqs):
     assert differing <= max(1, len(seqs) * w.n_kv_heads // 2)
 
 
+def test_strided_cache_views(H, cuda):
+    """The cache is described by explicit strides (include/herald.h): pages that are a VIEW into a larger allocation (two
+    extra head slots per token, a one-head offset) must give the same selection, pools, dense attention and fused
+    retrieval outputs as the packed copy -- scan loads, gather copies and the TMA page boxes all go through the strides."""
+    w = synth.Workload("strided", 2, (1500, 333), 8, 2, 16, 3, 100, "planted", 6)
+    inp = synth.make_inputs(w, seed=777, device=cuda, spare_pages=2, hostile_tails=True)
+    n_pages, P, Hkv, d = inp["k_pages"].shape
+    big_k = torch.full((n_pages, P, Hkv + 2, d), 7.0, dtype=torch.bfloat16, device=cuda)
+    big_v = torch.full((n_pages, P, Hkv + 2, d), float("nan"), dtype=torch.bfloat16, device=cuda)
+    big_k[:, :, 1:Hkv + 1] = inp["k_pages"]
+    big_v[:, :, 1:Hkv + 1] = inp["v_pages"]
+    views = dict(inp, k_pages=big_k[:, :, 1:Hkv + 1], v_pages=big_v[:, :, 1:Hkv + 1])
+    assert not views["k_pages"].is_contiguous()
+    ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
+    cap = max(ks) + w.block_size
+    max_seq = (w.max_seq_len + 15) // 16 * 16
+    shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, max_seq, inp["page_table"].shape[1], cap, 0)
+    k_per_seq = torch.tensor(ks, dtype=torch.int32, device=cuda)
+    results = []
+    for x in (inp, views):
+        cache = H.make_cache(x["k_pages"], x["v_pages"], x["page_table"], x["seq_lens"])
+        sel_idx = torch.full((w.batch, w.n_kv_heads, cap), -7, dtype=torch.int32, device=cuda)
+        sel_cnt = torch.full((w.batch, w.n_kv_heads), -7, dtype=torch.int32, device=cuda)
+        scores = torch.zeros((w.batch, w.n_kv_heads, max_seq), dtype=torch.float32, device=cuda)
+        rep = torch.zeros((w.batch, w.n_q_heads, 128), dtype=torch.float32, device=cuda)
+        ws = H.alloc_workspace(H.herald_select_rep_workspace_bytes(shape), cuda)
+        H.herald_select_rep(shape, cache, x["q_rep"], k_per_seq, sel_idx, sel_cnt, scores, rep, None, ws)
+        sel2, cnt2 = torch.full_like(sel_idx, -7), torch.full_like(sel_cnt, -7)
+        sc2 = torch.zeros_like(scores)
+        H.herald_select(shape, cache, x["q_rep"], k_per_seq, sel2, cnt2, sc2, ws)
+        pk = torch.zeros((w.batch, w.n_kv_heads, cap, 128), dtype=torch.bfloat16, device=cuda)
+        pv = torch.zeros_like(pk)
+        H.herald_gather(shape, cache, sel2, cnt2, pk, pv)
+        dense = torch.zeros((w.batch, w.block_size, w.n_q_heads, 128), dtype=torch.float32, device=cuda)
+        wa = H.alloc_workspace(H.herald_attn_workspace_bytes(shape), cuda)
+        H.herald_dense_attn(shape, cache, x["q_blk"][0], x["k_blk"][0], x["v_blk"][0], dense, None, wa)
+        q_x = synth.make_q_x(x["q_rep"], 16, seed=3)
+        sel3, cnt3 = torch.full_like(sel_idx, -7), torch.full_like(sel_cnt, -7)
+        H.herald_select_xq(shape, cache, q_x, 16, k_per_seq, sel3, cnt3, None, ws)          # 64 score rows: the tcgen05 scan
+        torch.cuda.synchronize()
+        results.append((sel_idx, sel_cnt, scores, rep, sel2, cnt2, sc2, pk, pv, dense, sel3, cnt3))
+    for a_, b_ in zip(*results):
+        assert torch.equal(a_, b_)
+    # and the packed run is right (one oracle check ties the pair to the paper)
+    oi = oracle_inputs(inp)
+    sel_o, _ = O.select(oi["q_rep"], oi["k_pages"], oi["page_table"], oi["seq_lens"], ks, w.n_kv_heads, 128 ** -0.5)
+    pk_o, _, pl_o = O.gather(oi["k_pages"], oi["v_pages"], oi["page_table"], sel_o, cap)
+    assert np.array_equal(results[0][5].cpu().numpy(), pl_o)
+    for b in range(w.batch):
+        for h in range(w.n_kv_heads):
+            n = int(pl_o[b, h])
+            assert np.array_equal(synth.to_u16(results[1][7][b, h, :n]), pk_o[b, h, :n])
+
+
 def test_select_edge_cases(H, cuda):
     # empty sequence, k = 0, k >= L (identity), k > pool capacity (clamped)
     w = synth.Workload("edge", 4, (0, 40, 33, 64), 4, 2, 16, 3, 100, "plain")
