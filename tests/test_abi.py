@@ -90,3 +90,33 @@ def test_workspace_too_small_is_reported(H):
     with pytest.raises(H.HeraldError) as ei:       # the size check fails before any device access
         H.herald_select(shape, cache, 256, 256, 256, 256, None, (4096, 256), stream=0)
     assert ei.value.code == H.ERR_WORKSPACE_TOO_SMALL
+
+
+def test_follow_up_entries_check_their_arguments_before_any_cuda_call(H):
+    """herald_select_xq / herald_select_rep / herald_rep_attn / herald_sparse_attn_groups: NULL pointers, a query count out of
+    range, a workspace that is too small and a bad group count are reported without touching the device."""
+    shape = H.make_shape(2, 8, 4, 16, 1024, 64, 64)
+    cache = H.Cache(256, 256, 16 * 4 * 128, 4 * 128, 128, 256, 256)
+    big = (256, 1 << 30)
+    cases = [
+        (lambda: H.herald_select_xq(shape, cache, None, 2, 256, 256, 256, None, big, stream=0), H.ERR_INVALID_ARG),
+        (lambda: H.herald_select_xq(shape, cache, 256, 0, 256, 256, 256, None, big, stream=0), H.ERR_INVALID_ARG),
+        (lambda: H.herald_select_xq(shape, cache, 256, 129, 256, 256, 256, None, big, stream=0), H.ERR_INVALID_ARG),     # 129 x G=2 > 256 rows
+        (lambda: H.herald_select_xq(shape, cache, 256, 2, 256, 256, 256, None, (256, 256), stream=0), H.ERR_WORKSPACE_TOO_SMALL),
+        (lambda: H.herald_select_rep(shape, cache, 256, 256, 256, 256, None, None, None, big, stream=0), H.ERR_INVALID_ARG),   # rep_out NULL
+        (lambda: H.herald_select_rep(shape, cache, 256, 256, 256, 256, None, 256, None, (256, 256), stream=0), H.ERR_WORKSPACE_TOO_SMALL),
+        (lambda: H.herald_rep_attn(shape, cache, 256, None, None, big, stream=0), H.ERR_INVALID_ARG),
+        (lambda: H.herald_rep_attn(shape, cache, 256, 256, None, (256, 256), stream=0), H.ERR_WORKSPACE_TOO_SMALL),
+        (lambda: H.herald_sparse_attn_groups(shape, 0, 256, 256, 256, 256, 256, 256, 256, None, big, stream=0), H.ERR_INVALID_ARG),
+        (lambda: H.herald_sparse_attn_groups(shape, 2, 256, 256, None, 256, 256, 256, 256, None, big, stream=0), H.ERR_INVALID_ARG),
+    ]
+    for i, (call, code) in enumerate(cases):
+        with pytest.raises(H.HeraldError) as ei:
+            call()
+        assert ei.value.code == code, (i, ei.value.code, str(ei.value))
+    # the fused entry needs both workspaces and a log-sum-exp plane
+    assert H.herald_select_rep_workspace_bytes(shape) > H.herald_select_workspace_bytes(shape) + H.herald_rep_attn_workspace_bytes(shape) - 256
+    shape1 = H.make_shape(2, 8, 4, 16, 1024, 64, 64, 1)
+    with pytest.raises(H.HeraldError) as ei:          # x queries: the aggregation is only defined for max-logit (reading 25)
+        H.herald_select_xq(shape1, cache, 256, 2, 256, 256, 256, None, big, stream=0)
+    assert ei.value.code == H.ERR_INVALID_ARG
