@@ -424,8 +424,19 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 }
                 __syncwarp();
             }
+            // dense mode: the page ids of a tile are fetched one tile ahead, so that their round trip does not sit between a
+            // ring slot falling free and its TMA requests
+            auto tile_phys = [&](int jj) -> int {
+                const int tt = t0 + jj;
+                if (!paged || jj >= nt || tt == 0) return 0;
+                const int n_pg = (tile_valid(jj) + kPageSize - 1) / kPageSize;
+                return lane < n_pg ? __ldg(p.page_table + (int64_t)b_pool * p.max_pages + (tt - 1) * (kTcBN / kPageSize) + lane) : 0;
+            };
+            int phys_next = tile_phys(0);
             for (int j = 0; j < nt; ++j) {
                 const int stage = j % kTcStages, t = t0 + j;
+                const int my_phys = phys_next;
+                phys_next = tile_phys(j + 1);
                 if (j >= kTcStages) mbar_wait(bar(bar_empty + stage), ((j / kTcStages) - 1) & 1);
                 if (!is_k && j == 0) named_bar_sync(9, 64);   // Q and K_0 are requested before any V tile
                 const uint32_t dst = ring + stage * kTcTileBytes, full = bar(bar_full + stage);
@@ -447,8 +458,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 if (paged && t > 0) {
                     // dense mode: the 128 tokens of the tile are 8 pages of the cache; page i lands on tile rows [16i, 16i+16)
                     // (2 KB per half: a whole number of 1 KB swizzle atoms).  Pages past the sequence are not requested.
-                    const int page0 = (t - 1) * (kTcBN / kPageSize), n_pg = (valid + kPageSize - 1) / kPageSize;
-                    const int my_phys = lane < n_pg ? __ldg(p.page_table + (int64_t)b_pool * p.max_pages + page0 + lane) : 0;
+                    const int n_pg = (valid + kPageSize - 1) / kPageSize;
                     if (lane == 0) mbar_arrive_expect_tx(land, (uint32_t)n_pg * kPageSize * 256u);
                     __syncwarp();
                     if (lane < n_pg) {
