@@ -32,10 +32,12 @@
 //             is only raised when it grows by more than 2^kTcRescaleThreshold ("lazy rescale"; P, l and O are
 //             fp32/bf16-ranged, so the threshold only guards overflow): O in TMEM is then rescaled in place.
 //   merge     split-KV partials never leave the chip: tile row r is owned by CTA r / rows_own of the cluster; the
-//             other CTAs stage their unnormalised O rows and (max, sum) and send them to the owner's shared memory
-//             with one bulk DSMEM copy each (cp.async.bulk shared::cta -> shared::cluster, mbarrier-tracked); the
+//             other CTAs write their unnormalised O rows and (max, sum) straight from registers into the owner's
+//             shared memory (st.shared::cluster into the owner's K ring, which its last QK^T has released: every CTA
+//             tells its peers so with a remote mbarrier arrive as soon as that MMA has completed, about a tile
+//             period before the partials exist), then arrive on the owner's merge barrier (release.cluster).  The
 //             owner merges with its own registers, normalises, stages the rows in shared memory and writes `out`
-//             with fully coalesced 512-byte rows.
+//             with fully coalesced 512-byte rows.  No cluster-wide barrier after the main loop, no staging copy.
 #pragma once
 #include <cuda.h>
 
@@ -67,26 +69,17 @@ constexpr float kTcRescaleThreshold = 40.f;      // log2 units
 constexpr int kTcRowFloats = kHeadDim + 4;       // 528-byte rows: 16-byte accesses of 8 consecutive rows hit 8 bank groups
 constexpr int kTcRecvO = kTcSmemK;                                               // float [S-1 sources][rows_own][132]
 constexpr int kTcRecvML = kTcRecvO + kTcBM * kTcRowFloats * 4;                   // float2 [S-1 sources][ml_stride]
-constexpr int kTcPushO = kTcSmemV;                                               // float [S-1 owners][rows_own][132], then
-                                                                                 // float2 [S-1][ml_stride], then the output rows
+constexpr int kTcStageO = kTcSmemV;                                              // float [rows_own][132]: the finished rows
 static_assert(kTcRecvML + (kTcBM + 2 * kTcMaxSplits) * 8 <= kTcSmemV, "receive buffers must fit in the K ring");
-constexpr int tc_merge_stage_bytes(int S) {      // bytes of the V ring used by the merge for a cluster of S CTAs
-    const int rows_own = (kTcBM + S - 1) / S, ml_stride = (rows_own + 1) & ~1;
-    return (S - 1) * (rows_own * kTcRowFloats * 4 + ml_stride * 8) + rows_own * kTcRowFloats * 4;
-}
-constexpr bool tc_merge_fits() {
-    for (int S = 1; S <= kTcMaxSplits; ++S)
-        if (tc_merge_stage_bytes(S) > kTcStages * kTcTileBytes) return false;
-    return true;
-}
-static_assert(tc_merge_fits(), "push + output staging must fit in the V ring");
+static_assert(kTcBM * kTcRowFloats * 4 <= kTcStages * kTcTileBytes, "output staging must fit in the V ring");
 
 // barrier slots (8 bytes each) inside the misc area
 enum { kBarKFull = 0, kBarKEmpty = kBarKFull + kTcStages, kBarVFull = kBarKEmpty + kTcStages, kBarVEmpty = kBarVFull + kTcStages,
        kBarSFull = kBarVEmpty + kTcStages, kBarPFull = kBarSFull + kTcSBufs, kBarPvDone = kBarPFull + kTcSBufs,
-       kBarQFull = kBarPvDone + kTcSBufs, kBarVTail, kBarMerge, kBarAck, kBarCount };
-constexpr int kTcMiscTmemPtr = 200;              // uint32
+       kBarQFull = kBarPvDone + kTcSBufs, kBarVTail, kBarMerge, kBarPeerReady, kBarQkDone, kBarCount };
+constexpr int kTcMiscTmemPtr = 240;              // uint32
 constexpr int kTcMiscMax = 256;                  // bf16 [2 buffers][4 column quarters][128 rows]; float [4][128] for the row sums
+static_assert(kBarCount <= 32, "one barrier per lane of the initialising warp");
 static_assert(kBarCount * 8 <= kTcMiscTmemPtr, "barriers overlap the TMEM pointer slot");
 static_assert(kTcMiscMax + 2 * 4 * 128 * 2 <= kTcMiscBytes, "exchange buffer overflows the misc area");
 
@@ -113,7 +106,9 @@ struct AttnParams {
 
 #ifdef HERALD_ATTN_TRACE
 #define HERALD_STAMP(slot) do { if (p.trace && (slot) < 64) p.trace[(((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * 64 + (slot)] = clock64(); } while (0)
+#define HERALD_GSTAMP(slot) do { if (p.trace) { unsigned long long gt_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_)); p.trace[(((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * 64 + (slot)] = gt_; } } while (0)
 #else
+#define HERALD_GSTAMP(slot) do { } while (0)
 #define HERALD_STAMP(slot) do { } while (0)
 #endif
 
@@ -157,25 +152,40 @@ __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::
 __device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t threads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
-__device__ __forceinline__ void cluster_sync_all() {   // every thread of every CTA of the cluster
-    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+// the same wait with acquire semantics at cluster scope: the barrier is arrived on by other CTAs of the cluster
+// (mbarrier.arrive.release.cluster) after they have written this CTA's shared memory
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
+    for (uint32_t spins = 0;; ++spins) {
+        uint32_t done;
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        if (done) return;
+        if (spins > (1u << 26)) __trap();
+    }
 }
+// cluster barrier in two halves (every thread of every CTA of the cluster executes both): the arrive publishes the
+// barrier initialisation, the wait comes right before the first remote operation so that its latency is hidden
+__device__ __forceinline__ void cluster_arrive_all() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait_all() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 __device__ __forceinline__ uint32_t map_to_cta(uint32_t smem_addr, uint32_t cta_rank) {
     uint32_t r;
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_addr), "r"(cta_rank));
     return r;
 }
-__device__ __forceinline__ void st_cluster_f4(uint32_t addr, float a, float b, float c, float d) {
-    asm volatile("st.shared::cluster.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+// asynchronous stores into the shared memory of another CTA of the cluster; each one counts its bytes on the destination's
+// mbarrier (complete_tx), so the sender needs neither a fence nor an arrive and the receiver sees the data once its wait
+// on that barrier returns
+__device__ __forceinline__ void st_async_f4(uint32_t addr, float a, float b, float c, float d, uint32_t bar_cluster) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1, %2, %3, %4}, [%5];"
+                 ::"r"(addr), "f"(a), "f"(b), "f"(c), "f"(d), "r"(bar_cluster) : "memory");
 }
-__device__ __forceinline__ void st_cluster_f2(uint32_t addr, float a, float b) {
-    asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(a), "f"(b) : "memory");
-}
-
-// local shared memory -> shared memory of another CTA of the cluster; completion counts bytes on the destination's mbarrier
-__device__ __forceinline__ void dsmem_bulk_copy(uint32_t dst_cluster, uint32_t src_cta, uint32_t bytes, uint32_t bar_cluster) {
-    asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst_cluster), "r"(src_cta), "r"(bytes), "r"(bar_cluster) : "memory");
+__device__ __forceinline__ void st_async_f2(uint32_t addr, float a, float b, uint32_t bar_cluster) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];"
+                 ::"r"(addr), "f"(a), "f"(b), "r"(bar_cluster) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive_remote(uint32_t bar_cluster) {
     asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster) : "memory");
@@ -321,9 +331,11 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     const int rows_box = p.ipt * G;                          // tile rows the Q box writes (zeros past the block)
     const int rows_own = (rows_box + S - 1) / S;             // tile rows merged and written by each CTA of the cluster (zero rows past the box are nobody's)
     const int ml_stride = (rows_own + 1) & ~1;               // float2 per source, padded to 16 bytes
+    const int n_own = max(0, min(rows_own, rows_box - split * rows_own));   // rows of the box this CTA merges
+    const int merge_bytes = (S - 1) * n_own * (kHeadDim * 4 + 8);   // partial rows and (m, l) the other CTAs send to this one
     const int g_inv = (65536 + G - 1) / G;                   // (r * g_inv) >> 16 == r / G for r < 128, G <= 8
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    if (tid == 0) HERALD_STAMP(0);
+    if (tid == 0) { HERALD_STAMP(0); HERALD_GSTAMP(60); }
 
     const uint32_t misc = sbase + kTcSmemMisc;
     auto bar = [&](int i) { return misc + 8u * i; };
@@ -336,30 +348,20 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(misc + kTcMiscTmemPtr), "n"(kTcTmemCols));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     } else if (warp == kTcKWarp) {
-        if (lane == 0) {
-            for (int s = 0; s < kTcStages; ++s) {
-                mbar_init(bar(kBarKFull + s), 1);
-                mbar_init(bar(kBarKEmpty + s), 1);
-                mbar_init(bar(kBarVFull + s), 1);
-                mbar_init(bar(kBarVEmpty + s), 1);
-            }
-            for (int s = 0; s < kTcSBufs; ++s) {
-                mbar_init(bar(kBarSFull + s), 1);
-                mbar_init(bar(kBarPFull + s), kTcSoftmaxWarps);
-                mbar_init(bar(kBarPvDone + s), 1);   // PV_j commits to slot j % 3
-            }
-            mbar_init(bar(kBarQFull), 1);
-            mbar_init(bar(kBarVTail), 1);
-            mbar_init(bar(kBarMerge), 1);
-            mbar_init(bar(kBarAck), S > 1 ? S - 1 : 1);
+        // one barrier per lane: every count is 1 except P-full (one arrive per softmax warp) and peer-ready (one per peer)
+        if (lane < kBarCount) {
+            const bool is_p = lane >= kBarPFull && lane < kBarPFull + kTcSBufs;
+            mbar_init(bar(lane), is_p ? kTcSoftmaxWarps : (lane == kBarPeerReady && S > 1 ? S - 1 : 1));
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-            // the partial rows the other CTAs of the cluster will send (nothing can arrive before the first cluster barrier)
-            mbar_arrive_expect_tx(bar(kBarMerge), (uint32_t)((S - 1) * (rows_own * kTcRowFloats * 4 + ml_stride * 8)));
-            asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_q) : "memory");
-            asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_k) : "memory");
-            asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_v) : "memory");
-            asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_kb) : "memory");
-            asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_vb) : "memory");
+        }
+        __syncwarp();
+        if (lane == 0) {
+            // the partial rows the other CTAs of the cluster will send (st.async, counted in bytes)
+            if (merge_bytes > 0) mbar_arrive_expect_tx(bar(kBarMerge), (uint32_t)merge_bytes);
+        }
+        if (lane < 5) {
+            const CUtensorMap* tm = lane == 0 ? &tm_q : lane == 1 ? &tm_k : lane == 2 ? &tm_v : lane == 3 ? &tm_kb : &tm_vb;
+            asm volatile("prefetch.tensormap [%0];" ::"l"(tm) : "memory");
         }
     } else if (warp < kTcSoftmaxWarps) {
         // Q rows the TMA box does not write are zeros (all 16 chunks of a row, so the swizzle does not matter)
@@ -373,12 +375,16 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_ptr_gen;
+    if (S > 1) cluster_arrive_all();   // the barriers of this CTA are initialised: remote arrives may come from here on
     if (tid == 0) HERALD_STAMP(1);
 
     // Programmatic dependent launch: this grid may have been scheduled while the previous kernel of the stream was
     // still draining.  Everything above is on-chip; nothing is read from global memory before that kernel has
-    // completed and flushed.
+    // completed and flushed.  (Requesting pool tiles or reading the pool lengths ahead of the wait was measured: the early
+    // requests queue in front of the Q tile and compete with the draining grid, 16.4 -> 16.7 us per C2 step.)
     asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (tid == 0) HERALD_GSTAMP(61);
+    if (S > 1) cluster_wait_all();     // ... and so are those of every other CTA of the cluster
     // blocks are dispatched in blockIdx order: with a plan (attn_plan_kernel) slot z holds the unit with the z-th longest
     // pool, so that the long units start first and the short ones fill the tail of a multi-wave grid
     const int unit = p.unit_order ? p.unit_order[blockIdx.z] : (int)blockIdx.z;
@@ -386,14 +392,15 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     const int b_pool = b % p.pool_batch, unit_pool = b_pool * p.n_kv_heads + h;   // whose keys: the group's prefix owner
     const bool paged = p.page_table != nullptr;
     const int n_pool = paged ? max(0, min(p.seq_lens[b_pool], p.max_seq_len)) : max(0, min(p.pool_len[unit_pool], p.cap));
-    const int n_tiles = 1 + (n_pool + kTcBN - 1) / kTcBN;    // key tile 0 = the in-block rows, tile t >= 1 = pool rows [128(t-1), 128t)
+    const int n_pool_tiles = (n_pool + kTcBN - 1) / kTcBN;
+    const int n_tiles = n_pool_tiles + 1;                    // key tile t < n_pool_tiles = pool rows [128t, 128t+128); the last tile = the in-block rows
     const int per = (n_tiles + S - 1) / S;
     const int t0 = split * per, t1 = min(n_tiles, t0 + per);
     const int nt = max(t1 - t0, 0);                          // tile j of this CTA is key tile t0 + j
 
     auto tile_valid = [&](int j) {  // valid keys of this CTA's j-th tile (>= 1)
         const int t = t0 + j;
-        return t == 0 ? B : min(kTcBN, n_pool - (t - 1) * kTcBN);
+        return t == n_pool_tiles ? B : min(kTcBN, n_pool - t * kTcBN);
     };
     auto tile_cols = [&](int j) {   // key columns of the tile that the MMAs touch (multiple of 16)
         return (tile_valid(j) + 15) & ~15;
@@ -428,9 +435,9 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
             // ring slot falling free and its TMA requests
             auto tile_phys = [&](int jj) -> int {
                 const int tt = t0 + jj;
-                if (!paged || jj >= nt || tt == 0) return 0;
+                if (!paged || jj >= nt || tt == n_pool_tiles) return 0;
                 const int n_pg = (tile_valid(jj) + kPageSize - 1) / kPageSize;
-                return lane < n_pg ? __ldg(p.page_table + (int64_t)b_pool * p.max_pages + (tt - 1) * (kTcBN / kPageSize) + lane) : 0;
+                return lane < n_pg ? __ldg(p.page_table + (int64_t)b_pool * p.max_pages + tt * (kTcBN / kPageSize) + lane) : 0;
             };
             int phys_next = tile_phys(0);
             for (int j = 0; j < nt; ++j) {
@@ -444,18 +451,18 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 const bool fix = !is_k && cols != valid;      // V rows [valid, cols) must be zeros: land on kBarVTail first
                 const uint32_t land = fix ? bar(kBarVTail) : full;
                 if (elect_one()) {
-                    if (t == 0) {   // in-block rows: box = (64 channels, 1 head, B rows, 1 sequence) per half
+                    if (t == n_pool_tiles) {   // in-block rows: box = (64 channels, 1 head, B rows, 1 sequence) per half
                         mbar_arrive_expect_tx(land, (uint32_t)B * 256u);
                         tma_load_4d(dst, map_blk, 0, h, 0, b, land);
                         tma_load_4d(dst + kTcHalfBytes, map_blk, 64, h, 0, b, land);
                     } else if (!paged) {   // pool rows: box = (64 channels, pool_box rows, 1 unit) per half; rows past cap are zero-filled
                         mbar_arrive_expect_tx(land, (uint32_t)p.pool_box * 256u);
-                        tma_load_3d(dst, map, 0, (t - 1) * kTcBN, unit_pool, land);
-                        tma_load_3d(dst + kTcHalfBytes, map, 64, (t - 1) * kTcBN, unit_pool, land);
+                        tma_load_3d(dst, map, 0, t * kTcBN, unit_pool, land);
+                        tma_load_3d(dst + kTcHalfBytes, map, 64, t * kTcBN, unit_pool, land);
                     }
                 }
                 __syncwarp();
-                if (paged && t > 0) {
+                if (paged && t != n_pool_tiles) {
                     // dense mode: the 128 tokens of the tile are 8 pages of the cache; page i lands on tile rows [16i, 16i+16)
                     // (2 KB per half: a whole number of 1 KB swizzle atoms).  Pages past the sequence are not requested.
                     const int n_pg = (valid + kPageSize - 1) / kPageSize;
@@ -489,7 +496,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 const int stage = j % kTcStages, sb = j % kTcSBufs;
                 mbar_wait(bar(kBarKFull + stage), (j / kTcStages) & 1);
                 tc_fence_after();
-                if (lane == 0) HERALD_STAMP(8 + 4 * j);
+                if (lane == 0) { HERALD_STAMP(8 + 4 * j); if (j == 0) HERALD_GSTAMP(58); }
                 if (elect_one()) {
                     const uint32_t k_lo = umma_desc_lo(sbase + kTcSmemK + stage * kTcTileBytes, 16);
                     const uint32_t idesc_s = umma_idesc(1, 1, 0, 0, kTcBM, tile_cols(j));
@@ -502,6 +509,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                     }
                     umma_commit(bar(kBarSFull + sb));
                     umma_commit(bar(kBarKEmpty + stage));
+                    if (j == nt - 1) umma_commit(bar(kBarQkDone));   // the K ring is dead from here on (merge receive buffer)
                 }
                 __syncwarp();
             };
@@ -533,11 +541,11 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 __syncwarp();
             };
             mbar_wait(bar(kBarQFull), 0);
-            issue_qk(0);
-            if (nt > 1) issue_qk(1);
-            for (int j = 0; j < nt; ++j) {
+            if (lane == 0) HERALD_GSTAMP(57);
+#pragma unroll 1
+            for (int j = -2; j < nt; ++j) {   // QK^T runs two tiles ahead of PV
                 if (j + 2 < nt) issue_qk(j + 2);
-                issue_pv(j);
+                if (j >= 0) issue_pv(j);
             }
         } else {
             // =========================== softmax warps ===========================
@@ -545,7 +553,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 const int sb = j % kTcSBufs, eb = j & 1;
                 mbar_wait(bar(kBarSFull + sb), (j / kTcSBufs) & 1);
                 tc_fence_after();
-                if (tid == 0) HERALD_STAMP(8 + 4 * j + 1);
+                if (tid == 0) { HERALD_STAMP(8 + 4 * j + 1); if (j == 0) HERALD_GSTAMP(62); }
                 float s[32];
                 tmem_ld32_async(lane_base + sb * 128 + cq * 32, s);
                 tmem_wait_ld();
@@ -623,14 +631,16 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     }
 
     // ---- merge of the split-KV partials inside the cluster, normalisation, output -----------------------
-    // The V ring of this CTA is dead once its softmax warps have seen the last PV complete (every MMA and every TMA
-    // write of the CTA is then done): it stages what this CTA sends and the rows it writes out.  The K ring receives
-    // the other CTAs' partial rows, so nothing is sent before the cluster barrier that every CTA passes after its main loop.
+    // The K ring of a CTA is dead once its last QK^T has completed: it receives the other CTAs' partial rows.  The
+    // K producer (idle by then) waits for that MMA and tells every peer with a remote arrive on its kBarPeerReady;
+    // this happens about a tile period before any partial exists, so no sender ever waits for it in practice.
+    if (warp == kTcKWarp && S > 1) {
+        if (nt > 0) mbar_wait(bar(kBarQkDone), 0);
+        if (lane < S - 1) mbar_arrive_remote(map_to_cta(bar(kBarPeerReady), lane < split ? lane : lane + 1));
+    }
     // the next kernel of the stream may be scheduled from here on: its blocks take the SMs as this grid's blocks exit
     asm volatile("griddepcontrol.launch_dependents;");
     const int owner = row / rows_own, row_l = row - owner * rows_own;
-    const int push_ml_off = kTcPushO + (S - 1) * rows_own * kTcRowFloats * 4;
-    const int stage_off = push_ml_off + (S - 1) * ml_stride * 8;
     float o[32];
     float l_tot = 0.f;
     if (warp < kTcSoftmaxWarps) {
@@ -644,50 +654,34 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
 #pragma unroll
             for (int i = 0; i < 32; ++i) o[i] = 0.f;
         }
+        if (tid == 0) HERALD_STAMP(6);
         if (owner != split && row < rows_box) {
-            // stage this quarter row (unnormalised) and (m, l) for its owner; slots skip the sender / the owner itself
-            const int d = owner < split ? owner : owner - 1;
-            float4* dst = reinterpret_cast<float4*>(sgen + kTcPushO + ((d * rows_own + row_l) * kTcRowFloats + cq * 32) * 4);
+            // this quarter row (unnormalised) and (m, l) go straight into the owner's receive buffer; slots skip the owner itself
+            mbar_wait_cluster(bar(kBarPeerReady), 0);
+            const int src_slot = split < owner ? split : split - 1;
+            const uint32_t bar_owner = map_to_cta(bar(kBarMerge), owner);
+            const uint32_t dst = map_to_cta(sbase + kTcRecvO + ((src_slot * rows_own + row_l) * kTcRowFloats + cq * 32) * 4, owner);
 #pragma unroll
-            for (int i = 0; i < 8; ++i) dst[i] = make_float4(o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
-            if (cq == 0)
-                *reinterpret_cast<float2*>(sgen + push_ml_off + (d * ml_stride + row_l) * 8) = make_float2(nt > 0 ? m_used : -INFINITY, l_tot);
+            for (int i = 0; i < 8; ++i) st_async_f4(dst + 16 * i, o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3], bar_owner);
+            if (cq == 0)   // an empty split sends (-inf, 0) and zero rows
+                st_async_f2(map_to_cta(sbase + kTcRecvML + (src_slot * ml_stride + row_l) * 8, owner), nt > 0 ? m_used : -INFINITY, l_tot, bar_owner);
         }
-        fence_proxy_async_smem();
     }
-    tc_fence_before();
-    __syncwarp();
-    if (S > 1) cluster_sync_all(); else __syncthreads();   // staging complete here, main loops complete everywhere
     if (tid == 0) HERALD_STAMP(5);
-    if (tid < (S - 1) * 8) {
-        // bulk copies to each owner: this CTA's rows of that owner's slice in 8 chunks (8 threads), then their (m, l)
-        const int d = tid >> 3, chunk = tid & 7, dst_cta = d < split ? d : d + 1;
-        const int src_slot = split < dst_cta ? split : split - 1;
-        const uint32_t bar_remote = map_to_cta(bar(kBarMerge), dst_cta);
-        const int rows_chunk = (rows_own + 7) >> 3, r0 = chunk * rows_chunk, nr = min(rows_chunk, rows_own - r0);
-        if (nr > 0)
-            dsmem_bulk_copy(map_to_cta(sbase + kTcRecvO + (src_slot * rows_own + r0) * kTcRowFloats * 4, dst_cta),
-                            sbase + kTcPushO + (d * rows_own + r0) * kTcRowFloats * 4, nr * kTcRowFloats * 4, bar_remote);
-        if (chunk == 0)
-            dsmem_bulk_copy(map_to_cta(sbase + kTcRecvML + src_slot * ml_stride * 8, dst_cta),
-                            sbase + push_ml_off + d * ml_stride * 8, ml_stride * 8, bar_remote);
-    }
-    if (warp < kTcSoftmaxWarps && S > 1) {
-        mbar_wait(bar(kBarMerge), 0);
-        // every partial row addressed to this CTA has landed: release the senders (they may not exit before)
-        if (tid < S - 1) mbar_arrive_remote(map_to_cta(bar(kBarAck), tid < split ? tid : tid + 1));
-    }
-    if (tid == 0) HERALD_STAMP(3);
-    if (warp < kTcSoftmaxWarps && owner == split) {
+    if (warp < kTcSoftmaxWarps && owner == split && row < rows_box) {
+        if (merge_bytes > 0) mbar_wait_cluster(bar(kBarMerge), 0);   // every partial row addressed to this CTA has landed
+        if (tid == 0) HERALD_STAMP(3);
         if (row < rows_valid) {
             const float* recv_o = reinterpret_cast<const float*>(sgen + kTcRecvO);
             const float2* recv_ml = reinterpret_cast<const float2*>(sgen + kTcRecvML);
             float mstar = nt > 0 ? m_used : -INFINITY;
+#pragma unroll 1
             for (int s = 0; s < S - 1; ++s) mstar = fmaxf(mstar, recv_ml[s * ml_stride + row_l].x);
             const float w_self = nt > 0 ? fast_exp2(m_used - mstar) : 0.f;
             float den = w_self * l_tot;
 #pragma unroll
             for (int i = 0; i < 32; ++i) o[i] *= w_self;
+#pragma unroll 1
             for (int s = 0; s < S - 1; ++s) {
                 const float2 ml = recv_ml[s * ml_stride + row_l];
                 if (ml.x == -INFINITY) continue;                  // empty split: its rows carry nothing
@@ -701,7 +695,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 }
             }
             const float inv = 1.f / den;
-            float4* dst = reinterpret_cast<float4*>(sgen + stage_off + (row_l * kTcRowFloats + cq * 32) * 4);
+            // the V ring is dead (this thread has seen the last PV of the CTA complete): it stages the finished rows
+            float4* dst = reinterpret_cast<float4*>(sgen + kTcStageO + (row_l * kTcRowFloats + cq * 32) * 4);
 #pragma unroll
             for (int i = 0; i < 8; ++i) dst[i] = make_float4(o[4 * i] * inv, o[4 * i + 1] * inv, o[4 * i + 2] * inv, o[4 * i + 3] * inv);
             if (p.lse && cq == 0) {
@@ -710,11 +705,12 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 p.lse[orow] = (mstar + log2f(den)) * 0.6931471805599453f;
             }
         }
+        if (tid == 0) HERALD_STAMP(7);
     }
     __syncthreads();
     {
         // coalesced copy of this CTA's finished rows: one warp writes one 512-byte row per instruction
-        const float* stage = reinterpret_cast<const float*>(sgen + stage_off);
+        const float* stage = reinterpret_cast<const float*>(sgen + kTcStageO);
         const int r_begin = split * rows_own, r_end = min(min(kTcBM, r_begin + rows_own), rows_valid);
         for (int rl = warp; rl < r_end - r_begin; rl += kTcThreads / 32) {
             const int r = r_begin + rl, bi = (r * g_inv) >> 16;   // r / G
@@ -722,9 +718,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
             *reinterpret_cast<float4*>(p.out + orow * kHeadDim + lane * 4) = *reinterpret_cast<const float4*>(stage + rl * kTcRowFloats + lane * 4);
         }
     }
-    // a CTA may not exit while a bulk copy out of its shared memory is in flight: every owner it sent rows to has acknowledged
-    if (S > 1) mbar_wait(bar(kBarAck), 0);
-    if (tid == 0) HERALD_STAMP(4);
+    // a CTA may not exit while a peer can still arrive on its barriers: every peer has announced its receive buffer by now
+    // (the partial rows addressed to this CTA have landed: the merge waited for them)
+    if (S > 1 && tid == 0) mbar_wait_cluster(bar(kBarPeerReady), 0);
+    if (tid == 0) { HERALD_STAMP(4); HERALD_GSTAMP(63); }
 
     // ---- teardown ----
     if (warp == kTcMmaWarp) {
