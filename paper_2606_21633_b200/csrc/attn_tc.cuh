@@ -384,11 +384,20 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     // requests queue in front of the Q tile and compete with the draining grid, 16.4 -> 16.7 us per C2 step.)
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (tid == 0) HERALD_GSTAMP(61);
-    if (S > 1) cluster_wait_all();     // ... and so are those of every other CTA of the cluster
     // blocks are dispatched in blockIdx order: with a plan (attn_plan_kernel) slot z holds the unit with the z-th longest
     // pool, so that the long units start first and the short ones fill the tail of a multi-wave grid
     const int unit = p.unit_order ? p.unit_order[blockIdx.z] : (int)blockIdx.z;
     const int b = unit / p.n_kv_heads, h = unit % p.n_kv_heads;
+    if (warp == kTcKWarp) {
+        // the Q tile is what the first MMA waits for longest: it is requested before the pool length is even read
+        // (one box of q_blk [batch][B][H_q][128] = (64 channels, G heads, ipt block rows) per half)
+        if (elect_one()) {
+            mbar_arrive_expect_tx(bar(kBarQFull), (uint32_t)rows_box * 256u);
+            tma_load_4d(sbase + kTcSmemQ, &tm_q, 0, h * G, i0, b, bar(kBarQFull));
+            tma_load_4d(sbase + kTcSmemQ + kTcHalfBytes, &tm_q, 64, h * G, i0, b, bar(kBarQFull));
+        }
+        __syncwarp();
+    }
     const int b_pool = b % p.pool_batch, unit_pool = b_pool * p.n_kv_heads + h;   // whose keys: the group's prefix owner
     const bool paged = p.page_table != nullptr;
     const int n_pool = paged ? max(0, min(p.seq_lens[b_pool], p.max_seq_len)) : max(0, min(p.pool_len[unit_pool], p.cap));
@@ -422,15 +431,6 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
             const uint32_t ring = sbase + (is_k ? kTcSmemK : kTcSmemV);
             uint8_t* ring_gen = sgen + (is_k ? kTcSmemK : kTcSmemV);
             int n_fixed = 0;                                  // V tiles whose tail rows were zeroed so far (phase of kBarVTail)
-            if (is_k) {
-                if (elect_one()) {
-                    // Q tile: one box of q_blk [batch][B][H_q][128] = (64 channels, G heads, ipt block rows) per half
-                    mbar_arrive_expect_tx(bar(kBarQFull), (uint32_t)rows_box * 256u);
-                    tma_load_4d(sbase + kTcSmemQ, &tm_q, 0, h * G, i0, b, bar(kBarQFull));
-                    tma_load_4d(sbase + kTcSmemQ + kTcHalfBytes, &tm_q, 64, h * G, i0, b, bar(kBarQFull));
-                }
-                __syncwarp();
-            }
             // dense mode: the page ids of a tile are fetched one tile ahead, so that their round trip does not sit between a
             // ring slot falling free and its TMA requests
             auto tile_phys = [&](int jj) -> int {
@@ -527,7 +527,9 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
 #pragma unroll
                         for (int kk = 0; kk < 8; ++kk) {
                             umma_ts(o_base, p_base + kk * 8, v_lo + kk * 128, hi_k, idesc_pv, (j > 0 || kk > 0) ? 1u : 0u);
+#ifndef HERALD_EXP_NOLO
                             umma_ts(o_base, p_base + 64 + kk * 8, v_lo + kk * 128, hi_k, idesc_pv, 1u);
+#endif
                         }
                     } else {
                         for (int kk = 0; kk < ksteps; ++kk) {
@@ -597,9 +599,11 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                     const float e0 = fast_exp2(x0), e1 = fast_exp2(x1);
                     fadd2(sum0, sum1, sum0, sum1, e0, e1);
                     hi[i] = pack_bf16(e0, e1);
+#ifndef HERALD_EXP_NOLO
                     float r0, r1;
                     ffma2v(r0, r1, __uint_as_float(hi[i] << 16), __uint_as_float(hi[i] & 0xffff0000u), -1.f, e0, e1);   // e - hi, exact
                     lo[i] = pack_bf16(r0, r1);
+#endif
                 }
                 l_run = l_run * alpha + (sum0 + sum1);
                 if (any) {   // rare: the running maximum of some row grew past the threshold -> rescale O in place
@@ -615,7 +619,9 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 // Both halves go to TMEM as the A operand of the PV MMA: row = lane, two keys per 32-bit column; P_hi in
                 // columns [0,64) of the S buffer, P_lo in [64,128), this thread's quarter row at [cq*16, cq*16+16) of each.
                 tmem_st16(lane_base + sb * 128 + cq * 16, hi);
+#ifndef HERALD_EXP_NOLO
                 tmem_st16(lane_base + sb * 128 + 64 + cq * 16, lo);
+#endif
                 tmem_wait_st();
                 tc_fence_before();
                 __syncwarp();
@@ -634,8 +640,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     // The K ring of a CTA is dead once its last QK^T has completed: it receives the other CTAs' partial rows.  The
     // K producer (idle by then) waits for that MMA and tells every peer with a remote arrive on its kBarPeerReady;
     // this happens about a tile period before any partial exists, so no sender ever waits for it in practice.
+    if (warp == kTcKWarp && nt == 0) mbar_wait(bar(kBarQFull), 0);   // the Q box was requested: it must have landed before the CTA exits
     if (warp == kTcKWarp && S > 1) {
         if (nt > 0) mbar_wait(bar(kBarQkDone), 0);
+        cluster_wait_all();   // every CTA of the cluster has initialised its barriers (only this warp arrives on a peer's before it is told to)
         if (lane < S - 1) mbar_arrive_remote(map_to_cta(bar(kBarPeerReady), lane < split ? lane : lane + 1));
     }
     // the next kernel of the stream may be scheduled from here on: its blocks take the SMs as this grid's blocks exit
