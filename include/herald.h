@@ -266,6 +266,13 @@ typedef struct herald_profile {
 /* Stores `prof` (host pointer, must outlive the following pipeline steps) for this thread.  Host only. */
 int herald_pipeline_set_profile(const herald_profile_t* prof);
 
+/* Test hook (no effect on results): the following herald_pipeline_step calls of this thread put a kernel that idles for
+ * `main_us` microseconds on the main stream right after the retrieval stream has been forked, and one that idles for
+ * `retrieval_us` at the head of the retrieval stream's work.  PAPER.md:191: the schedule "affects only the selection and never
+ * the generated output": the pools swap only at the block boundary -- so outputs and pools must not depend
+ * on either delay (tests/test_gpu_full_size.py).  0, 0 switches the hook off; at most 1 s each.  Host only. */
+int herald_pipeline_set_debug_delay(uint32_t main_us, uint32_t retrieval_us);
+
 /* Host-buffer variant used for end-to-end timing: per block, the step's inputs come from (pinned)
  * HOST memory and its outputs return to HOST memory, all asynchronously on the pipeline's streams:
  *   H2D  host_q_rep[l] -> layers[l].q_rep ; host_q_blk/k_blk/v_blk[l] -> layers[l].q_blk/k_blk/v_blk

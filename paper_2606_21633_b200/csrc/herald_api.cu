@@ -23,6 +23,7 @@ namespace herald {
 static thread_local char g_err[512] = "";
 static thread_local const herald_profile_t* g_prof = nullptr;   // timing hooks (herald_pipeline_set_profile)
 static thread_local bool g_prof_armed = false;
+static thread_local uint32_t g_delay_main_us = 0, g_delay_retrieval_us = 0;   // test hook (herald_pipeline_set_debug_delay)
 #ifdef HERALD_ATTN_TRACE
 static unsigned long long* g_attn_trace = nullptr;               // debug builds only: device buffer [CTAs][64]
 #endif                   // true only inside the last layer's retrieval
@@ -75,6 +76,16 @@ static int check_cache(const herald_cache_t* c, bool need_v) {
     if (c->page_stride % 8 || c->token_stride % 8 || c->head_stride % 8 || c->head_stride < kHeadDim)
         return fail(HERALD_ERR_INVALID_ARG, "cache strides must be multiples of 8 elements, head_stride >= 128");
     return HERALD_OK;
+}
+
+// Test hook: one thread that sleeps until the global timer has advanced by `ns` (an artificial delay on a stream).
+__global__ void delay_kernel(unsigned long long ns) {
+    unsigned long long t0, t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+    do {
+        __nanosleep(1000);
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    } while (t - t0 < ns);
 }
 
 // ---- select workspace layout ------------------------------------------------------------------
@@ -986,6 +997,7 @@ int herald_pipeline_step(herald_pipeline_t* p) {
         if (e != cudaSuccess) return cuda_fail(e, "record fork");
         e = cudaStreamWaitEvent(s_ret, ev_fork, 0);
         if (e != cudaSuccess) return cuda_fail(e, "wait fork");
+        if (g_delay_retrieval_us) delay_kernel<<<1, 1, 0, s_ret>>>((unsigned long long)g_delay_retrieval_us * 1000ull);
         int last_sparse = -1;
         for (int l = 0; l < p->n_layers; ++l)
             if (!p->layers[l].dense) last_sparse = l;
@@ -1026,6 +1038,7 @@ int herald_pipeline_step(herald_pipeline_t* p) {
             rc = retrieval();
             if (rc) return rc;
             forked = true;
+            if (g_delay_main_us) delay_kernel<<<1, 1, 0, s_main>>>((unsigned long long)g_delay_main_us * 1000ull);
         }
         if (s == p->n_steps) break;
         for (int l = 0; l < p->n_layers; ++l) {
@@ -1060,6 +1073,13 @@ int herald_debug_set_attn_trace(void* dev_buf) {
     return HERALD_OK;
 }
 #endif
+
+int herald_pipeline_set_debug_delay(uint32_t main_us, uint32_t retrieval_us) {
+    if (main_us > 1000000u || retrieval_us > 1000000u) return fail(HERALD_ERR_INVALID_ARG, "debug delay above one second");
+    g_delay_main_us = main_us;
+    g_delay_retrieval_us = retrieval_us;
+    return HERALD_OK;
+}
 
 int herald_pipeline_set_profile(const herald_profile_t* prof) {
     g_prof = prof;

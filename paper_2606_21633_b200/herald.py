@@ -28,7 +28,8 @@ EXPORTS = ("herald_last_error", "herald_budget_rows", "herald_select_workspace_b
            "herald_dense_attn", "herald_rep_attn_workspace_bytes", "herald_rep_attn",
            "herald_select_rep_workspace_bytes", "herald_select_rep",
            "herald_cache_write_block", "herald_pool_append_block",
-           "herald_pipeline_step", "herald_pipeline_step_host", "herald_pipeline_set_profile")
+           "herald_pipeline_step", "herald_pipeline_step_host", "herald_pipeline_set_profile",
+           "herald_pipeline_set_debug_delay")
 
 
 class HeraldError(RuntimeError):
@@ -266,6 +267,15 @@ _lib.herald_pipeline_set_profile.argtypes = [C.POINTER(Profile)]
 def herald_pipeline_set_profile(prof):
     """prof: a Profile struct (kept alive by the caller) or None."""
     _check(_lib.herald_pipeline_set_profile(C.byref(prof) if prof is not None else None))
+
+
+_lib.herald_pipeline_set_debug_delay.restype = C.c_int
+_lib.herald_pipeline_set_debug_delay.argtypes = [C.c_uint32, C.c_uint32]
+
+
+def herald_pipeline_set_debug_delay(main_us: int, retrieval_us: int):
+    """Test hook: idle kernels on the main / retrieval stream inside the following pipeline steps (0, 0 = off)."""
+    _check(_lib.herald_pipeline_set_debug_delay(int(main_us), int(retrieval_us)))
 
 
 def alloc_workspace(nbytes: int, device) -> torch.Tensor:
