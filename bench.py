@@ -294,7 +294,7 @@ def main():
     rs_sweep = None
     if args.scan_ctas is None:
         # untimed calibration: which SM budget for the overlapped score scan gives the shortest block step
-        rs_sweep = pipe.tune_schedule(tune_start=args.start_after_step is None)
+        rs_sweep = pipe.tune_schedule()
     graphs = None
     if not args.no_graph:
         # the block step is launch-bound (18 kernels of 5-60 us): capture it once per pool parity and replay
@@ -504,7 +504,8 @@ def main():
                    "l2": f"K cache {tokens * w.n_kv_heads * 256 / 2**20:.0f} MiB > 126 MB L2 (no flush needed); the active pool "
                          f"({rows * 512 / 1e6:.0f} MB) is reused by all {n_steps} steps by design",
                    "start_after_step": int(pipe.c.start_after_step), "scan_ctas": int(pipe.c.scan_ctas),
-                   "schedule_sweep_ms (scan_ctas/start_after_step, untimed calibration, eager)": rs_sweep,
+                   "scan_head_permille": int(pipe.c.scan_head_permille),
+                   "schedule_sweep_ms (scan_ctas/start_after_step/scan_head_permille, untimed calibration by herald_pipeline_tune, eager)": rs_sweep,
                    "attn_grid_ctas": H.herald_attn_grid_ctas(shape),
                    "launch": "eager" if graphs is None else "one CUDA graph per pool parity, replayed"},
         "breakdown": {

@@ -18,6 +18,10 @@
  *     library allocates nothing, frees nothing and never synchronises with the host;
  *     all work is enqueued on the stream(s) passed in and is CUDA-graph capturable
  *     (pools are "allocated at initialization and reused across blocks").
+ *     Two exceptions, both host-side helpers: herald_pipeline_tune (a calibration that times block steps) and
+ *     herald_pipeline_step_host (eager only: it orders itself after the previous call's download with an event).
+ *   - one-time per-device setup (shared-memory opt-in, SM count) is kept per device ordinal; a host thread uses the
+ *     device that is current when it calls.  batch * n_kv_heads must not exceed 65535.
  *   - pointers are DEVICE pointers unless the comment says "host"; all device pointers
  *     must be 16-byte aligned.  bf16 = IEEE bfloat16 bit patterns (uint16).
  *   - head_dim must be 128, page_size 16, G = n_q_heads / n_kv_heads an integer <= 8;
@@ -79,6 +83,24 @@ typedef struct herald_cache {
     const int32_t* seq_lens;   /* [batch]                    */
 } herald_cache_t;
 
+/* Launch-geometry overrides (tests, sweeps, profiling).  Every field 0 = the library chooses, which is what every
+ * BASELINE number uses.  The library reads no environment variable; this struct is the only knob.  The values are copied
+ * and apply to the following calls of the CALLING THREAD (workspace-size queries included); NULL restores the defaults.
+ * Results do not depend on any of them (tests/test_gpu_parity.py runs the parity cases under forced geometries). */
+#define HERALD_XQ_AUTO 0
+#define HERALD_XQ_MMA_SYNC 1
+#define HERALD_XQ_TCGEN05 2
+typedef struct herald_tuning {
+    int32_t attn_splits;     /* KV splits (= cluster size) of the attention grid, 1..8                                   */
+    int32_t attn_m_tiles;    /* M tiles per (sequence, KV head); only values above the minimum ceil(B*G/128) are honoured */
+    int32_t attn_total_ctas; /* the attention grid is split over the keys until it reaches this many blocks (default: SMs) */
+    int32_t attn_no_pdl;     /* non-zero: attention kernels are launched without programmatic stream serialization          */
+    int32_t scan_ctas;       /* grid of every score scan (overrides herald_pipeline_t.scan_ctas)                          */
+    int32_t scan_head_major; /* non-zero: the head-major scan even where the page-major one applies                       */
+    int32_t xq_path;         /* herald_select_xq: HERALD_XQ_AUTO / _MMA_SYNC / _TCGEN05                                    */
+} herald_tuning_t;
+int herald_set_tuning(const herald_tuning_t* tuning);
+
 /* Message for the last error returned on this thread ("" if none).  Host only. */
 const char* herald_last_error(void);
 
@@ -87,8 +109,9 @@ const char* herald_last_error(void);
 int32_t herald_budget_rows(int32_t seq_len, int32_t permille);
 
 /* Workspace sizes in bytes for herald_select / herald_sparse_attn with this shape.  Host only;
- * return 0 on an invalid shape.  The two stages run concurrently in the pipeline, so they need
- * two distinct workspaces. */
+ * return 0 on an invalid shape.  (SURVEY.md section 8(b) lists one herald_workspace_bytes: it is two queries because the
+ * two stages run concurrently on the two streams of the pipeline and therefore need two distinct workspaces; the NEXT
+ * entries have their own herald_*_workspace_bytes beside them.) */
 size_t herald_select_workspace_bytes(const herald_shape_t* shape);
 size_t herald_attn_workspace_bytes(const herald_shape_t* shape);
 
@@ -234,13 +257,21 @@ typedef struct herald_pipeline {
     int32_t start_after_step; /* 0 .. n_steps                                           */
     int32_t active;           /* index of the ACTIVE pool buffer; flipped on success    */
     int32_t scan_ctas;        /* grid of the retrieval stream's score scan (1024-thread blocks, one per SM; each takes
-                                 1/scan_ctas of the cache); 0 = one block per SM of the device.  The scan is a long
+                                 1/scan_ctas of the cache); 0 = the SMs the attention grid leaves free, at least an eighth of the
+                                 device (herald_pipeline_tune measures the alternatives).  The scan is a long
                                  bandwidth-bound kernel and the attention blocks need whole SMs:
                                    <= the SMs the attention grid leaves free: the scan streams K beside the denoising
                                       steps without ever taking their SMs (denoising-bound shapes);
                                    a multiple of the SM count: short blocks in several waves, time-sliced with the
                                       attention launches (selection-bound shapes; "bound by the slower
                                       stream", Fig. 14)                                              */
+    int32_t scan_head_permille; /* 0..1000: that many thousandths of the (first sparse layer's) score scan run with one block per
+                                 SM BEFORE the main stream's next denoising step starts (the main stream waits for them), the rest
+                                 with scan_ctas blocks beside the steps.  The retrieval stream needs a fixed amount of SM time
+                                 (an SM draws ~77 GB/s from L2/HBM); when the SMs the attention grid leaves free cannot deliver it
+                                 inside the denoising window, a head start costs less than a retrieval stream that outlasts the
+                                 window.  0 = everything beside the steps (max-logit aggregation only;
+                                 ignored with HERALD_AGG_SOFTMAX_SUM) */
     herald_layer_t* layers;   /* host array [n_layers]                                  */
     int32_t* sel_idx;         /* int32 [batch][H_kv][pool_capacity] scratch (retrieval stream) */
     void* ws_select;
@@ -254,6 +285,18 @@ typedef struct herald_pipeline {
 } herald_pipeline_t;
 
 int herald_pipeline_step(herald_pipeline_t* pipe);
+
+/* Calibration of the schedule of a pipeline (how the retrieval stream shares the device with the denoising steps): runs
+ * eager block steps -- each a complete, valid step, so the pools stay consistent -- for a handful of
+ * (scan_ctas, start_after_step, scan_head_permille) candidates, `reps` timed steps each after two warm-up steps, timed with
+ * CUDA events on the main stream, and leaves the fastest candidate in *pipe.  This is the ONE entry of the library that
+ * creates (and destroys) two events and synchronises with the host; call it once outside any timed region or graph
+ * capture.  table (optional, host): receives up to table_cap measured candidates, *n_table how many.  Host only. */
+typedef struct herald_schedule {
+    int32_t scan_ctas, start_after_step, scan_head_permille;
+    float ms_per_step;
+} herald_schedule_t;
+int herald_pipeline_tune(herald_pipeline_t* pipe, int32_t reps, herald_schedule_t* table, int32_t table_cap, int32_t* n_table);
 
 /* Optional timing hooks for the retrieval stream (measurement only, no effect on results): caller-created
  * events recorded on the retrieval stream around the stages of the LAST layer's selection inside
@@ -291,7 +334,15 @@ typedef struct herald_host_io {
     void* const* host_out;
 } herald_host_io_t;
 
+/* host_q_rep[l] may be NULL for a layer with `dense` set.  Every pointer is validated before anything is enqueued.
+ * Not capturable into a CUDA graph (see Conventions). */
 int herald_pipeline_step_host(herald_pipeline_t* pipe, const herald_host_io_t* io);
+
+#ifdef HERALD_ATTN_TRACE
+/* Debug builds only (-DHERALD_ATTN_TRACE; not part of the release ABI): the attention kernel writes clock64 / globaltimer
+ * stamps of its phases to dev_buf ([blocks of the grid][64] uint64, device memory) on every following launch; NULL stops. */
+int herald_debug_set_attn_trace(void* dev_buf);
+#endif
 
 #ifdef __cplusplus
 }

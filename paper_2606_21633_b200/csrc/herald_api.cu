@@ -4,7 +4,6 @@
 
 #include <cstdarg>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 
 #include "attn_tc.cuh"
@@ -43,10 +42,8 @@ static int cuda_fail(cudaError_t e, const char* what) {
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-static int env_int(const char* name, int dflt) {
-    const char* s = getenv(name);
-    return (s && *s) ? atoi(s) : dflt;
-}
+// launch-geometry overrides of this thread (herald_set_tuning); all zero = automatic
+static thread_local herald_tuning_t g_tune = {0, 0, 0, 0, 0, 0, 0};
 
 static int check_shape(const herald_shape_t* s) {
     if (!s) return fail(HERALD_ERR_INVALID_ARG, "shape is NULL");
@@ -64,6 +61,9 @@ static int check_shape(const herald_shape_t* s) {
     if (s->agg_mode != HERALD_AGG_MAX_LOGIT && s->agg_mode != HERALD_AGG_SOFTMAX_SUM)
         return fail(HERALD_ERR_INVALID_ARG, "agg_mode must be 0 or 1");
     if (!(s->sm_scale > 0.f)) return fail(HERALD_ERR_INVALID_ARG, "sm_scale must be > 0");
+    if ((int64_t)s->batch * s->n_kv_heads > 65535)
+        return fail(HERALD_ERR_UNSUPPORTED, "batch * n_kv_heads = %lld exceeds 65535 (a grid dimension of the gather and attention kernels)",
+                    (long long)s->batch * s->n_kv_heads);
     return HERALD_OK;
 }
 
@@ -94,14 +94,32 @@ struct SelectWs {
     int scan_ctas;
 };
 
+// One-time setup is per DEVICE (cudaFuncSetAttribute applies to the current device; so does the SM count): small tables
+// indexed by the device ordinal.  Races between host threads are benign (the same values are written twice).
+constexpr int kMaxDevices = 64;
+static int current_device() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) dev = 0;
+    return dev;
+}
 static int sm_count() {
-    static int n = 0;
-    if (n == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
-            n = 148;   // B200
+    static int n[kMaxDevices] = {0};
+    const int dev = current_device();
+    if (n[dev] == 0) {
+        int v = 0;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) v = 148;   // B200
+        n[dev] = v;
     }
-    return n;
+    return n[dev];
+}
+// opt a kernel into `bytes` of dynamic shared memory once per device; `done` is that kernel's table
+template <typename Kernel>
+static cudaError_t ensure_smem(Kernel kernel, int bytes, bool (&done)[kMaxDevices]) {
+    const int dev = current_device();
+    if (done[dev]) return cudaSuccess;
+    const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) done[dev] = true;
+    return e;
 }
 
 // grid of the score scan (0 = one block per SM); set by herald_pipeline_step around its select calls
@@ -110,7 +128,7 @@ static thread_local int g_scan_ctas = 0;
 // Grid of the scan: one 1024-thread CTA per SM it may occupy, or several waves of them.
 static int scan_ctas_for(const herald_shape_t* s) {
     (void)s;
-    int n = env_int("HERALD_SCAN_CTAS", 0);
+    int n = g_tune.scan_ctas;
     if (n <= 0) n = g_scan_ctas > 0 ? g_scan_ctas : sm_count();
     if (n > kScanMaxCtas) n = kScanMaxCtas;
     return n;
@@ -150,15 +168,15 @@ static AttnGeom attn_geom(const herald_shape_t* s, bool dense = false) {
     // an M tile is `ipt` whole block rows x G heads (<= 128 rows), balanced over the tiles
     const int rows_cap = kTcBM / G;
     a.m_tiles = (s->block_size + rows_cap - 1) / rows_cap;
-    const int forced_mt = env_int("HERALD_ATTN_MTILES", 0);
+    const int forced_mt = g_tune.attn_m_tiles;
     if (forced_mt > a.m_tiles && forced_mt <= s->block_size) a.m_tiles = forced_mt;
     a.ipt = (s->block_size + a.m_tiles - 1) / a.m_tiles;
     // one CTA per SM: split the keys of a unit over a cluster until the grid covers the 148 SMs once
     const int max_keys = dense ? s->max_seq_len : s->pool_capacity;
     const int max_tiles = 1 + (max_keys + kTcBN - 1) / kTcBN;   // the in-block rows are a key tile of their own
-    const int target = env_int("HERALD_ATTN_TOTAL_CTAS", 148);
+    const int target = g_tune.attn_total_ctas > 0 ? g_tune.attn_total_ctas : sm_count();
     int splits = units > 0 ? target / (units * a.m_tiles) : 1;
-    const int forced = env_int("HERALD_ATTN_SPLITS", 0);
+    const int forced = g_tune.attn_splits;
     if (forced > 0) splits = forced;
     if (splits > max_tiles) splits = max_tiles;
     if (splits > kTcMaxSplits) splits = kTcMaxSplits;
@@ -201,7 +219,7 @@ struct MapSlot {
     CUtensorMap map;
     bool used;
 };
-constexpr int kMapSlots = 4096;      // power of two
+constexpr int kMapSlots = 512;       // power of two; ~70 KB of thread-local storage per thread that launches attention
 constexpr int kMapProbe = 8;
 static thread_local MapSlot g_maps[kMapSlots];
 
@@ -385,12 +403,9 @@ static int launch_topk(const herald_shape_t* shape, const herald_cache_t* cache,
     tp.n_kv_heads = shape->n_kv_heads;
     tp.max_seq_len = shape->max_seq_len;
     tp.cap = shape->pool_capacity;
-    static bool topk_attr_set = false;
-    if (!topk_attr_set) {
-        e = cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTopkMaxSmemBytes);
-        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(topk)");
-        topk_attr_set = true;
-    }
+    static bool topk_attr[kMaxDevices] = {false};
+    e = ensure_smem(topk_kernel, kTopkMaxSmemBytes, topk_attr);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(topk)");
     // shared memory of the one-pass path: a bit per position and room for 1/8 of the positions in the threshold bin
     // (N(0,1)-like scores put 1-5 % of them there); what does not fit takes the multi-pass path
     tp.bitmap_words = (shape->max_seq_len + 31) / 32;
@@ -413,9 +428,13 @@ static int launch_topk(const herald_shape_t* shape, const herald_cache_t* cache,
     return HERALD_OK;
 }
 
-int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep,
+// herald_select in phases.  The pipeline runs the score scan in two launches (herald_pipeline_t.scan_head_permille): a head part
+// over the first `head` thousandths of the cache on every SM, before the denoising steps start, and the rest on the SMs
+// the attention grid leaves free, beside them; the level-1 histogram accumulates over both (global atomics).
+enum { kSelectAll = 0, kSelectHead = 1, kSelectTail = 2 };
+static int select_impl(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep,
                   const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, float* scores_out, void* ws,
-                  size_t ws_bytes, herald_stream_t stream_) {
+                  size_t ws_bytes, herald_stream_t stream_, int phase, int head_permille) {
     int rc = check_shape(shape);
     if (rc) return rc;
     rc = check_cache(cache, false);
@@ -433,10 +452,13 @@ int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, cons
     uint8_t* wsb = static_cast<uint8_t*>(ws);
     uint32_t* hist1 = reinterpret_cast<uint32_t*>(wsb + w.hist1);
     float* scores = scores_out ? scores_out : reinterpret_cast<float*>(wsb + w.scores);
-    cudaError_t e = cudaMemsetAsync(hist1, 0, (size_t)units * kBins1 * sizeof(uint32_t), stream);
-    if (e != cudaSuccess) return cuda_fail(e, "memset hist1");
+    cudaError_t e = cudaSuccess;
+    if (phase != kSelectTail) {
+        e = cudaMemsetAsync(hist1, 0, (size_t)units * kBins1 * sizeof(uint32_t), stream);
+        if (e != cudaSuccess) return cuda_fail(e, "memset hist1");
+    }
     const herald_profile_t* prof = g_prof_armed ? g_prof : nullptr;
-    if (prof && prof->scan_begin) cudaEventRecord(static_cast<cudaEvent_t>(prof->scan_begin), stream);
+    if (prof && prof->scan_begin && phase != kSelectTail) cudaEventRecord(static_cast<cudaEvent_t>(prof->scan_begin), stream);
 
     if (shape->max_seq_len > 0) {
         ScanParams sp{};
@@ -457,18 +479,18 @@ int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, cons
         sp.max_seq_len = shape->max_seq_len;
         sp.max_pages = shape->max_pages_per_seq;
         sp.sm_scale = shape->sm_scale;
-        const int scan_ctas = scan_ctas_for(shape);
+        sp.part_lo = phase == kSelectTail ? head_permille : 0;
+        sp.part_hi = phase == kSelectHead ? head_permille : 1000;
+        // the head part runs alone on the device: one block per SM whatever the overlapped part is given
+        const int scan_ctas = phase == kSelectHead ? (g_tune.scan_ctas > 0 ? g_tune.scan_ctas : sm_count()) : scan_ctas_for(shape);
         dim3 grid(scan_ctas);
         const int Hkv = shape->n_kv_heads;
-        if (shape->agg_mode == HERALD_AGG_MAX_LOGIT && Hkv <= 8 && kScanWarps % Hkv == 0 && !env_int("HERALD_SCAN_HEAD_MAJOR", 0)) {
+        if (shape->agg_mode == HERALD_AGG_MAX_LOGIT && Hkv <= 8 && kScanWarps % Hkv == 0 && !g_tune.scan_head_major) {
             // page-major order: the warps next to each other read the head tiles of one page (whole pages for DRAM)
             const size_t smem = (size_t)Hkv * kBins1 * sizeof(uint32_t);
-            static bool pm_attr_set = false;
-            if (!pm_attr_set) {
-                e = cudaFuncSetAttribute(scan_pm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 8 * kBins1 * (int)sizeof(uint32_t));
-                if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(scan)");
-                pm_attr_set = true;
-            }
+            static bool pm_attr[kMaxDevices] = {false};
+            e = ensure_smem(scan_pm_kernel, 8 * kBins1 * (int)sizeof(uint32_t), pm_attr);
+            if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(scan)");
             scan_pm_kernel<<<grid, kScanThreads, smem, stream>>>(sp);
         } else if (shape->agg_mode == HERALD_AGG_MAX_LOGIT) {
             scan_kernel<0><<<grid, kScanThreads, 0, stream>>>(sp);
@@ -494,11 +516,18 @@ int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, cons
         if (e != cudaSuccess) return cuda_fail(e, "scan launch");
     }
 
+    if (phase == kSelectHead) return HERALD_OK;
     if (prof && prof->scan_end) cudaEventRecord(static_cast<cudaEvent_t>(prof->scan_end), stream);
     rc = launch_topk(shape, cache, scores, hist1, k_per_seq, sel_idx, sel_cnt, stream);
     if (rc) return rc;
     if (prof && prof->topk_end) cudaEventRecord(static_cast<cudaEvent_t>(prof->topk_end), stream);
     return HERALD_OK;
+}
+
+int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep,
+                  const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, float* scores_out, void* ws,
+                  size_t ws_bytes, herald_stream_t stream_) {
+    return select_impl(shape, cache, q_rep, k_per_seq, sel_idx, sel_cnt, scores_out, ws, ws_bytes, stream_, kSelectAll, 0);
 }
 
 int herald_select_xq(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_x, int32_t x,
@@ -532,8 +561,7 @@ int herald_select_xq(const herald_shape_t* shape, const herald_cache_t* cache, c
         // a dense contraction from ~32 score rows per KV head on: tcgen05 (scan_xq_tc.cuh); below that the rows fit a few
         // mma.sync tiles and the kernel is an HBM stream either way (scan_xq.cuh).  HERALD_XQ_TC = 0 / 1 forces one.
         const int rows = x * G;
-        const int want_tc = env_int("HERALD_XQ_TC", -1);
-        if (want_tc == 1 || (want_tc != 0 && rows >= 32)) {
+        if (g_tune.xq_path == HERALD_XQ_TCGEN05 || (g_tune.xq_path != HERALD_XQ_MMA_SYNC && rows >= 32)) {
             CUtensorMap tm_k, tm_q;
             rc = make_paged_map(&tm_k, cache->k_pages, cache, shape->n_kv_heads);
             if (rc) return rc;
@@ -552,13 +580,10 @@ int herald_select_xq(const herald_shape_t* shape, const herald_cache_t* cache, c
             tp.x = x;
             tp.sm_scale = shape->sm_scale;
             const int xt_ctas = scan_ctas_for(shape);
-            tp.set_size = (xt_ctas >= shape->n_kv_heads && !env_int("HERALD_SCAN_HEAD_MAJOR", 0)) ? shape->n_kv_heads : 1;
-            static bool xt_attr_set = false;
-            if (!xt_attr_set) {
-                e = cudaFuncSetAttribute(scan_xq_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kXtSmemBytes + 1024);
-                if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(scan_xq_tc)");
-                xt_attr_set = true;
-            }
+            tp.set_size = (xt_ctas >= shape->n_kv_heads && !g_tune.scan_head_major) ? shape->n_kv_heads : 1;
+            static bool xt_attr[kMaxDevices] = {false};
+            e = ensure_smem(scan_xq_tc_kernel, kXtSmemBytes + 1024, xt_attr);
+            if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(scan_xq_tc)");
             scan_xq_tc_kernel<<<xt_ctas, kXtThreads, kXtSmemBytes + 1024, stream>>>(tm_k, tm_q, tp);
         } else {
             ScanXqParams sp{};
@@ -578,12 +603,9 @@ int herald_select_xq(const herald_shape_t* shape, const herald_cache_t* cache, c
             sp.max_pages = shape->max_pages_per_seq;
             sp.x = x;
             sp.sm_scale = shape->sm_scale;
-            static bool xq_attr_set = false;
-            if (!xq_attr_set) {
-                e = cudaFuncSetAttribute(scan_xq_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kXqMaxSmemBytes);
-                if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(scan_xq)");
-                xq_attr_set = true;
-            }
+            static bool xq_attr[kMaxDevices] = {false};
+            e = ensure_smem(scan_xq_kernel, kXqMaxSmemBytes, xq_attr);
+            if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(scan_xq)");
             const int n_tiles = (x * G + 7) / 8;
             scan_xq_kernel<<<scan_ctas_for(shape), kScanThreads, (size_t)n_tiles * kXqTileBytes, stream>>>(sp);
         }
@@ -650,11 +672,10 @@ static int sparse_attn_impl(const herald_shape_t* shape, const void* pool_k, con
     g_err[0] = 0;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
 
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmemBytes);
+    static bool attn_attr[kMaxDevices] = {false};
+    {
+        const cudaError_t e = ensure_smem(attn_tc_kernel, kTcSmemBytes, attn_attr);
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(attn)");
-        attr_set = true;
     }
     CUtensorMap tm_k, tm_v, tm_q, tm_kb, tm_vb;
     rc = dense ? make_paged_map(&tm_k, pool_k, dense_cache, shape->n_kv_heads) : make_pool_map(&tm_k, pool_k, units_pool, shape->pool_capacity);
@@ -703,7 +724,7 @@ static int sparse_attn_impl(const herald_shape_t* shape, const void* pool_k, con
         attr[n_attr].val.clusterDim.z = 1;
         ++n_attr;
     }
-    if (env_int("HERALD_ATTN_PDL", 1)) {
+    if (!g_tune.attn_no_pdl) {
         // consecutive denoising steps: the next grid is scheduled while this one runs its merge and takes each SM as
         // it is released (the kernel itself waits, griddepcontrol.wait, before its first global read)
         attr[n_attr].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -848,10 +869,10 @@ static int rep_attn_launch(const herald_shape_t* shape, const herald_cache_t* ca
     rp.max_pages = shape->max_pages_per_seq;
     rp.scale_log2 = shape->sm_scale * 1.4426950408889634f;
     const int n_ctas = std::min(2 * sm_count(), kRepMaxCtas);   // persistent: two CTAs per SM
-    static thread_local bool rep_attr_set = false;   // over the 48 KB default: opt in once
-    if (!rep_attr_set) {
-        cudaFuncSetAttribute(rep_attn_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kRepSmemBytes);
-        rep_attr_set = true;
+    static bool rep_attr[kMaxDevices] = {false};   // over the 48 KB default: opt in once per device
+    {
+        const cudaError_t ea = ensure_smem(rep_attn_kernel, kRepSmemBytes, rep_attr);
+        if (ea != cudaSuccess) return cuda_fail(ea, "cudaFuncSetAttribute(rep_attn)");
     }
     rep_attn_kernel<<<n_ctas, kRepThreads, kRepSmemBytes, stream>>>(rp);
     cudaError_t e = cudaGetLastError();
@@ -964,6 +985,17 @@ static int attn_plan(const herald_shape_t* shape, const int32_t* pool_len, int32
     return HERALD_OK;
 }
 
+// Grid of the overlapped score scan when the caller leaves herald_pipeline_t.scan_ctas at 0: the SMs the attention grid
+// leaves free, at least an eighth of the device (a scan grid larger than that takes SMs the next attention launch needs and
+// was measured slower than running the two streams one after the other).
+static int default_scan_ctas(const herald_shape_t* sh) {
+    const int n_sm = sm_count(), attn = herald_attn_grid_ctas(sh);
+    if (attn <= 0) return n_sm;
+    const int rem = attn % n_sm;                         // blocks of the attention grid's last wave
+    const int spare = rem == 0 ? 0 : n_sm - rem, floor8 = n_sm / 8 > 0 ? n_sm / 8 : 1;
+    return spare > floor8 ? spare : floor8;
+}
+
 static int check_pipeline(const herald_pipeline_t* p) {
     if (!p) return fail(HERALD_ERR_INVALID_ARG, "pipeline is NULL");
     int rc = check_shape(&p->shape);
@@ -973,10 +1005,21 @@ static int check_pipeline(const herald_pipeline_t* p) {
         return fail(HERALD_ERR_INVALID_ARG, "pipeline: bad n_steps / start_after_step");
     if (p->active != 0 && p->active != 1) return fail(HERALD_ERR_INVALID_ARG, "pipeline: active must be 0 or 1");
     if (p->scan_ctas < 0) return fail(HERALD_ERR_INVALID_ARG, "pipeline: scan_ctas must be >= 0");
+    if (p->scan_head_permille < 0 || p->scan_head_permille > 1000)
+        return fail(HERALD_ERR_INVALID_ARG, "pipeline: scan_head_permille must be 0..1000");
     if (!p->sel_idx || !p->ws_select || !p->ws_attn || !p->ev_fork || !p->ev_join)
         return fail(HERALD_ERR_INVALID_ARG, "pipeline: NULL scratch / workspace / event");
     if (p->main_stream == p->retrieval_stream)
         return fail(HERALD_ERR_INVALID_ARG, "pipeline: main and retrieval streams must differ");
+    for (int l = 0; l < p->n_layers; ++l) {       // nothing is enqueued unless every layer is complete
+        const herald_layer_t* ly = &p->layers[l];
+        if (!ly->q_blk || !ly->k_blk || !ly->v_blk || !ly->out) return fail(HERALD_ERR_INVALID_ARG, "pipeline: layer %d has a NULL block tensor", l);
+        int rc2 = check_cache(&ly->cache, true);
+        if (rc2) return rc2;
+        if (!ly->dense && (!ly->q_rep || !ly->k_per_seq || !ly->pool_k[0] || !ly->pool_k[1] || !ly->pool_v[0] || !ly->pool_v[1] ||
+                           !ly->pool_len[0] || !ly->pool_len[1]))
+            return fail(HERALD_ERR_INVALID_ARG, "pipeline: sparse layer %d has a NULL q_rep / k_per_seq / pool pointer", l);
+    }
     return HERALD_OK;
 }
 
@@ -991,6 +1034,10 @@ int herald_pipeline_step(herald_pipeline_t* p) {
     const size_t q_step = (size_t)sh->batch * sh->block_size * sh->n_q_heads * kHeadDim;
     const size_t kv_step = (size_t)sh->batch * sh->block_size * sh->n_kv_heads * kHeadDim;
     cudaError_t e;
+    const int scan_ctas = p->scan_ctas > 0 ? p->scan_ctas : default_scan_ctas(sh);
+    // head part of the first sparse layer's scan: on every SM, and the main stream waits for it (max-logit aggregation only)
+    const int head = sh->agg_mode == HERALD_AGG_MAX_LOGIT ? p->scan_head_permille : 0;
+    bool head_pending = false;
 
     auto retrieval = [&]() -> int {
         e = cudaEventRecord(ev_fork, s_main);
@@ -1005,9 +1052,25 @@ int herald_pipeline_step(herald_pipeline_t* p) {
             herald_layer_t* ly = &p->layers[l];
             if (ly->dense) continue;                      // keeps its full KV: nothing to select
             g_prof_armed = (l == last_sparse);
-            g_scan_ctas = p->scan_ctas;
-            int r = herald_select(sh, &ly->cache, ly->q_rep, ly->k_per_seq, p->sel_idx, ly->pool_len[idle], nullptr,
+            g_scan_ctas = scan_ctas;
+            int r;
+            if (head > 0 && !head_pending) {
+                r = select_impl(sh, &ly->cache, ly->q_rep, ly->k_per_seq, p->sel_idx, ly->pool_len[idle], nullptr, p->ws_select,
+                                p->ws_select_bytes, s_ret, kSelectHead, head);
+                if (r == HERALD_OK) {
+                    // the main stream resumes here; the wait is enqueued now because the join records the same event again below
+                    e = cudaEventRecord(ev_join, s_ret);
+                    if (e == cudaSuccess) e = cudaStreamWaitEvent(s_main, ev_join, 0);
+                    if (e != cudaSuccess) r = cuda_fail(e, "record / wait scan head");
+                    head_pending = true;
+                }
+                if (r == HERALD_OK)
+                    r = select_impl(sh, &ly->cache, ly->q_rep, ly->k_per_seq, p->sel_idx, ly->pool_len[idle], nullptr, p->ws_select,
+                                    p->ws_select_bytes, s_ret, kSelectTail, head);
+            } else {
+                r = herald_select(sh, &ly->cache, ly->q_rep, ly->k_per_seq, p->sel_idx, ly->pool_len[idle], nullptr,
                                   p->ws_select, p->ws_select_bytes, s_ret);
+            }
             g_prof_armed = false;
             g_scan_ctas = 0;
             if (r) return r;
@@ -1074,6 +1137,74 @@ int herald_debug_set_attn_trace(void* dev_buf) {
 }
 #endif
 
+int herald_pipeline_tune(herald_pipeline_t* p, int32_t reps, herald_schedule_t* table, int32_t table_cap, int32_t* n_table) {
+    int rc = check_pipeline(p);
+    if (rc) return rc;
+    if (reps < 1 || reps > 1000) return fail(HERALD_ERR_INVALID_ARG, "herald_pipeline_tune: reps must be 1..1000");
+    cudaStream_t s_main = static_cast<cudaStream_t>(p->main_stream), s_ret = static_cast<cudaStream_t>(p->retrieval_stream);
+    cudaEvent_t a, b;
+    cudaError_t e = cudaEventCreate(&a);
+    if (e != cudaSuccess) return cuda_fail(e, "event create");
+    e = cudaEventCreate(&b);
+    if (e != cudaSuccess) { cudaEventDestroy(a); return cuda_fail(e, "event create"); }
+    const int n_sm = sm_count(), spare = default_scan_ctas(&p->shape), start0 = p->start_after_step;
+    int n = 0;
+    float best_ms = 0.f;
+    herald_schedule_t best{p->scan_ctas, p->start_after_step, p->scan_head_permille, 0.f};
+    auto time_one = [&](int ctas, int start, int head) -> int {
+        p->scan_ctas = ctas; p->start_after_step = start; p->scan_head_permille = head;
+        int r = HERALD_OK;
+        for (int i = 0; i < 2 && r == HERALD_OK; ++i) r = herald_pipeline_step(p);
+        if (r) return r;
+        cudaStreamSynchronize(s_main); cudaStreamSynchronize(s_ret);
+        cudaEventRecord(a, s_main);
+        for (int i = 0; i < reps && r == HERALD_OK; ++i) r = herald_pipeline_step(p);
+        if (r) return r;
+        cudaEventRecord(b, s_main);
+        cudaError_t ee = cudaEventSynchronize(b);
+        if (ee != cudaSuccess) return cuda_fail(ee, "herald_pipeline_tune: step failed");
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, a, b);
+        ms /= (float)reps;
+        if (table && n < table_cap) table[n] = herald_schedule_t{ctas, start, head, ms};
+        ++n;
+        if (best_ms == 0.f || ms < best_ms) { best_ms = ms; best = herald_schedule_t{ctas, start, head, ms}; }
+        return HERALD_OK;
+    };
+    // 1. the scan grid beside the denoising steps: around the SMs the attention grid leaves free; every SM; every SM after the last step
+    const int grids[3] = {spare - 2, spare, n_sm / 8};
+    for (int i = 0; i < 3 && rc == HERALD_OK; ++i) {
+        bool dup = grids[i] < 8 && grids[i] != spare;
+        for (int j = 0; j < i; ++j) dup = dup || grids[j] == grids[i];
+        if (!dup && grids[i] >= 1) rc = time_one(grids[i], start0, 0);
+    }
+    if (rc == HERALD_OK) rc = time_one(n_sm, start0, 0);
+    if (rc == HERALD_OK && start0 != p->n_steps && p->n_steps > 0) rc = time_one(n_sm, p->n_steps, 0);
+    // 2. with the best overlapped grid: how much of the scan runs on every SM before the denoising steps start
+    if (rc == HERALD_OK && best.scan_ctas < n_sm && p->shape.agg_mode == HERALD_AGG_MAX_LOGIT) {
+        const int ctas = best.scan_ctas, start = best.start_after_step;
+        const int heads[5] = {100, 200, 300, 450, 600};
+        for (int i = 0; i < 5 && rc == HERALD_OK; ++i) rc = time_one(ctas, start, heads[i]);
+    }
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    p->scan_ctas = best.scan_ctas; p->start_after_step = best.start_after_step; p->scan_head_permille = best.scan_head_permille;
+    if (n_table) *n_table = n < table_cap ? n : table_cap;
+    return rc;
+}
+
+int herald_set_tuning(const herald_tuning_t* t) {
+    if (!t) {
+        g_tune = herald_tuning_t{0, 0, 0, 0, 0, 0, 0};
+        return HERALD_OK;
+    }
+    if (t->attn_splits < 0 || t->attn_splits > kTcMaxSplits || t->attn_m_tiles < 0 || t->attn_total_ctas < 0 || t->scan_ctas < 0 ||
+        t->xq_path < HERALD_XQ_AUTO || t->xq_path > HERALD_XQ_TCGEN05)
+        return fail(HERALD_ERR_INVALID_ARG, "herald_set_tuning: value out of range (attn_splits 0..%d, xq_path 0..2, the rest >= 0)", kTcMaxSplits);
+    g_tune = *t;
+    return HERALD_OK;
+}
+
 int herald_pipeline_set_debug_delay(uint32_t main_us, uint32_t retrieval_us) {
     if (main_us > 1000000u || retrieval_us > 1000000u) return fail(HERALD_ERR_INVALID_ARG, "debug delay above one second");
     g_delay_main_us = main_us;
@@ -1091,6 +1222,9 @@ int herald_pipeline_step_host(herald_pipeline_t* p, const herald_host_io_t* io) 
     if (rc) return rc;
     if (!io || !io->host_q_rep || !io->host_q_blk || !io->host_k_blk || !io->host_v_blk || !io->host_out)
         return fail(HERALD_ERR_INVALID_ARG, "pipeline_step_host: NULL host io");
+    for (int l = 0; l < p->n_layers; ++l)
+        if ((!p->layers[l].dense && !io->host_q_rep[l]) || !io->host_q_blk[l] || !io->host_k_blk[l] || !io->host_v_blk[l] || !io->host_out[l])
+            return fail(HERALD_ERR_INVALID_ARG, "pipeline_step_host: layer %d has a NULL host pointer", l);
     cudaStream_t s_main = static_cast<cudaStream_t>(p->main_stream);
     cudaStream_t s_ret = static_cast<cudaStream_t>(p->retrieval_stream);
     cudaEvent_t ev_fork = static_cast<cudaEvent_t>(p->ev_fork), ev_join = static_cast<cudaEvent_t>(p->ev_join);
@@ -1104,7 +1238,9 @@ int herald_pipeline_step_host(herald_pipeline_t* p, const herald_host_io_t* io) 
     for (int l = 0; l < p->n_layers; ++l) {
         herald_layer_t* ly = &p->layers[l];
         // inputs are enqueued on the main stream; the fork event orders the retrieval stream after them
-        e = cudaMemcpyAsync(const_cast<void*>(ly->q_rep), io->host_q_rep[l], q_rep_bytes, cudaMemcpyHostToDevice, s_main);
+        e = cudaSuccess;
+        if (!ly->dense)                       // a dense layer has no representative query (host_q_rep[l] may be NULL)
+            e = cudaMemcpyAsync(const_cast<void*>(ly->q_rep), io->host_q_rep[l], q_rep_bytes, cudaMemcpyHostToDevice, s_main);
         if (e == cudaSuccess)
             e = cudaMemcpyAsync(const_cast<void*>(ly->q_blk), io->host_q_blk[l], q_step * p->n_steps * 2, cudaMemcpyHostToDevice, s_main);
         if (e == cudaSuccess)

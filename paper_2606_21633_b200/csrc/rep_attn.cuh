@@ -297,6 +297,8 @@ __global__ void __launch_bounds__(kHeadDim * kRepMergeSlices) rep_attn_merge_ker
     if (n_pages == 0) {       // no cached token: zeros, lse = -inf
         if (slice == 0) p.out[(int64_t)row * kHeadDim + ch] = 0.f;
         if (p.lse && tid == 0) p.lse[row] = -INFINITY;
+        // (see the end of the kernel) completion of this grid must imply completion of the top-k it runs beside
+        if (!p.merge_waits) asm volatile("griddepcontrol.wait;" ::: "memory");
         return;
     }
     if (tid == 0) {           // the row's partial list: one thread does the 64-bit divisions
@@ -360,6 +362,11 @@ __global__ void __launch_bounds__(kHeadDim * kRepMergeSlices) rep_attn_merge_ker
         p.out[(int64_t)row * kHeadDim + ch] = num / den;
         if (p.lse && ch == 0) p.lse[row] = (ms + log2f(den)) * 0.6931471805599453f;
     }
+    // herald_select_rep (merge_waits == 0): this grid runs BESIDE the top-k it was launched behind (the top-k releases its
+    // dependents at once; the partials were complete before that).  It is the last kernel the entry enqueues, so whatever is
+    // ordered behind it -- a programmatic launch, the next node of a captured graph -- must also be behind the top-k, which is
+    // still reading the score plane / histogram and writing sel_idx / sel_cnt: wait for it here, after the outputs are written.
+    if (!p.merge_waits) asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 }  // namespace herald

@@ -30,6 +30,8 @@ struct ScanParams {
     float2* stats_part;   // [batch*H_kv][G][gridDim.x] (m, l)       (mode 1)
     uint32_t* hist1;      // [batch*H_kv][kBins1]                    (mode 0)
     int32_t batch, n_q_heads, n_kv_heads, max_seq_len, max_pages;
+    int32_t part_lo, part_hi;   // this launch covers [part_lo, part_hi) thousandths of the tile space (0, 1000 = all of it): the
+                                // pipeline runs a head part on every SM before the denoising steps and the rest beside them
     float sm_scale;
 };
 
@@ -45,6 +47,11 @@ __device__ __forceinline__ int seq_pages(const ScanParams& p, int b) {
     return (min(p.seq_lens[b], p.max_seq_len) + kPageSize - 1) / kPageSize;
 }
 __device__ __forceinline__ int64_t cta_range_begin(int64_t total, int cta, int n_ctas) { return total * cta / n_ctas; }
+// the same cut inside the part [lo, hi) thousandths of the tile space
+__device__ __forceinline__ int64_t cta_part_begin(int64_t total, int lo, int hi, int cta, int n_ctas) {
+    const int64_t r0 = total * lo / 1000, r1 = total * hi / 1000;
+    return r0 + (r1 - r0) * cta / n_ctas;
+}
 
 template <int kMode>
 __global__ void __launch_bounds__(kScanThreads, 1) scan_kernel(const ScanParams p) {
@@ -65,7 +72,9 @@ __global__ void __launch_bounds__(kScanThreads, 1) scan_kernel(const ScanParams 
         for (int i = threadIdx.x; i < kBins1; i += kScanThreads) s_hist[i] = 0;
     __syncthreads();
     const int64_t total = s_total;
-    const int64_t g0 = cta_range_begin(total, blockIdx.x, gridDim.x), g1 = cta_range_begin(total, blockIdx.x + 1, gridDim.x);
+    // (mode 1 always covers the whole space: its partial statistics are indexed by the same cut in aggregate_softmax_kernel)
+    const int64_t g0 = kMode == 0 ? cta_part_begin(total, p.part_lo, p.part_hi, blockIdx.x, gridDim.x) : cta_range_begin(total, blockIdx.x, gridDim.x);
+    const int64_t g1 = kMode == 0 ? cta_part_begin(total, p.part_lo, p.part_hi, blockIdx.x + 1, gridDim.x) : cta_range_begin(total, blockIdx.x + 1, gridDim.x);
 
     // walk the units that intersect [g0, g1)
     int64_t unit_begin = 0;   // global tile index of the current unit's page 0
@@ -214,7 +223,8 @@ __global__ void __launch_bounds__(kScanThreads, 1) scan_pm_kernel(const ScanPara
     for (int i = threadIdx.x; i < H * kBins1; i += kScanThreads) s_hist_pm[i] = 0;
     __syncthreads();
     const int64_t total = s_total;
-    const int64_t g0 = cta_range_begin(total, blockIdx.x, gridDim.x), g1 = cta_range_begin(total, blockIdx.x + 1, gridDim.x);
+    const int64_t g0 = cta_part_begin(total, p.part_lo, p.part_hi, blockIdx.x, gridDim.x);
+    const int64_t g1 = cta_part_begin(total, p.part_lo, p.part_hi, blockIdx.x + 1, gridDim.x);
     uint32_t* my_hist = s_hist_pm + h * kBins1;
     const bool v0 = 2 * tig < G, v1 = 2 * tig + 1 < G;
 

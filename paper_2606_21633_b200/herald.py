@@ -23,12 +23,12 @@ _lib = C.CDLL(LIB_PATH)
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE_TOO_SMALL, ERR_CUDA = 0, -1, -2, -3, -4
 AGG_MAX_LOGIT, AGG_SOFTMAX_SUM = 0, 1
 
-EXPORTS = ("herald_last_error", "herald_budget_rows", "herald_select_workspace_bytes",
+EXPORTS = ("herald_last_error", "herald_set_tuning", "herald_budget_rows", "herald_select_workspace_bytes",
            "herald_attn_workspace_bytes", "herald_attn_grid_ctas", "herald_select", "herald_select_xq", "herald_gather", "herald_sparse_attn", "herald_sparse_attn_groups",
            "herald_dense_attn", "herald_rep_attn_workspace_bytes", "herald_rep_attn",
            "herald_select_rep_workspace_bytes", "herald_select_rep",
            "herald_cache_write_block", "herald_pool_append_block",
-           "herald_pipeline_step", "herald_pipeline_step_host", "herald_pipeline_set_profile",
+           "herald_pipeline_step", "herald_pipeline_tune", "herald_pipeline_step_host", "herald_pipeline_set_profile",
            "herald_pipeline_set_debug_delay")
 
 
@@ -60,17 +60,30 @@ class Layer(C.Structure):
 class Pipeline(C.Structure):
     _fields_ = [("shape", Shape), ("n_layers", C.c_int32), ("n_steps", C.c_int32),
                 ("start_after_step", C.c_int32), ("active", C.c_int32), ("scan_ctas", C.c_int32),
-                ("layers", C.POINTER(Layer)),
+                ("scan_head_permille", C.c_int32), ("layers", C.POINTER(Layer)),
                 ("sel_idx", C.c_void_p), ("ws_select", C.c_void_p), ("ws_select_bytes", C.c_size_t),
                 ("ws_attn", C.c_void_p), ("ws_attn_bytes", C.c_size_t),
                 ("main_stream", C.c_void_p), ("retrieval_stream", C.c_void_p),
                 ("ev_fork", C.c_void_p), ("ev_join", C.c_void_p)]
 
 
+class Schedule(C.Structure):
+    _fields_ = [("scan_ctas", C.c_int32), ("start_after_step", C.c_int32), ("scan_head_permille", C.c_int32),
+                ("ms_per_step", C.c_float)]
+
+
 class HostIO(C.Structure):
     _fields_ = [("host_q_rep", C.POINTER(C.c_void_p)), ("host_q_blk", C.POINTER(C.c_void_p)),
                 ("host_k_blk", C.POINTER(C.c_void_p)), ("host_v_blk", C.POINTER(C.c_void_p)),
                 ("host_out", C.POINTER(C.c_void_p))]
+
+
+class Tuning(C.Structure):
+    _fields_ = [("attn_splits", C.c_int32), ("attn_m_tiles", C.c_int32), ("attn_total_ctas", C.c_int32),
+                ("attn_no_pdl", C.c_int32), ("scan_ctas", C.c_int32), ("scan_head_major", C.c_int32), ("xq_path", C.c_int32)]
+
+
+XQ_AUTO, XQ_MMA_SYNC, XQ_TCGEN05 = 0, 1, 2
 
 
 class Profile(C.Structure):
@@ -118,6 +131,8 @@ _lib.herald_pool_append_block.restype = C.c_int
 _lib.herald_pool_append_block.argtypes = [C.POINTER(Shape)] + [C.c_void_p] * 6
 _lib.herald_pipeline_step.restype = C.c_int
 _lib.herald_pipeline_step.argtypes = [C.POINTER(Pipeline)]
+_lib.herald_pipeline_tune.restype = C.c_int
+_lib.herald_pipeline_tune.argtypes = [C.POINTER(Pipeline), C.c_int32, C.POINTER(Schedule), C.c_int32, C.POINTER(C.c_int32)]
 _lib.herald_pipeline_step_host.restype = C.c_int
 _lib.herald_pipeline_step_host.argtypes = [C.POINTER(Pipeline), C.POINTER(HostIO)]
 
@@ -150,6 +165,19 @@ def _ws(ws):
 def _check(rc):
     if rc != 0:
         raise HeraldError(rc, _lib.herald_last_error().decode())
+
+
+_lib.herald_set_tuning.restype = C.c_int
+_lib.herald_set_tuning.argtypes = [C.POINTER(Tuning)]
+
+
+def herald_set_tuning(**fields):
+    """Launch-geometry overrides for the following calls of this thread; no arguments = the defaults."""
+    if not fields:
+        _check(_lib.herald_set_tuning(None))
+    else:
+        t = Tuning(**fields)
+        _check(_lib.herald_set_tuning(C.byref(t)))
 
 
 def herald_last_error() -> str:
@@ -287,7 +315,8 @@ class BlockPipeline:
     """Owns the device buffers of a dual-stream block pipeline (pools, workspaces, streams, events)
     and the ctypes structs that describe them.  Marshalling and memory ownership only."""
 
-    def __init__(self, shape: Shape, layers, n_steps: int, start_after_step: int = 0, device="cuda", scan_ctas=None):
+    def __init__(self, shape: Shape, layers, n_steps: int, start_after_step: int = 0, device="cuda", scan_ctas=None,
+                 scan_head_permille: int = 0):
         """layers: list of dicts with torch tensors k_pages, v_pages, page_table, seq_lens, q_rep, k_per_seq,
         q_blk, k_blk, v_blk ([n_steps, ...]); optional "dense": True for a layer that keeps its full KV."""
         dev = torch.device(device)
@@ -326,10 +355,9 @@ class BlockPipeline:
         p = Pipeline()
         p.shape, p.n_layers, p.n_steps, p.start_after_step, p.active = shape, len(layers), n_steps, start_after_step, 0
         if scan_ctas is None:
-            # the score scan takes the SMs the attention grid leaves free (at least 1/8 of the device)
-            n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
-            scan_ctas = max(n_sm - herald_attn_grid_ctas(shape), n_sm // 8)
+            scan_ctas = 0          # the library's default: the SMs the attention grid leaves free
         p.scan_ctas = int(scan_ctas)
+        p.scan_head_permille = int(scan_head_permille)
         p.layers = C.cast(self.layer_arr, C.POINTER(Layer))
         p.sel_idx = _ptr(self.sel_idx)
         p.ws_select, p.ws_select_bytes = _ptr(self.ws_select), self.ws_select.numel()
@@ -360,56 +388,27 @@ class BlockPipeline:
     def step_host(self, io: HostIO):
         herald_pipeline_step_host(self.c, io)
 
-    def tune_schedule(self, candidates=None, reps=4, tune_start=True):
-        """Pick how the retrieval stream shares the device with the denoising steps by timing eager block steps
-        (CUDA events on the main stream) for a few schedules (scan_ctas, start_after_step):
-          * scan grid = the SMs the attention grid leaves free: the scan streams K beside the attention launches
-            (denoising-bound shapes);
-          * scan grid = every SM, started with the block or only after the last denoising step (selection-bound
-            shapes, where both streams are HBM-bound and overlapping them buys nothing: "bound by the
-            slower stream", Fig. 14).
-        Returns {"scan_ctas/start_after_step": ms per step}; leaves the fastest schedule set.  Pool contents stay
-        valid (every step is a complete block step)."""
-        n_sm = torch.cuda.get_device_properties(self.device).multi_processor_count
-        if candidates is None:
-            spare = n_sm - herald_attn_grid_ctas(self.shape)
-            start0 = int(self.c.start_after_step)
-            candidates = [(c, start0) for c in sorted({c for c in (spare - 2, spare, n_sm // 8) if c >= 8})]
-            candidates.append((n_sm, start0))
-            if tune_start and start0 != self.n_steps:
-                candidates.append((n_sm, self.n_steps))
-        table = {}
-        for ctas, start in candidates:
-            self.c.scan_ctas, self.c.start_after_step = int(ctas), int(start)
-            for _ in range(2):
-                self.step()
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            torch.cuda.synchronize(self.device)
-            a.record(self.main_stream)
-            for _ in range(reps):
-                self.step()
-            b.record(self.main_stream)
-            torch.cuda.synchronize(self.device)
-            table[(int(ctas), int(start))] = a.elapsed_time(b) / reps
-        best = min(table, key=table.get)
-        self.c.scan_ctas, self.c.start_after_step = best
-        return {f"{c}/{st}": ms for (c, st), ms in table.items()}
+    def tune_schedule(self, reps=4):
+        """herald_pipeline_tune: times a handful of schedules (scan grid, start step, head start of the scan) with eager block
+        steps outside any timed region and leaves the fastest one set.  Returns {"scan_ctas/start/head_permille": ms per step}."""
+        table = (Schedule * 32)()
+        n = C.c_int32(0)
+        _check(_lib.herald_pipeline_tune(C.byref(self.c), int(reps), table, 32, C.byref(n)))
+        return {f"{t.scan_ctas}/{t.start_after_step}/{t.scan_head_permille}": t.ms_per_step for t in table[:n.value]}
 
     # ---- CUDA graphs: one captured block step per pool parity (launch-bound inner loop, no per-launch host cost) ----
-    def capture(self, io: HostIO = None):
-        """Capture herald_pipeline_step (or the host-IO variant) twice, once per value of ``active``, into two CUDA
-        graphs whose root is the main stream; the retrieval stream joins the capture through the fork/join events.
-        Run at least one eager step first (function attributes and tensor maps are set up on first use)."""
+    def capture(self):
+        """Capture herald_pipeline_step twice, once per value of ``active``, into two CUDA graphs whose root is the main
+        stream; the retrieval stream joins the capture through the fork/join events.  Run at least one eager step first
+        (function attributes and tensor maps are set up on first use).  herald_pipeline_step_host is eager-only: it orders
+        itself after the previous call's download through an event recorded outside any capture."""
         graphs = {}
         start = self.active
         for _ in range(2):
             parity = self.active
             g = torch.cuda.CUDAGraph()
             with torch.cuda.graph(g, stream=self.main_stream, capture_error_mode="thread_local"):
-                if io is None:
-                    herald_pipeline_step(self.c)
-                else:
-                    herald_pipeline_step_host(self.c, io)
+                herald_pipeline_step(self.c)
             graphs[parity] = g                      # the capture flipped ->active exactly like an eager step
         assert self.active == start
         return graphs

@@ -23,6 +23,7 @@ def H():
 def declared_functions():
     text = open(os.path.join(ROOT, "include", "herald.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    text = re.sub(r"#ifdef HERALD_ATTN_TRACE.*?#endif", "", text, flags=re.S)      # debug builds only, not in the release ABI
     return sorted(set(re.findall(r"\b(herald_[a-z_]+)\s*\(", text)))
 
 
@@ -120,3 +121,69 @@ def test_follow_up_entries_check_their_arguments_before_any_cuda_call(H):
     with pytest.raises(H.HeraldError) as ei:          # x queries: the aggregation is only defined for max-logit (reading 25)
         H.herald_select_xq(shape1, cache, 256, 2, 256, 256, 256, None, big, stream=0)
     assert ei.value.code == H.ERR_INVALID_ARG
+
+
+def test_tuning_struct_is_the_only_knob(H):
+    """No environment variable is read by the library (no env-var magic); geometry overrides go
+    through herald_set_tuning, are validated, and change the attention grid the size query reports."""
+    src = open(os.path.join(ROOT, "paper_2606_21633_b200", "csrc", "herald_api.cu")).read()
+    assert "getenv" not in src
+    shape = H.make_shape(8, 28, 4, 32, 32768, 2048, 1639 + 32)
+    try:
+        base = H.herald_attn_grid_ctas(shape)
+        assert base == 128                                   # 2 KV splits x 2 M tiles x 32 units on 148 SMs
+        H.herald_set_tuning(attn_splits=1)
+        assert H.herald_attn_grid_ctas(shape) == 64
+        H.herald_set_tuning(attn_splits=4)
+        assert H.herald_attn_grid_ctas(shape) == 256
+        for bad in (dict(attn_splits=9), dict(attn_splits=-1), dict(xq_path=3), dict(scan_ctas=-2)):
+            with pytest.raises(H.HeraldError) as ei:
+                H.herald_set_tuning(**bad)
+            assert ei.value.code == H.ERR_INVALID_ARG
+        assert H.herald_attn_grid_ctas(shape) == 256         # a rejected call changes nothing
+    finally:
+        H.herald_set_tuning()
+    assert H.herald_attn_grid_ctas(shape) == base
+
+
+def test_too_many_units_is_unsupported(H):
+    shape = H.make_shape(20000, 8, 4, 16, 1024, 64, 64)      # 80000 (sequence, KV head) units > 65535
+    assert H.herald_select_workspace_bytes(shape) == 0
+    cache = H.Cache(256, 256, 16 * 4 * 128, 4 * 128, 128, 256, 256)
+    with pytest.raises(H.HeraldError) as ei:
+        H.herald_gather(shape, cache, 256, 256, 256, 256, stream=0)
+    assert ei.value.code == H.ERR_UNSUPPORTED
+
+
+def test_pipeline_arguments_are_validated_before_anything_is_enqueued(H):
+    shape = H.make_shape(2, 8, 4, 16, 1024, 64, 64)
+    layers = (H.Layer * 1)()
+    ly = layers[0]
+    ly.cache = H.Cache(256, 256, 16 * 4 * 128, 4 * 128, 128, 256, 256)
+    ly.q_rep = ly.k_per_seq = ly.q_blk = ly.k_blk = ly.v_blk = ly.out = 256
+    for j in range(2):
+        ly.pool_k[j] = ly.pool_v[j] = ly.pool_len[j] = 256
+    p = H.Pipeline()
+    p.shape, p.n_layers, p.n_steps, p.start_after_step, p.active, p.scan_ctas, p.scan_head_permille = shape, 1, 3, 0, 0, 0, 0
+    p.layers = C.cast(layers, C.POINTER(H.Layer))
+    p.sel_idx = p.ws_select = p.ws_attn = 256
+    p.ws_select_bytes = p.ws_attn_bytes = 1 << 30
+    p.main_stream, p.retrieval_stream, p.ev_fork, p.ev_join = 1, 2, 256, 256
+    def expect(code):
+        with pytest.raises(H.HeraldError) as ei:
+            H.herald_pipeline_step(p)
+        assert ei.value.code == code, str(ei.value)
+        assert p.active == 0                                  # a rejected step does not swap the pools
+    p.scan_head_permille = 1001
+    expect(H.ERR_INVALID_ARG)
+    p.scan_head_permille = 0
+    p.start_after_step = 4
+    expect(H.ERR_INVALID_ARG)
+    p.start_after_step = 0
+    ly.pool_v[1] = None                                       # a sparse layer needs both pool buffers ...
+    expect(H.ERR_INVALID_ARG)
+    ly.dense = 1                                              # ... a dense one does not, but still its block tensors
+    ly.out = None
+    expect(H.ERR_INVALID_ARG)
+    p.retrieval_stream = 1
+    expect(H.ERR_INVALID_ARG)

@@ -255,3 +255,61 @@ def test_pipeline_is_independent_of_stream_delays(H, cuda, start_after):
         for blk in range(2):
             for a, b in zip(base[blk], got[blk]):
                 assert torch.equal(a.view(torch.uint8), b.view(torch.uint8)), (main_us, retrieval_us, blk)
+
+
+def test_fused_retrieval_chained_in_one_graph(H, cuda):
+    """herald_select_rep -> herald_gather -> attention, twice back to back with different representative queries, captured
+    in ONE CUDA graph: the second selection reuses the workspace (histogram, score plane) of the first, so everything the
+    first enqueued -- its top-k included -- must be complete when the entry's last kernel is (the graph orders the next
+    node only behind that one).  Pools of both rounds against the oracle."""
+    w = synth.Workload("chain", 2, (9000, 4100), 28, 4, 32, 3, 50, "planted", 12)
+    inp = synth.make_inputs(w, seed=808, device=cuda, spare_pages=1, hostile_tails=True)
+    ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
+    cap = max(ks) + w.block_size
+    shape = _shape(H, w, inp, cap)
+    cache = H.make_cache(inp["k_pages"], inp["v_pages"], inp["page_table"], inp["seq_lens"])
+    k_per_seq = torch.tensor(ks, dtype=torch.int32, device=cuda)
+    g = torch.Generator(device=cuda)
+    g.manual_seed(809)
+    q_reps = [inp["q_rep"], torch.randn(inp["q_rep"].shape, generator=g, device=cuda).to(torch.bfloat16)]
+    sel_idx = torch.zeros((w.batch, w.n_kv_heads, cap), dtype=torch.int32, device=cuda)
+    sel_cnt = [torch.zeros((w.batch, w.n_kv_heads), dtype=torch.int32, device=cuda) for _ in range(2)]
+    pools_k = [torch.zeros((w.batch, w.n_kv_heads, cap, 128), dtype=torch.bfloat16, device=cuda) for _ in range(2)]
+    pools_v = [torch.zeros_like(pools_k[0]) for _ in range(2)]
+    rep_out = torch.empty((w.batch, w.n_q_heads, 128), dtype=torch.float32, device=cuda)
+    outs = [torch.empty((w.batch, w.block_size, w.n_q_heads, 128), dtype=torch.float32, device=cuda) for _ in range(2)]
+    ws = H.alloc_workspace(H.herald_select_rep_workspace_bytes(shape), cuda)
+    ws_att = H.alloc_workspace(H.herald_attn_workspace_bytes(shape), cuda)
+    st = torch.cuda.Stream()
+
+    def chain():
+        for r in range(2):
+            H.herald_select_rep(shape, cache, q_reps[r], k_per_seq, sel_idx, sel_cnt[r], None, rep_out, None, ws, st)
+            H.herald_gather(shape, cache, sel_idx, sel_cnt[r], pools_k[r], pools_v[r], st)
+            H.herald_sparse_attn(shape, pools_k[r], pools_v[r], sel_cnt[r], inp["q_blk"][r], inp["k_blk"][r], inp["v_blk"][r], outs[r], None, ws_att, st)
+
+    with torch.cuda.stream(st):
+        chain()                          # eager once: one-time setup
+    torch.cuda.synchronize()
+    gr = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(gr, stream=st, capture_error_mode="thread_local"):
+        chain()
+    for it in range(5):
+        for t in pools_k + pools_v:
+            t.zero_()
+        torch.cuda.synchronize()
+        with torch.cuda.stream(st):
+            gr.replay()
+        torch.cuda.synchronize()
+        for r in range(2):
+            for b in range(w.batch):
+                L = w.seq_lens[b]
+                kp, vp, ident = _seq_view(inp, b, L, cuda)
+                sel_o, _ = O.select(synth.to_u16(q_reps[r][b:b + 1]), kp, ident, np.array([L]), [ks[b]], w.n_kv_heads, 128 ** -0.5)
+                pk_o, pv_o, pl_o = O.gather(kp, vp, ident, sel_o, cap)
+                assert np.array_equal(sel_cnt[r][b].cpu().numpy(), pl_o[0])
+                n = ks[b]
+                assert np.array_equal(synth.to_u16(pools_k[r][b])[:, :n], pk_o[0][:, :n]), (it, r, b)
+                assert np.array_equal(synth.to_u16(pools_v[r][b])[:, :n], pv_o[0][:, :n]), (it, r, b)
+                if it == 0:
+                    _check_attn("chain", {k: v for k, v in inp.items()}, b, r, pools_k[r], pools_v[r], pl_o, outs[r])

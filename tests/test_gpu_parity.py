@@ -17,6 +17,13 @@ def H():
     return herald
 
 
+@pytest.fixture
+def tuning(H):
+    """herald_set_tuning for one test; the defaults come back afterwards."""
+    yield H.herald_set_tuning
+    H.herald_set_tuning()
+
+
 def run_select(H, w, inp, ks, agg_mode=0, cap=None, want_scores=True):
     dev = inp["k_pages"].device
     cap = cap if cap is not None else max(max(ks), 1) + w.block_size
@@ -83,14 +90,12 @@ XQ_CASES = [("tiny_ragged", 1), ("tiny_ragged", 3), ("one_token", 2), ("g7_ragge
 
 @pytest.mark.parametrize("path", ["auto", "mma_sync", "tcgen05"])
 @pytest.mark.parametrize("case,x", XQ_CASES)
-def test_select_xq_matches_oracle(H, cuda, case, x, path, monkeypatch):
+def test_select_xq_matches_oracle(H, cuda, case, x, path, tuning):
     """herald_select_xq (NEXT-4, Fig. 8): x queries per sequence, maximum over the x*G score rows
     (reading 25).  Same bar as herald_select: scores within 1e-4, index sets exact outside the band.
     Both kernels (mma.sync below ~32 score rows per KV head, tcgen05 above) are forced over every case."""
     if path != "auto":
-        monkeypatch.setenv("HERALD_XQ_TC", "1" if path == "tcgen05" else "0")
-    else:
-        monkeypatch.delenv("HERALD_XQ_TC", raising=False)
+        tuning(xq_path=H.XQ_TCGEN05 if path == "tcgen05" else H.XQ_MMA_SYNC)
     c = SELECT_CASES[case]
     w = c["w"]
     inp = synth.make_inputs(w, seed=100 + len(case), device=cuda, spare_pages=c["spare"], hostile_tails=c["hostile"])
@@ -126,11 +131,10 @@ def test_select_xq_matches_oracle(H, cuda, case, x, path, monkeypatch):
 
 
 @pytest.mark.parametrize("ctas", [1, 5, 37])
-def test_select_xq_small_grids(H, cuda, ctas, monkeypatch):
+def test_select_xq_small_grids(H, cuda, ctas, tuning):
     """Grids smaller than H_kv (no CTA sets), not a multiple of it (idle CTAs past the last set), and a single CTA."""
-    monkeypatch.setenv("HERALD_SCAN_CTAS", str(ctas))
-    for path in ("0", "1"):
-        monkeypatch.setenv("HERALD_XQ_TC", path)
+    for path in (H.XQ_MMA_SYNC, H.XQ_TCGEN05):
+        tuning(scan_ctas=ctas, xq_path=path)
         c = SELECT_CASES["g8_h8"]
         w = c["w"]
         inp = synth.make_inputs(w, seed=321, device=cuda, spare_pages=1, hostile_tails=True)
@@ -441,8 +445,8 @@ def test_sparse_attn_matches_oracle(H, cuda, case):
 
 
 @pytest.mark.parametrize("splits", [1, 2, 3, 5, 8])
-def test_sparse_attn_split_kv_is_consistent(H, cuda, splits, monkeypatch):
-    monkeypatch.setenv("HERALD_ATTN_SPLITS", str(splits))
+def test_sparse_attn_split_kv_is_consistent(H, cuda, splits, tuning):
+    tuning(attn_splits=splits)
     batch, B, Hq, Hkv, cap = 1, 32, 14, 2, 600
     q, kb, vb, pk, pv, pl = _attn_case(cuda, batch, B, Hq, Hkv, cap, [[600, 100]], seed=77)
     shape = H.make_shape(batch, Hq, Hkv, B, 16, 1, cap)
@@ -458,11 +462,11 @@ def test_sparse_attn_split_kv_is_consistent(H, cuda, splits, monkeypatch):
 
 
 @pytest.mark.parametrize("splits", [1, 2])
-def test_sparse_attn_late_peaks_rescale_the_accumulator(H, cuda, splits, monkeypatch):
+def test_sparse_attn_late_peaks_rescale_the_accumulator(H, cuda, splits, tuning):
     """The running row maximum is lazy (it moves only when a tile exceeds it by 2^40): keys planted deep in the pool that
     match one query row each make the logit of that row jump by hundreds of log2 units in a late tile, so the in-place
     rescale of the accumulator in TMEM runs -- in some rows of a tile and not in others, more than once per row."""
-    monkeypatch.setenv("HERALD_ATTN_SPLITS", str(splits))
+    tuning(attn_splits=splits)
     batch, B, Hq, Hkv, cap = 1, 32, 14, 2, 900
     q, kb, vb, pk, pv, pl = _attn_case(cuda, batch, B, Hq, Hkv, cap, [[900, 520]], seed=311)
     G = Hq // Hkv
@@ -520,10 +524,10 @@ def test_sparse_attn_groups_share_the_pools(H, cuda, n_groups):
 
 
 @pytest.mark.parametrize("splits", [7, 8])
-def test_sparse_attn_more_splits_than_tile_rows(H, cuda, splits, monkeypatch):
+def test_sparse_attn_more_splits_than_tile_rows(H, cuda, splits, tuning):
     """G = 1, B = 8: the M tile has 8 real rows, so with 7 or 8 KV splits some CTAs of the cluster own no row at all;
-    they still send their partials and are still acknowledged."""
-    monkeypatch.setenv("HERALD_ATTN_SPLITS", str(splits))
+    they still send their partials."""
+    tuning(attn_splits=splits)
     batch, B, Hq, Hkv, cap = 2, 8, 2, 2, 1100
     q, kb, vb, pk, pv, pl = _attn_case(cuda, batch, B, Hq, Hkv, cap, [[1100, 900], [130, 0]], seed=78)
     shape = H.make_shape(batch, Hq, Hkv, B, 16, 1, cap)
