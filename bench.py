@@ -9,6 +9,9 @@ B=32, T=16 -> 15 attention steps, 5 % budget -> k=1639, 16-token pages, 0.5 % pl
   join + pool swap.
 value = block tokens/s = batch*B / t_step with every input resident in HBM; `e2e` runs the same step
 through herald_pipeline_step_host with per-step inputs in pinned HOST memory and outputs copied back.
+Beside the C2 line the default run also reports, under `breakdown`: compact lines for C1, C3 and C4@5
+(`other_workloads`), the Fig. 14 analogue (`fig14_sweep`: T x start_after_step on C2),
+L2-cold attention, and median / min over repeated timed regions.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
 
@@ -86,7 +89,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.FIELDS}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._pump, daemon=True)
             self.thread.start()
@@ -126,16 +129,29 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 # the oracle arm (cpu_baseline and --impl reference)
 # ------------------------------------------------------------------------------------------------
-def oracle_block_step(host, n_seq, n_steps):
+def workload_desc(w, n_layers, ks):
+    lens = f"ragged {min(w.seq_lens)}..{w.max_seq_len}" if len(set(w.seq_lens)) > 1 else str(w.max_seq_len)
+    return (f"{w.name}: {n_layers} layer(s) {w.n_q_heads}/{w.n_kv_heads}/128 heads, batch {w.batch} x {lens} paged (16-token pages), "
+            f"B={w.block_size}, T={w.denoise_steps} ({w.n_attn_steps} attention steps), budget {w.permille / 10:g}% k={max(ks)}, "
+            f"structure {w.structure}")
+
+
+def oracle_block_step(host, n_seq, n_steps, stage_s=None):
     """One block step of the oracle on the first n_seq sequences of the workload (host NumPy inputs)."""
     from oracle import herald_oracle as O
     sl = slice(0, n_seq)
     H_kv = host["k_pages"].shape[2]
+    t0 = time.perf_counter()
     sel, _ = O.select(host["q_rep"][sl], host["k_pages"], host["page_table"][sl], host["seq_lens"][sl],
                       host["ks"][:n_seq], H_kv, 128 ** -0.5)
+    t1 = time.perf_counter()
     pk, pv, pl = O.gather(host["k_pages"], host["v_pages"], host["page_table"][sl], sel, host["cap"])
+    t2 = time.perf_counter()
     for s in range(n_steps):
         O.sparse_attn(host["q_blk"][s][sl], host["k_blk"][s][sl], host["v_blk"][s][sl], pk, pv, pl, 128 ** -0.5)
+    t3 = time.perf_counter()
+    if stage_s is not None:
+        stage_s.append((t1 - t0, t2 - t1, (t3 - t2) / max(n_steps, 1)))
 
 
 def host_inputs(w, inp, ks, cap):
@@ -155,33 +171,50 @@ def blas_threads():
 
 
 def time_oracle(host, w, n_seq, reps):
-    times = []
+    """The oracle as it stands on the host cores: whole block steps (all BLAS threads), their stages, and one
+    single-threaded block step on one sequence."""
+    times, stages = [], []
     for _ in range(reps):
         t0 = time.perf_counter()
-        oracle_block_step(host, n_seq, w.n_attn_steps)
+        oracle_block_step(host, n_seq, w.n_attn_steps, stages)
         times.append(time.perf_counter() - t0)
     t = statistics.median(times)
-    return {"value": n_seq * w.block_size / t, "unit": "tokens/s", "cores": blas_threads(), "kind": "oracle",
-            "sample": f"{n_seq} of {w.batch} sequences of {w.name} (select + gather + {w.n_attn_steps} attention steps), "
-                      f"median of {reps} block steps, {t:.2f} s each; NumPy fp64, BLAS threads as configured"}
+    st = [statistics.median(x[i] for x in stages) for i in range(3)]
+    out = {"value": n_seq * w.block_size / t, "unit": "tokens/s", "cores": blas_threads(), "kind": "oracle",
+           "sample": f"{n_seq} of {w.batch} sequences of {w.name} (select + gather + {w.n_attn_steps} attention steps), "
+                     f"median of {reps} block steps, {t:.2f} s each; NumPy fp64, BLAS threads as configured",
+           "per_stage_s": {"select (scores + aggregate + top-k)": st[0], "gather": st[1], "attention, one step": st[2],
+                           "sequences": n_seq}}
+    try:
+        from threadpoolctl import threadpool_limits
+        with threadpool_limits(limits=1):
+            s1 = []
+            t0 = time.perf_counter()
+            oracle_block_step(host, 1, w.n_attn_steps, s1)
+            t1 = time.perf_counter() - t0
+        out["single_thread"] = {"value": w.block_size / t1, "unit": "tokens/s", "cores": 1,
+                                "sample": f"1 of {w.batch} sequences, one block step, {t1:.2f} s",
+                                "per_stage_s": {"select (scores + aggregate + top-k)": s1[0][0], "gather": s1[0][1],
+                                                "attention, one step": s1[0][2], "sequences": 1}}
+    except Exception as exc:                      # threadpoolctl missing: say so rather than guess
+        out["single_thread"] = {"unavailable": repr(exc)}
+    return out
 
 
 def run_reference(args):
-    """--impl reference: the fp64 oracle as it stands, on host cores, same config/metric."""
+    """--impl reference: the fp64 oracle as it stands, on host cores, same workload / metric as the CUDA arm."""
     rank, _, world = dist_env()
     if rank != 0:
         return 0
     import torch
     from oracle import herald_oracle as O
     from paper_2606_21633_b200 import synth
-    w = synth.config(WORKLOAD)
-    n_seq = 1                                  # bounded sample: one sequence of the batch per step
-    sub = synth.Workload(w.name, n_seq, w.seq_lens[:n_seq], w.n_q_heads, w.n_kv_heads, w.block_size, w.denoise_steps,
-                         w.permille, w.structure, w.planted_per_unit)
-    inp = synth.make_inputs(sub, SEED, "cpu")
-    ks = [O.budget_rows(L, w.permille) for L in sub.seq_lens]
+    w = synth.config(args.workload)
+    inp = synth.make_inputs(w, SEED, "cpu")
+    ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
     cap = max(ks) + w.block_size
-    host = host_inputs(sub, inp, ks, cap)
+    host = host_inputs(w, inp, ks, cap)
+    n_seq = w.batch                            # the whole batch of the workload per step (about 1.7 s on C2)
     for _ in range(args.warmup):
         oracle_block_step(host, n_seq, w.n_attn_steps)
     t0 = time.perf_counter()
@@ -192,19 +225,14 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": "tokens/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{WORKLOAD}: single layer 28/4/128 heads, batch 8 x 32768 paged (16-token pages), B=32, T=16 "
-                                   "(15 attention steps), budget 5% k=1639, structure planted",
-                       "note": f"oracle timed on a bounded sample: {n_seq} of {w.batch} sequences per step"},
+            "config": {"workload": workload_desc(w, 1, ks)},
             "cpu_baseline": {"value": value, "unit": "tokens/s", "cores": blas_threads(), "kind": "oracle",
-                             "sample": f"{n_seq} of {w.batch} sequences of {WORKLOAD} per step"},
+                             "sample": f"the whole batch ({n_seq} sequences) of {w.name} per step"},
             "e2e": {"value": value, "unit": "tokens/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
     return 0
 
 
-# ------------------------------------------------------------------------------------------------
-# the CUDA arm
-# ------------------------------------------------------------------------------------------------
 def load_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -213,6 +241,262 @@ def load_peaks():
         return {"hbm_gbs": p["hbm_gbs"], "bf16_tflops": p["bf16_tflops"],
                 "bf16_tflops_sustained": p.get("bf16_tflops_sustained", p["bf16_tflops"]), "source": "measured"}
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ------------------------------------------------------------------------------------------------
+class Rig:
+    """One workload resident on the device: inputs, the block pipeline, and the timers every line of the report uses."""
+
+    def __init__(self, H, synth, torch, name, dev, seed, n_layers=None, dense_layers=0, start_after=0, scan_ctas=None,
+                 denoise_steps=None):
+        from dataclasses import replace
+        self.H, self.torch, self.dev = H, torch, dev
+        w = synth.config(name)
+        if denoise_steps is not None:
+            w = replace(w, denoise_steps=denoise_steps)
+        self.w = w
+        self.ks = [H.herald_budget_rows(L, w.permille) for L in w.seq_lens]
+        self.cap = max(self.ks) + w.block_size
+        self.n_steps = w.n_attn_steps
+        n_layers = n_layers or w.n_layers
+        if n_layers > 1:      # layers of the stack (C5): own cache, q_rep, block inputs, pools and outputs each; keep what fits
+            pages = sum((L + 15) // 16 for L in w.seq_lens)
+            per_layer = (pages * 16 * w.n_kv_heads * 256 * 2 + 4 * w.batch * w.n_kv_heads * self.cap * 256
+                         + self.n_steps * w.batch * w.block_size * (w.n_q_heads * (512 + 256) + w.n_kv_heads * 512))
+            free_b, _ = torch.cuda.mem_get_info(dev)
+            fit = int((free_b * 0.92 - 3e9) // per_layer)
+            if fit < n_layers:
+                print(f"bench.py: {n_layers} layers need {n_layers * per_layer / 1e9:.0f} GB, {free_b / 1e9:.0f} GB are free: "
+                      f"running {max(fit, 1)} layers", file=sys.stderr)
+                n_layers = max(fit, 1)
+        self.n_layers = n_layers
+        self.inps = [synth.make_inputs(w, seed + 97 * l, dev) for l in range(n_layers)]
+        inp = self.inp = self.inps[0]
+        self.shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, (w.max_seq_len + 15) // 16 * 16,
+                                  inp["page_table"].shape[1], self.cap)
+        self.k_per_seq = torch.tensor(self.ks, dtype=torch.int32, device=dev)
+        layers = [dict(k_pages=x["k_pages"], v_pages=x["v_pages"], page_table=x["page_table"], seq_lens=x["seq_lens"],
+                       q_rep=x["q_rep"], k_per_seq=self.k_per_seq, q_blk=x["q_blk"], k_blk=x["k_blk"], v_blk=x["v_blk"]) for x in self.inps]
+        self.n_dense = max(0, min(dense_layers, n_layers - 1))
+        for ly in layers[n_layers - self.n_dense:]:   # (which layers are dense does not matter to the step; layer 0 stays sparse for the stage timings)
+            ly["dense"] = True
+        self.pipe = H.BlockPipeline(self.shape, layers, self.n_steps, start_after, dev, scan_ctas=scan_ctas)
+        self.units = w.batch * w.n_kv_heads
+        self.graphs = None
+        self.side = torch.cuda.Stream(device=dev)
+        # ---- algorithmic work per block step (DESIGN.md section 6) ----
+        G, M = w.group, w.block_size * w.group
+        self.tokens = sum(w.seq_lens)
+        self.scan_bytes = self.tokens * w.n_kv_heads * (256 + 4)          # K row read + fp32 score written
+        self.rows = sum(self.ks) * w.n_kv_heads
+        self.gather_bytes = self.rows * 1024                              # 512 B read + 512 B written per row
+        n_keys = [k + w.block_size for k in self.ks]
+        self.attn_flops = sum(4 * M * n * 128 for n in n_keys) * w.n_kv_heads     # QK^T + PV per attention step
+        self.attn_bytes = sum(n * 512 for n in n_keys) * w.n_kv_heads + self.units * M * (256 + 512)
+
+    def ev(self):
+        return self.torch.cuda.Event(enable_timing=True)
+
+    def warm(self, n=3):
+        for _ in range(n):
+            self.pipe.step()
+        self.torch.cuda.synchronize()
+
+    def capture(self):
+        self.graphs = self.pipe.capture()
+        for _ in range(2):
+            self.pipe.replay(self.graphs)
+        self.torch.cuda.synchronize()
+
+    def run_block(self):
+        if self.graphs is not None:
+            self.pipe.replay(self.graphs)
+        else:
+            self.pipe.step()
+
+    def time_block(self, steps):
+        """ms per block step over `steps` back-to-back steps (CUDA events on the main stream)."""
+        a, b = self.ev(), self.ev()
+        self.torch.cuda.synchronize()
+        a.record(self.pipe.main_stream)
+        for _ in range(steps):
+            self.run_block()
+        b.record(self.pipe.main_stream)
+        self.torch.cuda.synchronize()
+        return a.elapsed_time(b) / steps
+
+    def stage_times(self, n_sets=8):
+        """scan / top-k / gather inside the overlapped step: eager steps with CUDA events on the retrieval stream."""
+        H = self.H
+        prof_events, profs = [], []
+        for _ in range(n_sets):
+            e4 = [self.ev() for _ in range(4)]
+            for e in e4:
+                e.record(self.pipe.retrieval_stream)
+            prof_events.append(e4)
+            profs.append(H.Profile(*[e.cuda_event for e in e4]))
+        for i in range(n_sets):
+            H.herald_pipeline_set_profile(profs[i])
+            self.pipe.step()
+        self.torch.cuda.synchronize()
+        H.herald_pipeline_set_profile(None)
+        mean = statistics.mean
+        return (mean(e4[0].elapsed_time(e4[1]) for e4 in prof_events), mean(e4[1].elapsed_time(e4[2]) for e4 in prof_events),
+                mean(e4[2].elapsed_time(e4[3]) for e4 in prof_events))
+
+    def time_isolated(self, fn, reps=20, warm=3, timed=5):
+        """ms per call of `fn`: `reps` calls captured in one CUDA graph (no host launch cost between them), replayed."""
+        torch, side = self.torch, self.side
+        with torch.cuda.stream(side):
+            for _ in range(warm):
+                fn()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side, capture_error_mode="thread_local"):
+            for _ in range(reps):
+                fn()
+        with torch.cuda.stream(side):
+            g.replay()
+            torch.cuda.synchronize()
+            a, b = self.ev(), self.ev()
+            a.record(side)
+            for _ in range(timed):
+                g.replay()
+            b.record(side)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / (reps * timed)
+
+    def isolated_stages(self, cold_attention=False):
+        """Every stage alone, inputs in HBM: select, the scan kernel by itself, gather, one attention step."""
+        H, torch, w, inp, side, shape = self.H, self.torch, self.w, self.inp, self.side, self.shape
+        dev, pipe = self.dev, self.pipe
+        cache = self.cache = H.make_cache(inp["k_pages"], inp["v_pages"], inp["page_table"], inp["seq_lens"])
+        sel_idx = self.sel_idx = torch.zeros((self.units, self.cap), dtype=torch.int32, device=dev)
+        sel_cnt = self.sel_cnt = torch.zeros((self.units,), dtype=torch.int32, device=dev)
+        ws_sel = self.ws_sel = H.alloc_workspace(H.herald_select_workspace_bytes(shape), dev)
+        ws_att = self.ws_att = H.alloc_workspace(H.herald_attn_workspace_bytes(shape), dev)
+        act = pipe.active
+        out1 = self.out1 = torch.empty((w.batch, w.block_size, w.n_q_heads, 128), dtype=torch.float32, device=dev)
+        res = {}
+        res["select_alone_ms"] = self.time_isolated(lambda: H.herald_select(shape, cache, inp["q_rep"], self.k_per_seq, sel_idx, sel_cnt, None, ws_sel, side))
+        # the scan kernel by itself, two ways.  (1) Difference of two captured graphs of 20 x herald_select with k = 0 (memset,
+        # scan, a top-k that exits at once): over the real cache, and over the same cache with every sequence length 0 (the
+        # same three launches with nothing to scan) -- launch overheads and the two small kernels cancel.  (2) herald_select's
+        # own timing hooks: events recorded right before and after the kernel in eager launches; this one still carries the
+        # event / launch latency of an eager stream (a few us) and is the upper bound.
+        k_zero = torch.zeros_like(self.k_per_seq)
+        empty_cache = H.make_cache(inp["k_pages"], inp["v_pages"], inp["page_table"], torch.zeros_like(inp["seq_lens"]))
+        t_full = self.time_isolated(lambda: H.herald_select(shape, cache, inp["q_rep"], k_zero, sel_idx, sel_cnt, None, ws_sel, side))
+        t_empty = self.time_isolated(lambda: H.herald_select(shape, empty_cache, inp["q_rep"], k_zero, sel_idx, sel_cnt, None, ws_sel, side))
+        res["scan_kernel_ms"] = t_full - t_empty
+        res["scan_with_memset_and_empty_topk_ms"] = t_full
+        n_rep = 12
+        evs = [[self.ev() for _ in range(3)] for _ in range(n_rep)]
+        with torch.cuda.stream(side):
+            for e3 in evs:
+                for e in e3:
+                    e.record(side)                 # materialises the cudaEvent_t handles
+            profs = [H.Profile(e[0].cuda_event, e[1].cuda_event, e[2].cuda_event, None) for e in evs]
+            for i in range(n_rep):
+                H.herald_pipeline_set_profile(profs[i])
+                H.herald_select(shape, cache, inp["q_rep"], self.k_per_seq, sel_idx, sel_cnt, None, ws_sel, side)
+        torch.cuda.synchronize()
+        H.herald_pipeline_set_profile(None)
+        scan_k = sorted(e[0].elapsed_time(e[1]) for e in evs[2:])
+        res["scan_kernel_eager_events_ms"] = statistics.median(scan_k)
+        res["scan_kernel_eager_events_min_ms"] = scan_k[0]
+        res["topk_kernel_eager_events_ms"] = statistics.median(e[1].elapsed_time(e[2]) for e in evs[2:])
+        res["gather_alone_ms"] = self.time_isolated(lambda: H.herald_gather(shape, cache, sel_idx, sel_cnt, pipe.pools_k[0][1 - act], pipe.pools_v[0][1 - act], side))
+        step_i = [0]
+
+        def attn_once():
+            s = step_i[0] % self.n_steps
+            step_i[0] += 1
+            H.herald_sparse_attn(shape, pipe.pools_k[0][act], pipe.pools_v[0][act], pipe.pool_lens[0][act],
+                                 inp["q_blk"][s], inp["k_blk"][s], inp["v_blk"][s], out1, None, ws_att, side)
+        self.attn_once = attn_once
+        res["attn_step_alone_ms"] = self.time_isolated(attn_once, reps=self.n_steps)
+        if cold_attention:
+            # L2-cold: a 512 MiB stream is written between launches (the 126 MB L2 holds nothing of the pool afterwards);
+            # one eager launch between two events, so the figure carries ~2 us of launch latency the warm one does not
+            flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+            cold = []
+            with torch.cuda.stream(side):
+                for i in range(12):
+                    flush.fill_(i)
+                    a, b = self.ev(), self.ev()
+                    a.record(side)
+                    attn_once()
+                    b.record(side)
+                    cold.append((a, b))
+            torch.cuda.synchronize()
+            c = sorted(a.elapsed_time(b) for a, b in cold[2:])
+            res["attn_step_l2_cold_ms"] = statistics.median(c)
+            res["attn_step_l2_cold_min_ms"] = c[0]
+            del flush
+        return res
+
+
+def compact_line(rig, peaks, steps=10, regions=3):
+    """Block step, stage times and roofline fractions of one workload (breakdown.other_workloads)."""
+    rig.warm()
+    sweep = rig.pipe.tune_schedule()
+    rig.capture()
+    reg = sorted(rig.time_block(steps) for _ in range(regions))
+    ms = statistics.median(reg)
+    iso = rig.isolated_stages()
+    w, n_steps = rig.w, rig.n_steps
+    attn_live = ms / n_steps
+    denoise = iso["attn_step_alone_ms"] * n_steps
+    hbm_attn_bound = w.block_size * w.group < 128          # M = 64 shapes: the pool stream, not the tensor pipe, bounds the step
+    line = {"workload": workload_desc(w, rig.n_layers, rig.ks), "block_latency_ms": ms, "block_latency_min_ms": reg[0],
+            "tokens_per_s": w.batch * w.block_size / (ms * 1e-3),
+            "schedule": {"scan_ctas": int(rig.pipe.c.scan_ctas), "start_after_step": int(rig.pipe.c.start_after_step),
+                         "scan_head_permille": int(rig.pipe.c.scan_head_permille), "sweep_ms": sweep},
+            "scan_kernel_ms": iso["scan_kernel_ms"], "scan_gbs_alone": rig.scan_bytes / (iso["scan_kernel_ms"] * 1e-3) / 1e9,
+            "scan_frac_of_measured_hbm": rig.scan_bytes / (iso["scan_kernel_ms"] * 1e-3) / 1e9 / peaks["hbm_gbs"],
+            "scan_pct_of_8TBs": 100.0 * rig.scan_bytes / (iso["scan_kernel_ms"] * 1e-3) / 1e9 / 8000.0,
+            "select_alone_ms": iso["select_alone_ms"], "gather_alone_ms": iso["gather_alone_ms"],
+            "gather_gbs_alone": rig.gather_bytes / (iso["gather_alone_ms"] * 1e-3) / 1e9,
+            "attn_step_alone_ms": iso["attn_step_alone_ms"],
+            "attn_tflops_alone": rig.attn_flops / (iso["attn_step_alone_ms"] * 1e-3) / 1e12,
+            "attn_tflops_in_pipeline": rig.attn_flops / (attn_live * 1e-3) / 1e12,
+            "attn_frac_of_sustained_bf16": rig.attn_flops / (attn_live * 1e-3) / 1e12 / peaks["bf16_tflops_sustained"],
+            "attn_pool_gbs_alone": rig.attn_bytes / (iso["attn_step_alone_ms"] * 1e-3) / 1e9,
+            "attn_bound": "hbm (M = %d rows per unit: %.0f FLOP/B)" % (w.block_size * w.group, rig.attn_flops / rig.attn_bytes) if hbm_attn_bound else "tensor",
+            "denoise_alone_ms": denoise, "exposed_selection_ms": ms - denoise,
+            "exposed_selection_frac": (ms - denoise) / ms}
+    return line
+
+
+def fig14_sweep(H, synth, torch, dev, seed, scan_ctas):
+    """Fig. 14 analogue (retrieval latency ~constant in T, main-stream latency grows with T, small T is
+    retrieval-bound): C2 with T in {8, 16, 20, 32} denoising steps and the retrieval stream started after 0 (north_star)
+    or 2 steps.  Main stream = (T-1) x attention alone; retrieval = scan + top-k + gather inside the step."""
+    rows = []
+    for T in (8, 16, 20, 32):
+        rig = Rig(H, synth, torch, "C2", dev, seed, denoise_steps=T, scan_ctas=scan_ctas)
+        rig.warm()
+        iso_attn = None
+        for start in (0, 2):
+            rig.pipe.c.start_after_step = start
+            rig.graphs = None
+            rig.warm(2)
+            scan_ms, topk_ms, gather_ms = rig.stage_times(4)
+            rig.capture()
+            reg = sorted(rig.time_block(6) for _ in range(3))
+            if iso_attn is None:
+                iso_attn = rig.isolated_stages()["attn_step_alone_ms"]
+            main_ms = iso_attn * rig.n_steps
+            rows.append({"T": T, "start_after_step": start, "block_latency_ms": statistics.median(reg),
+                         "main_stream_alone_ms": main_ms, "retrieval_stream_ms": scan_ms + topk_ms + gather_ms,
+                         "exposed_ms": statistics.median(reg) - main_ms,
+                         "bound": "retrieval" if statistics.median(reg) - main_ms > 0.05 * statistics.median(reg) else "main"})
+        del rig
+        torch.cuda.empty_cache()
+    return rows
 
 
 def main():
@@ -224,14 +508,15 @@ def main():
     ap.add_argument("--workload", default=WORKLOAD)
     ap.add_argument("--layers", type=int, default=None, help="layers of the stack (default: the workload's; C5 has 28)")
     ap.add_argument("--start-after-step", type=int, default=None,
-                    help="denoising steps before the retrieval stream starts (default: 0 or T-1, calibrated)")
+                    help="denoising steps before the retrieval stream starts (default: 0, or what the calibration finds)")
     ap.add_argument("--dense-layers", type=int, default=0,
                     help="layers of the stack that keep their full KV and attend over the cache itself (PAPER.md:181: two in "
                          "the paper's models); 0 = every layer sparse, the configuration BASELINE.json quotes")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--scan-ctas", type=int, default=None,
-                    help="grid of the overlapped score scan (default: calibrated before the timed region)")
+                    help="grid of the overlapped score scan (default: calibrated by herald_pipeline_tune before the timed region)")
     ap.add_argument("--no-graph", action="store_true", help="launch every kernel eagerly instead of replaying the captured block step")
+    ap.add_argument("--quick", action="store_true", help="the C2 line only: no other workloads, no Fig. 14 sweep, no NEXT-row timings")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -244,72 +529,25 @@ def main():
     dev = torch.device("cuda", local_rank)
     torch.cuda.set_device(dev)
     peaks = load_peaks()
+    full = not args.quick and world == 1 and args.workload == WORKLOAD and not args.no_graph
 
-    w = synth.config(args.workload)
-    ks = [H.herald_budget_rows(L, w.permille) for L in w.seq_lens]
-    cap = max(ks) + w.block_size
-    n_steps = w.n_attn_steps
-    # layers of the stack (C5): every layer has its own cache, q_rep, block inputs, pools and outputs; keep what fits
-    n_layers = args.layers or w.n_layers
-    if n_layers > 1:
-        pages = sum((L + 15) // 16 for L in w.seq_lens)
-        per_layer = (pages * 16 * w.n_kv_heads * 256 * 2 + 4 * w.batch * w.n_kv_heads * cap * 256
-                     + n_steps * w.batch * w.block_size * (w.n_q_heads * (512 + 256) + w.n_kv_heads * 512))
-        free_b, _ = torch.cuda.mem_get_info(dev)
-        fit = int((free_b * 0.92 - 3e9) // per_layer)
-        if fit < n_layers:
-            print(f"bench.py: {n_layers} layers need {n_layers * per_layer / 1e9:.0f} GB, {free_b / 1e9:.0f} GB are free: "
-                  f"running {max(fit, 1)} layers", file=sys.stderr)
-            n_layers = max(fit, 1)
-    inps = [synth.make_inputs(w, SEED + rank + 97 * l, dev) for l in range(n_layers)]
-    inp = inps[0]
-    shape = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, (w.max_seq_len + 15) // 16 * 16,
-                         inp["page_table"].shape[1], cap)
-    k_per_seq = torch.tensor(ks, dtype=torch.int32, device=dev)
-    layers = [dict(k_pages=x["k_pages"], v_pages=x["v_pages"], page_table=x["page_table"], seq_lens=x["seq_lens"],
-                   q_rep=x["q_rep"], k_per_seq=k_per_seq, q_blk=x["q_blk"], k_blk=x["k_blk"], v_blk=x["v_blk"]) for x in inps]
-    n_dense = max(0, min(args.dense_layers, n_layers - 1))
-    for ly in layers[n_layers - n_dense:]:     # (which layers are dense does not matter to the step; layer 0 stays sparse for the stage timings)
-        ly["dense"] = True
-    pipe = H.BlockPipeline(shape, layers, n_steps, args.start_after_step or 0, dev, scan_ctas=args.scan_ctas)
-    units = w.batch * w.n_kv_heads
-    G, M = w.group, w.block_size * w.group
+    rig = Rig(H, synth, torch, args.workload, dev, SEED + rank, n_layers=args.layers, dense_layers=args.dense_layers,
+              start_after=args.start_after_step or 0, scan_ctas=args.scan_ctas)
+    w, pipe, inp, shape, n_steps, n_layers, n_dense = rig.w, rig.pipe, rig.inp, rig.shape, rig.n_steps, rig.n_layers, rig.n_dense
+    ks, cap, units, tokens = rig.ks, rig.cap, rig.units, rig.tokens
 
-    # ---- algorithmic work per block step ----
-    tokens = sum(w.seq_lens)
-    scan_bytes = tokens * w.n_kv_heads * (256 + 4)                    # K row read + fp32 score written
-    rows = sum(ks) * w.n_kv_heads
-    gather_bytes = rows * 1024                                        # 512 B read + 512 B written per row
-    n_keys = [k + w.block_size for k in ks]
-    attn_flops = sum(4 * M * n * 128 for n in n_keys) * w.n_kv_heads  # QK^T + PV per attention step
-    attn_bytes = sum(n * 512 for n in n_keys) * w.n_kv_heads + units * M * (256 + 512)
-
-    def ev():
-        return torch.cuda.Event(enable_timing=True)
-
-    # ---- warm-up (eager: sets function attributes, fills the tensor-map cache), then the timed region ----
-    for _ in range(max(args.warmup, 3)):
-        pipe.step()
-    torch.cuda.synchronize()
+    # ---- warm-up (eager: sets function attributes, fills the tensor-map cache), calibration, then the timed region ----
+    rig.warm(max(args.warmup, 3))
     rs_sweep = None
     if args.scan_ctas is None:
-        # untimed calibration: which SM budget for the overlapped score scan gives the shortest block step
+        # untimed calibration (herald_pipeline_tune): scan grid, start step and head start of the scan with the shortest block step
         rs_sweep = pipe.tune_schedule()
-    graphs = None
+        if args.start_after_step is not None:
+            pipe.c.start_after_step = args.start_after_step
     if not args.no_graph:
-        # the block step is launch-bound (18 kernels of 5-60 us): capture it once per pool parity and replay
-        graphs = pipe.capture()
-        for _ in range(2):
-            pipe.replay(graphs)
-        torch.cuda.synchronize()
+        rig.capture()       # the block step is launch-bound (18 kernels of 5-60 us): one CUDA graph per pool parity, replayed
 
-    def run_block():
-        if graphs is not None:
-            pipe.replay(graphs)
-        else:
-            pipe.step()
-
-    t_begin, t_end = ev(), ev()
+    t_begin, t_end = rig.ev(), rig.ev()
     clocks = ClockSampler(local_rank)
     clocks.start()
     time.sleep(0.3)
@@ -317,130 +555,84 @@ def main():
     torch.cuda.synchronize()
     t_begin.record(pipe.main_stream)
     for i in range(args.steps):
-        run_block()
+        rig.run_block()
     t_end.record(pipe.main_stream)
     torch.cuda.synchronize()
     barrier()
-    clock_info = clocks.stop()
     ms_total = max_over_ranks(t_begin.elapsed_time(t_end), dev)
     ms_step = ms_total / args.steps
     tokens_per_s = world * w.batch * w.block_size / (ms_step * 1e-3)
+    # the same region repeated (still under the clock sampler): median and minimum of the per-step time
+    regions = [ms_step] + [rig.time_block(args.steps) for _ in range(6)]
+    clock_info = clocks.stop()
+    regions_sorted = sorted(regions)
 
-    # ---- stage times inside the overlapped step: eager steps with CUDA events on the retrieval stream ----
-    n_sets = 8
-    prof_events, profs = [], []
-    for _ in range(n_sets):
-        e4 = [ev() for _ in range(4)]
-        for e in e4:
-            e.record(pipe.retrieval_stream)
-        prof_events.append(e4)
-        profs.append(H.Profile(*[e.cuda_event for e in e4]))
-    for i in range(n_sets):
-        H.herald_pipeline_set_profile(profs[i])
-        pipe.step()
-    torch.cuda.synchronize()
-    H.herald_pipeline_set_profile(None)
-    scan_ms = statistics.mean(e4[0].elapsed_time(e4[1]) for e4 in prof_events)
-    topk_ms = statistics.mean(e4[1].elapsed_time(e4[2]) for e4 in prof_events)
-    gather_ms = statistics.mean(e4[2].elapsed_time(e4[3]) for e4 in prof_events)
-
-    # ---- stage timings in isolation: `reps` launches captured in one CUDA graph (no host launch cost between them),
-    # replayed after warm-up; inputs in HBM ----
-    side = torch.cuda.Stream(device=dev)
-
-    def time_isolated(fn, reps=20, warm=3, timed=5):
-        with torch.cuda.stream(side):
-            for _ in range(warm):
-                fn()
-        torch.cuda.synchronize()
-        g = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(g, stream=side, capture_error_mode="thread_local"):
-            for _ in range(reps):
-                fn()
-        with torch.cuda.stream(side):
-            g.replay()
-            torch.cuda.synchronize()
-            a, b = ev(), ev()
-            a.record(side)
-            for _ in range(timed):
-                g.replay()
-            b.record(side)
-        torch.cuda.synchronize()
-        return a.elapsed_time(b) / (reps * timed)
-
-    cache = H.make_cache(inp["k_pages"], inp["v_pages"], inp["page_table"], inp["seq_lens"])
-    sel_idx = torch.zeros((units, cap), dtype=torch.int32, device=dev)
-    sel_cnt = torch.zeros((units,), dtype=torch.int32, device=dev)
-    ws_sel = H.alloc_workspace(H.herald_select_workspace_bytes(shape), dev)
-    ws_att = H.alloc_workspace(H.herald_attn_workspace_bytes(shape), dev)
-    act = pipe.active
-    out1 = torch.empty((w.batch, w.block_size, w.n_q_heads, 128), dtype=torch.float32, device=dev)
-    select_alone_ms = time_isolated(lambda: H.herald_select(shape, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, None, ws_sel, side))
-    # the paper's aggregation (softmax-normalised sum over the group; reading 1) beside the north-star one
-    shape_m1 = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, shape.max_seq_len, shape.max_pages_per_seq, cap,
-                            agg_mode=H.AGG_SOFTMAX_SUM)
-    ws_sel_m1 = H.alloc_workspace(H.herald_select_workspace_bytes(shape_m1), dev)
-    select_mode1_alone_ms = time_isolated(lambda: H.herald_select(shape_m1, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, None, ws_sel_m1, side))
-    del ws_sel_m1
-    gather_alone_ms = time_isolated(lambda: H.herald_gather(shape, cache, sel_idx, sel_cnt, pipe.pools_k[0][1 - act], pipe.pools_v[0][1 - act], side))
-    step_i = [0]
-
-    def attn_once():
-        s = step_i[0] % n_steps
-        step_i[0] += 1
-        H.herald_sparse_attn(shape, pipe.pools_k[0][act], pipe.pools_v[0][act], pipe.pool_lens[0][act],
-                             inp["q_blk"][s], inp["k_blk"][s], inp["v_blk"][s], out1, None, ws_att, side)
-    attn_alone_ms = time_isolated(attn_once, reps=n_steps)
-    # scan kernel alone: events around herald_select's scan stage via the profile hook is pipeline-only, so
-    # time select with k=0 (top-k exits immediately): scan + histogram + launch of an empty top-k
-    k_zero = torch.zeros_like(k_per_seq)
-    scan_alone_ms = time_isolated(lambda: H.herald_select(shape, cache, inp["q_rep"], k_zero, sel_idx, sel_cnt, None, ws_sel, side))
-    # NEXT-1 of SURVEY 8(f): a layer that keeps its full KV attends over the paged cache itself
-    dense_attn_ms = time_isolated(lambda: H.herald_dense_attn(shape, cache, inp["q_blk"][0], inp["k_blk"][0], inp["v_blk"][0], out1, None,
-                                                              ws_att, side), reps=4, warm=2, timed=3)
-    # NEXT-2: the representative query's own attention output (second HBM stream, over K and V)
-    rep_out = torch.empty((w.batch, w.n_q_heads, 128), dtype=torch.float32, device=dev)
-    ws_rep = H.alloc_workspace(H.herald_rep_attn_workspace_bytes(shape), dev)
-    rep_attn_ms = time_isolated(lambda: H.herald_rep_attn(shape, cache, inp["q_rep"], rep_out, None, ws_rep, side), reps=4, warm=2, timed=3)
-    # the 2B-token step: denoising group + draft group over the same pools, one launch against two
-    q2 = torch.stack([inp["q_blk"][0], inp["q_blk"][1 % n_steps]]).contiguous()
-    kb2 = torch.stack([inp["k_blk"][0], inp["k_blk"][1 % n_steps]]).contiguous()
-    vb2 = torch.stack([inp["v_blk"][0], inp["v_blk"][1 % n_steps]]).contiguous()
-    out2 = torch.empty((2,) + tuple(out1.shape), dtype=torch.float32, device=dev)
-    ws_att2 = H.alloc_workspace(2 * H.herald_attn_workspace_bytes(shape), dev)
-    attn_2b_ms = time_isolated(lambda: H.herald_sparse_attn_groups(shape, 2, pipe.pools_k[0][pipe.active], pipe.pools_v[0][pipe.active],
-                                                                   pipe.pool_lens[0][pipe.active], q2, kb2, vb2, out2, None, ws_att2, side))
-    del q2, kb2, vb2, out2, ws_att2
-    # the paper's fused retrieval kernel: selection and the representative query's output from ONE pass over K and V
-    ws_fused = H.alloc_workspace(H.herald_select_rep_workspace_bytes(shape), dev)
-    select_rep_fused_ms = time_isolated(lambda: H.herald_select_rep(shape, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, None, rep_out, None,
-                                                                    ws_fused, side), reps=4, warm=2, timed=3)
-    ws_fused_m1 = H.alloc_workspace(H.herald_select_rep_workspace_bytes(shape_m1), dev)
-    select_rep_fused_m1_ms = time_isolated(lambda: H.herald_select_rep(shape_m1, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, None, rep_out, None,
-                                                                       ws_fused_m1, side), reps=4, warm=2, timed=3)
-    del ws_fused, ws_fused_m1
-    # NEXT-4: the selection kernel against the number of queries x (Fig. 8: 32 -> 1 gives 8x on the CPU)
-    xq_sweep = {}
-    for x in (1, 2, 4, 8, 16, 32):
-        if x * w.group > 256:
-            break
-        q_x = synth.make_q_x(inp["q_rep"], x, seed=7000 + x)
-        xq_ms = time_isolated(lambda: H.herald_select_xq(shape, cache, q_x, x, k_per_seq, sel_idx, sel_cnt, None, ws_sel, side), reps=4, warm=2, timed=3)
-        xq_sweep[str(x)] = {"select_ms": xq_ms, "score_tflops": 2 * 128 * x * w.n_q_heads * tokens / (xq_ms * 1e-3) / 1e12}
-        del q_x
-    if xq_sweep:
-        x_max = max(xq_sweep, key=int)
-        for v in xq_sweep.values():
-            v["throughput_vs_x%s" % x_max] = xq_sweep[x_max]["select_ms"] / v["select_ms"]
-    dense_flops = sum(4 * M * (L + w.block_size) * 128 for L in w.seq_lens) * w.n_kv_heads
+    scan_ms, topk_ms, gather_ms = rig.stage_times(8)
+    iso = rig.isolated_stages(cold_attention=True)
+    cache, sel_idx, sel_cnt, ws_sel, ws_att, out1, side = rig.cache, rig.sel_idx, rig.sel_cnt, rig.ws_sel, rig.ws_att, rig.out1, rig.side
+    k_per_seq = rig.k_per_seq
+    select_alone_ms, gather_alone_ms, attn_alone_ms = iso["select_alone_ms"], iso["gather_alone_ms"], iso["attn_step_alone_ms"]
+    next_rows = {}
+    if not args.quick:
+        ti = rig.time_isolated
+        # the paper's aggregation (softmax-normalised sum over the group; reading 1) beside the north-star one
+        shape_m1 = H.make_shape(w.batch, w.n_q_heads, w.n_kv_heads, w.block_size, shape.max_seq_len, shape.max_pages_per_seq, cap,
+                                agg_mode=H.AGG_SOFTMAX_SUM)
+        ws_sel_m1 = H.alloc_workspace(H.herald_select_workspace_bytes(shape_m1), dev)
+        next_rows["select_softmax_sum_mode_alone_ms"] = ti(lambda: H.herald_select(shape_m1, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, None, ws_sel_m1, side)) * n_layers
+        del ws_sel_m1
+        # NEXT-1 of SURVEY 8(f): a layer that keeps its full KV attends over the paged cache itself
+        dense_attn_ms = ti(lambda: H.herald_dense_attn(shape, cache, inp["q_blk"][0], inp["k_blk"][0], inp["v_blk"][0], out1, None, ws_att, side),
+                           reps=4, warm=2, timed=3)
+        dense_flops = sum(4 * w.block_size * w.group * (L + w.block_size) * 128 for L in w.seq_lens) * w.n_kv_heads
+        next_rows["dense_attn_full_cache_ms"] = dense_attn_ms
+        next_rows["dense_attn_tflops"] = dense_flops / (dense_attn_ms * 1e-3) / 1e12
+        # NEXT-2: the representative query's own attention output (second HBM stream, over K and V)
+        rep_out = torch.empty((w.batch, w.n_q_heads, 128), dtype=torch.float32, device=dev)
+        ws_rep = H.alloc_workspace(H.herald_rep_attn_workspace_bytes(shape), dev)
+        rep_attn_ms = ti(lambda: H.herald_rep_attn(shape, cache, inp["q_rep"], rep_out, None, ws_rep, side), reps=4, warm=2, timed=3)
+        next_rows["rep_attn_ms"] = rep_attn_ms
+        next_rows["rep_attn_gbs"] = tokens * w.n_kv_heads * 512 / (rep_attn_ms * 1e-3) / 1e9
+        # the 2B-token step: denoising group + draft group over the same pools, one launch against two
+        q2 = torch.stack([inp["q_blk"][0], inp["q_blk"][1 % n_steps]]).contiguous()
+        kb2 = torch.stack([inp["k_blk"][0], inp["k_blk"][1 % n_steps]]).contiguous()
+        vb2 = torch.stack([inp["v_blk"][0], inp["v_blk"][1 % n_steps]]).contiguous()
+        out2 = torch.empty((2,) + tuple(out1.shape), dtype=torch.float32, device=dev)
+        ws_att2 = H.alloc_workspace(2 * H.herald_attn_workspace_bytes(shape), dev)
+        next_rows["attn_2b_step_one_launch_ms"] = ti(lambda: H.herald_sparse_attn_groups(
+            shape, 2, pipe.pools_k[0][pipe.active], pipe.pools_v[0][pipe.active], pipe.pool_lens[0][pipe.active], q2, kb2, vb2, out2, None, ws_att2, side))
+        del q2, kb2, vb2, out2, ws_att2
+        # the paper's fused retrieval kernel: selection and the representative query's output from ONE pass over K and V
+        ws_fused = H.alloc_workspace(H.herald_select_rep_workspace_bytes(shape), dev)
+        next_rows["select_rep_fused_ms"] = ti(lambda: H.herald_select_rep(shape, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, None, rep_out, None,
+                                                                         ws_fused, side), reps=4, warm=2, timed=3)
+        ws_fused_m1 = H.alloc_workspace(H.herald_select_rep_workspace_bytes(shape_m1), dev)
+        next_rows["select_rep_fused_softmax_sum_mode_ms"] = ti(lambda: H.herald_select_rep(shape_m1, cache, inp["q_rep"], k_per_seq, sel_idx, sel_cnt, None,
+                                                                                         rep_out, None, ws_fused_m1, side), reps=4, warm=2, timed=3)
+        next_rows["select_plus_rep_separate_ms"] = select_alone_ms + rep_attn_ms
+        del ws_fused, ws_fused_m1
+        # NEXT-4: the selection kernel against the number of queries x (Fig. 8: 32 -> 1 gives 8x on the CPU)
+        xq_sweep = {}
+        for x in (1, 2, 4, 8, 16, 32):
+            if x * w.group > 256:
+                break
+            q_x = synth.make_q_x(inp["q_rep"], x, seed=7000 + x)
+            xq_ms = ti(lambda: H.herald_select_xq(shape, cache, q_x, x, k_per_seq, sel_idx, sel_cnt, None, ws_sel, side), reps=4, warm=2, timed=3)
+            xq_sweep[str(x)] = {"select_ms": xq_ms, "score_tflops": 2 * 128 * x * w.n_q_heads * tokens / (xq_ms * 1e-3) / 1e12}
+            del q_x
+        if xq_sweep:
+            x_max = max(xq_sweep, key=int)
+            for v in xq_sweep.values():
+                v["throughput_vs_x%s" % x_max] = xq_sweep[x_max]["select_ms"] / v["select_ms"]
+        next_rows["select_xq_sweep"] = xq_sweep
     denoise_alone_ms = attn_alone_ms * n_steps * n_layers        # stage timings are per layer (layer 0), the block has n_layers
-    select_alone_ms, select_mode1_alone_ms = select_alone_ms * n_layers, select_mode1_alone_ms * n_layers
+    select_alone_block_ms = select_alone_ms * n_layers
     gather_alone_ms_block = gather_alone_ms * n_layers
 
     # ---- end to end through the host-buffer entry point ----
     hosts = []
     for l in range(n_layers):
-        host = {n: inps[l][n].cpu().pin_memory() for n in ("q_rep", "q_blk", "k_blk", "v_blk")}
+        host = {n: rig.inps[l][n].cpu().pin_memory() for n in ("q_rep", "q_blk", "k_blk", "v_blk")}
         host["out"] = torch.empty(pipe.outs[l].shape, dtype=torch.float32).pin_memory()
         hosts.append(host)
     io = pipe.make_host_io(hosts)
@@ -451,7 +643,7 @@ def main():
         pipe.step_host(io)
     torch.cuda.synchronize()
     barrier()
-    a, b = ev(), ev()
+    a, b = rig.ev(), rig.ev()
     a.record(pipe.main_stream)
     for _ in range(e2e_steps):
         pipe.step_host(io)
@@ -459,6 +651,34 @@ def main():
     torch.cuda.synchronize()
     e2e_ms = max_over_ranks(a.elapsed_time(b), dev) / e2e_steps
     e2e_tokens = world * w.batch * w.block_size / (e2e_ms * 1e-3)
+    # the link floor of that step: its larger copy direction at the rate one pinned copy of the same size reaches here
+    big = hosts[0]["out"]
+    dev_big = pipe.outs[0]
+    link = {}
+    for name, src, dst in (("d2h", dev_big, big), ("h2d", big, dev_big)):
+        ca, cb = rig.ev(), rig.ev()
+        with torch.cuda.stream(side):
+            dst.copy_(src, non_blocking=True)
+            ca.record(side)
+            for _ in range(3):
+                dst.copy_(src, non_blocking=True)
+            cb.record(side)
+        torch.cuda.synchronize()
+        link[name + "_gbs"] = 3 * big.numel() * 4 / (ca.elapsed_time(cb) * 1e-3) / 1e9
+    pcie_floor_ms = max(d2h / (link["d2h_gbs"] * 1e9), h2d / (link["h2d_gbs"] * 1e9)) * 1e3
+
+    # ---- the other workloads and the Fig. 14 analogue (N = 1, default run only) ----
+    other, fig14 = None, None
+    if full:
+        scan_ctas_c2 = int(pipe.c.scan_ctas)
+        del hosts, io
+        other = {}
+        for name in ("C1", "C3", "C4@5"):
+            r2 = Rig(H, synth, torch, name, dev, 21633 + 1000 * int(name[1]))
+            other[name] = compact_line(r2, peaks)
+            del r2
+            torch.cuda.empty_cache()
+        fig14 = fig14_sweep(H, synth, torch, dev, SEED, scan_ctas_c2)
 
     # ---- oracle on the host cores (rank 0, N=1 only) ----
     cpu_baseline = None
@@ -472,65 +692,75 @@ def main():
     if rank != 0:
         return 0
 
-    attn_tflops_step = attn_flops / (attn_alone_ms * 1e-3) / 1e12
-    attn_share = denoise_alone_ms / (denoise_alone_ms + select_alone_ms + gather_alone_ms_block)
-    scan_gbs_live = scan_bytes / (scan_ms * 1e-3) / 1e9
-    scan_gbs_alone = scan_bytes / (scan_alone_ms * 1e-3) / 1e9
+    attn_tflops_step = rig.attn_flops / (attn_alone_ms * 1e-3) / 1e12
+    attn_share = denoise_alone_ms / (denoise_alone_ms + select_alone_block_ms + gather_alone_ms_block)
+    scan_gbs_live = rig.scan_bytes / (scan_ms * 1e-3) / 1e9
+    scan_gbs_alone = rig.scan_bytes / (iso["scan_kernel_ms"] * 1e-3) / 1e9
     # attention inside the step: the main stream runs nothing else, so its per-launch time inside the timed
     # region is (step time) / n_steps when the retrieval stream is hidden
     attn_live_ms = ms_step / (n_steps * n_layers)
-    attn_tflops_live = attn_flops / (attn_live_ms * 1e-3) / 1e12
+    attn_tflops_live = rig.attn_flops / (attn_live_ms * 1e-3) / 1e12
     roofline = {"kernel": "attn_tc_kernel", "bound": "tensor", "achieved": attn_tflops_live,
                 "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s", "frac": attn_tflops_live / peaks["bf16_tflops_sustained"],
                 "traffic": NCU_ATTN_DRAM_BYTES.get(w.name),
                 "peak_source": peaks["source"] + " (sustained bf16, kernel timed inside a long step)",
+                "achieved_alone": attn_tflops_step, "frac_alone_of_burst_peak": attn_tflops_step / peaks["bf16_tflops"],
                 "note": f"dominant kernel by time share; achieved = 4*M*(n+B)*128 FLOP per launch / (step time / {n_steps * n_layers} launches); "
                         "traffic = dram__bytes_read+write per launch of the committed ncu capture (profiles/), cold L2"}
     roofline_scan = {"kernel": "scan_pm_kernel", "bound": "hbm", "achieved": scan_gbs_live, "peak": peaks["hbm_gbs"],
                      "unit": "GB/s", "frac": scan_gbs_live / peaks["hbm_gbs"], "traffic": NCU_SCAN_DRAM_BYTES.get(w.name),
                      "achieved_alone": scan_gbs_alone, "frac_alone": scan_gbs_alone / peaks["hbm_gbs"],
                      "pct_of_8TBs_alone": 100.0 * scan_gbs_alone / 8000.0, "peak_source": peaks["source"],
-                     "note": "live = CUDA events on the retrieval stream inside the timed region (shares HBM/SMs with "
-                             "attention); alone = select with k=0 timed in isolation"}
+                     "note": "live = CUDA events on the retrieval stream inside the timed region (shares HBM/SMs with attention); "
+                             "alone = the scan kernel by itself: a captured graph of 20 x (memset, scan, empty top-k) minus the same graph "
+                             "over empty sequences; breakdown.scan_kernel_eager_events_ms is the upper bound from events around the kernel "
+                             "in eager launches"}
+    breakdown = {
+        "block_latency_ms": ms_step, "block_latency_median_ms": statistics.median(regions), "block_latency_min_ms": regions_sorted[0],
+        "timed_regions": len(regions), "steps_per_region": args.steps,
+        "scan_gbs_alone": scan_gbs_alone, "scan_pct_of_8TBs_alone": 100.0 * scan_gbs_alone / 8000.0,
+        "scan_kernel_ms": iso["scan_kernel_ms"], "scan_with_memset_and_empty_topk_ms": iso["scan_with_memset_and_empty_topk_ms"],
+        "scan_kernel_eager_events_ms": iso["scan_kernel_eager_events_ms"], "scan_kernel_eager_events_min_ms": iso["scan_kernel_eager_events_min_ms"],
+        "scan_gbs_eager_events": rig.scan_bytes / (iso["scan_kernel_eager_events_ms"] * 1e-3) / 1e9,
+        "topk_kernel_eager_events_ms": iso["topk_kernel_eager_events_ms"],
+        "scan_gbs_in_pipeline": scan_gbs_live, "scan_ms_in_pipeline": scan_ms, "topk_ms_in_pipeline": topk_ms,
+        "gather_ms_in_pipeline": gather_ms, "select_alone_ms": select_alone_block_ms,
+        "gather_alone_ms": gather_alone_ms, "gather_gbs_alone": rig.gather_bytes / (gather_alone_ms * 1e-3) / 1e9,
+        "attn_step_alone_ms": attn_alone_ms, "attn_tflops_alone": attn_tflops_step,
+        "attn_step_l2_cold_ms": iso.get("attn_step_l2_cold_ms"), "attn_step_l2_cold_min_ms": iso.get("attn_step_l2_cold_min_ms"),
+        "attn_tflops_l2_cold": rig.attn_flops / (iso["attn_step_l2_cold_ms"] * 1e-3) / 1e12 if iso.get("attn_step_l2_cold_ms") else None,
+        "attn_tflops_in_pipeline": attn_tflops_live, "denoise_alone_ms": denoise_alone_ms,
+        "exposed_selection_ms": ms_step - denoise_alone_ms, "exposed_selection_frac": (ms_step - denoise_alone_ms) / ms_step,
+        "overlap_efficiency": (denoise_alone_ms + select_alone_block_ms + gather_alone_ms_block - ms_step) / (select_alone_block_ms + gather_alone_ms_block),
+        "n_layers": n_layers, "n_dense_layers": n_dense, "attn_time_share_alone": attn_share,
+        "algorithmic": {"scan_bytes": rig.scan_bytes, "gather_bytes": rig.gather_bytes, "attn_flops_per_step": rig.attn_flops,
+                        "attn_bytes_per_step": rig.attn_bytes}}
+    breakdown.update(next_rows)
+    if other is not None:
+        breakdown["other_workloads"] = other
+    if fig14 is not None:
+        breakdown["fig14_sweep"] = fig14
     line = {
         "metric": METRIC, "value": tokens_per_s, "unit": "tokens/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": f"{w.name}: {n_layers} layer(s) {w.n_q_heads}/{w.n_kv_heads}/128 heads, batch {w.batch} x "
-                               f"{'ragged ' + str(min(w.seq_lens)) + '..' + str(w.max_seq_len) if len(set(w.seq_lens)) > 1 else w.max_seq_len} "
-                               f"paged (16-token pages), B={w.block_size}, T={w.denoise_steps} ({n_steps} attention steps), "
-                               f"budget {w.permille / 10:g}% k={max(ks)}, structure {w.structure}",
+        "config": {"workload": workload_desc(w, n_layers, ks),
                    "parallelism": "replicas" if world > 1 else "single GPU",
                    "l2": f"K cache {tokens * w.n_kv_heads * 256 / 2**20:.0f} MiB > 126 MB L2 (no flush needed); the active pool "
-                         f"({rows * 512 / 1e6:.0f} MB) is reused by all {n_steps} steps by design",
+                         f"({rig.rows * 512 / 1e6:.0f} MB) is reused by all {n_steps} steps by design (L2-cold attention is reported in breakdown)",
                    "start_after_step": int(pipe.c.start_after_step), "scan_ctas": int(pipe.c.scan_ctas),
                    "scan_head_permille": int(pipe.c.scan_head_permille),
                    "schedule_sweep_ms (scan_ctas/start_after_step/scan_head_permille, untimed calibration by herald_pipeline_tune, eager)": rs_sweep,
                    "attn_grid_ctas": H.herald_attn_grid_ctas(shape),
-                   "launch": "eager" if graphs is None else "one CUDA graph per pool parity, replayed"},
-        "breakdown": {
-            "scan_gbs_alone": scan_gbs_alone, "scan_pct_of_8TBs_alone": 100.0 * scan_gbs_alone / 8000.0,
-            "scan_gbs_in_pipeline": scan_gbs_live, "scan_ms_in_pipeline": scan_ms, "topk_ms_in_pipeline": topk_ms,
-            "gather_ms_in_pipeline": gather_ms, "select_alone_ms": select_alone_ms, "select_softmax_sum_mode_alone_ms": select_mode1_alone_ms,
-            "scan_alone_ms": scan_alone_ms,
-            "gather_alone_ms": gather_alone_ms, "gather_gbs_alone": gather_bytes / (gather_alone_ms * 1e-3) / 1e9,
-            "attn_step_alone_ms": attn_alone_ms, "attn_tflops_alone": attn_tflops_step,
-            "attn_tflops_in_pipeline": attn_tflops_live, "denoise_alone_ms": denoise_alone_ms,
-            "block_latency_ms": ms_step, "exposed_selection_ms": ms_step - denoise_alone_ms,
-            "overlap_efficiency": (denoise_alone_ms + select_alone_ms + gather_alone_ms_block - ms_step) / (select_alone_ms + gather_alone_ms_block),
-            "n_layers": n_layers, "n_dense_layers": n_dense,
-            "rep_attn_ms": rep_attn_ms, "rep_attn_gbs": tokens * w.n_kv_heads * 512 / (rep_attn_ms * 1e-3) / 1e9,
-            "attn_2b_step_one_launch_ms": attn_2b_ms,
-            "select_rep_fused_ms": select_rep_fused_ms, "select_rep_fused_softmax_sum_mode_ms": select_rep_fused_m1_ms, "select_plus_rep_separate_ms": select_alone_ms / n_layers + rep_attn_ms,
-            "select_xq_sweep": xq_sweep,
-            "dense_attn_full_cache_ms": dense_attn_ms, "dense_attn_tflops": dense_flops / (dense_attn_ms * 1e-3) / 1e12,
-            "attn_time_share_alone": attn_share,
-            "algorithmic": {"scan_bytes": scan_bytes, "gather_bytes": gather_bytes, "attn_flops_per_step": attn_flops,
-                            "attn_bytes_per_step": attn_bytes}},
+                   "launch": "eager" if rig.graphs is None else "one CUDA graph per pool parity, replayed"},
+        "breakdown": breakdown,
         "roofline": roofline, "roofline_scan": roofline_scan,
         "cpu_baseline": cpu_baseline,
-        "e2e": {"value": e2e_tokens, "unit": "tokens/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-        "gpu_launches": args.steps * ((n_layers - n_dense) * (3 + n_steps) + n_dense * n_steps),   # per block step: scan, top-k, gather, T-1 x attention (timed region only)
+        "e2e": {"value": e2e_tokens, "unit": "tokens/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "pcie_floor_ms": pcie_floor_ms, "link_gbs_measured": link,
+                "note": "uploads on the main stream, downloads on the retrieval stream (full duplex); the floor is the larger direction at the "
+                        "rate one pinned copy of the output tensor reaches on this box"},
+        "gpu_launches": args.steps * ((n_layers - n_dense) * (3 + n_steps + (1 if int(pipe.c.scan_head_permille) > 0 else 0)) + n_dense * n_steps),   # per block step: scan (two launches with a head start), top-k, gather, T-1 x attention (first timed region only)
         "clocks": clock_info,
     }
     print(json.dumps(line))

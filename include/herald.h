@@ -300,7 +300,8 @@ int herald_pipeline_tune(herald_pipeline_t* pipe, int32_t reps, herald_schedule_
 
 /* Optional timing hooks for the retrieval stream (measurement only, no effect on results): caller-created
  * events recorded on the retrieval stream around the stages of the LAST layer's selection inside
- * herald_pipeline_step.  Any member may be NULL.  scan = score scan (+ aggregation in mode 1),
+ * herald_pipeline_step; a plain herald_select records scan_begin / scan_end / topk_end on its own stream as well
+ * (this is how bench.py times the scan kernel by itself).  Any member may be NULL.  scan = score scan (+ aggregation in mode 1),
  * topk = radix select, gather = pool fill.  Pass NULL to herald_pipeline_set_profile to switch off. */
 typedef struct herald_profile {
     herald_event_t scan_begin, scan_end, topk_end, gather_end;

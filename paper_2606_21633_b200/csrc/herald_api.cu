@@ -21,7 +21,8 @@ namespace herald {
 
 static thread_local char g_err[512] = "";
 static thread_local const herald_profile_t* g_prof = nullptr;   // timing hooks (herald_pipeline_set_profile)
-static thread_local bool g_prof_armed = false;
+static thread_local bool g_prof_armed = false;                    // inside a pipeline step: only the last sparse layer is timed
+static thread_local bool g_in_pipeline = false;
 static thread_local uint32_t g_delay_main_us = 0, g_delay_retrieval_us = 0;   // test hook (herald_pipeline_set_debug_delay)
 #ifdef HERALD_ATTN_TRACE
 static unsigned long long* g_attn_trace = nullptr;               // debug builds only: device buffer [CTAs][64]
@@ -457,7 +458,7 @@ static int select_impl(const herald_shape_t* shape, const herald_cache_t* cache,
         e = cudaMemsetAsync(hist1, 0, (size_t)units * kBins1 * sizeof(uint32_t), stream);
         if (e != cudaSuccess) return cuda_fail(e, "memset hist1");
     }
-    const herald_profile_t* prof = g_prof_armed ? g_prof : nullptr;
+    const herald_profile_t* prof = (g_prof_armed || !g_in_pipeline) ? g_prof : nullptr;   // a plain herald_select is timed too
     if (prof && prof->scan_begin && phase != kSelectTail) cudaEventRecord(static_cast<cudaEvent_t>(prof->scan_begin), stream);
 
     if (shape->max_seq_len > 0) {
@@ -1052,6 +1053,7 @@ int herald_pipeline_step(herald_pipeline_t* p) {
             herald_layer_t* ly = &p->layers[l];
             if (ly->dense) continue;                      // keeps its full KV: nothing to select
             g_prof_armed = (l == last_sparse);
+            g_in_pipeline = true;
             g_scan_ctas = scan_ctas;
             int r;
             if (head > 0 && !head_pending) {
@@ -1072,6 +1074,7 @@ int herald_pipeline_step(herald_pipeline_t* p) {
                                   p->ws_select, p->ws_select_bytes, s_ret);
             }
             g_prof_armed = false;
+            g_in_pipeline = false;
             g_scan_ctas = 0;
             if (r) return r;
             r = herald_gather(sh, &ly->cache, p->sel_idx, ly->pool_len[idle], ly->pool_k[idle], ly->pool_v[idle], s_ret);
