@@ -90,6 +90,9 @@ typedef struct herald_cache {
 #define HERALD_XQ_AUTO 0
 #define HERALD_XQ_MMA_SYNC 1
 #define HERALD_XQ_TCGEN05 2
+#define HERALD_ATTN_AUTO 0
+#define HERALD_ATTN_EXACT 1
+#define HERALD_ATTN_FAST_FIRST 2
 typedef struct herald_tuning {
     int32_t attn_splits;     /* KV splits (= cluster size) of the attention grid, 1..8                                   */
     int32_t attn_m_tiles;    /* M tiles per (sequence, KV head); only values above the minimum ceil(B*G/128) are honoured */
@@ -98,6 +101,9 @@ typedef struct herald_tuning {
     int32_t scan_ctas;       /* grid of every score scan (overrides herald_pipeline_t.scan_ctas)                          */
     int32_t scan_head_major; /* non-zero: the head-major scan even where the page-major one applies                       */
     int32_t xq_path;         /* herald_select_xq: HERALD_XQ_AUTO / _MMA_SYNC / _TCGEN05                                    */
+    int32_t attn_precision;  /* HERALD_ATTN_AUTO: attention blocks with a long share of the keys try the single-bf16 pass first
+                                (verified against the finished row statistics, redone exactly if they fail);
+                                _EXACT: bf16 hi+lo weights everywhere; _FAST_FIRST: every block tries the fast pass first       */
 } herald_tuning_t;
 int herald_set_tuning(const herald_tuning_t* tuning);
 
@@ -162,8 +168,12 @@ int herald_gather(const herald_shape_t* shape, const herald_cache_t* cache, cons
  *   pool_k/pool_v bf16 [batch][H_kv][pool_capacity][128] (the ACTIVE buffer); pool_len int32 [batch][H_kv]
  *   q_blk bf16 [batch][B][H_q][128]; k_blk, v_blk bf16 [batch][B][H_kv][128]
  *   out fp32 [batch][B][H_q][128]; lse optional fp32 [batch][B][H_q] = log sum_j exp(logit_j).
- *   ws >= herald_attn_workspace_bytes(shape), 256-byte aligned.  bf16 tensor-core products, fp32
- *   softmax and accumulation; softmax weights are rounded to bf16 for the PV product. */
+ *   ws >= herald_attn_workspace_bytes(shape), 256-byte aligned.  bf16 tensor-core products, fp32 softmax and accumulation.
+ *   The softmax weights enter the PV product as a bf16 pair hi + lo (2^-17 relative).  A thread block whose share of the
+ *   keys is long (>= 1536) first tries a single bf16 per weight, accepts the result only if every one of its rows has
+ *   sum_i p_i^2 <= 1/64 on the FINISHED row (then the rounding moves an output by ~1e-4 |v|), and otherwise redoes its tiles
+ *   exactly.  The workspace keeps one note per block from launch to launch ("failed: start exact");
+ *   its content never changes a result, so it needs no initialisation. */
 int herald_sparse_attn(const herald_shape_t* shape, const void* pool_k, const void* pool_v,
                        const int32_t* pool_len, const void* q_blk, const void* k_blk, const void* v_blk,
                        float* out, float* lse, void* ws, size_t ws_bytes, herald_stream_t stream);

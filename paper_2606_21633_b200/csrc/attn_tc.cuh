@@ -31,6 +31,20 @@
 //             accumulates the row sum, and writes P back over S_j in TMEM (tcgen05.st).  The running maximum
 //             is only raised when it grows by more than 2^kTcRescaleThreshold ("lazy rescale"; P, l and O are
 //             fp32/bf16-ranged, so the threshold only guards overflow): O in TMEM is then rescaled in place.
+//   precision modes.  EXACT: as above (P = bf16 hi + lo, the row maximum exchanged at every tile, O rescaled in place when
+//             it moves by more than 2^40).  FAST, tried first by blocks whose share of the keys is >= 1536 long: P is ONE bf16
+//             (8 PV MMAs per tile instead of 16; the TMEM-operand MMAs are the slower kind) and the row keeps the reference of
+//             its first tile without another exchange (any logit up to 2^100 above it is still far inside fp32), so the softmax
+//             warps run free of each other.  Because they no longer meet, a thread may only overwrite S columns it has read
+//             itself: P_hi goes to the first 16 of its own 32 S columns.
+//             Rounding a weight to 8 significant bits moves an output element by sum_i eps_i p_i v_i with |eps_i| <= 2^-8,
+//             pseudo-random: standard deviation <= 2^-8 sqrt(sum_i p_i^2) rms(v) / sqrt(3).  The fast pass accumulates
+//             sum_i e_i^2 per row next to the row sum and is ACCEPTED only if every row of the block has sum_i p_i^2 <= 1/64
+//             (<= 2.8e-4 rms(v) per element, 7 sigma inside the 2e-3 bar; one key alone may then weigh at most 1/8; flat rows
+//             over n keys have sum p^2 ~ e/n) and no logit rose past the 2^100 margin.  Otherwise the block goes through its
+//             tiles once more the exact way (a block-wide vote, taken while the last PV is still running) and leaves a note
+//             in the workspace that makes it start exact for its next 16 launches.  Blocks with short key shares never try:
+//             among a few hundred keys a 5-sigma logit already breaks the criterion, and one redone block delays its launch.
 //   merge     split-KV partials never leave the chip: tile row r is owned by CTA r / rows_own of the cluster; the
 //             other CTAs write their unnormalised O rows and (max, sum) straight from registers into the owner's
 //             shared memory (st.shared::cluster into the owner's K ring, which its last QK^T has released: every CTA
@@ -64,6 +78,12 @@ constexpr int kTcSmemBytes = kTcSmemMisc + kTcMiscBytes;                 // 231,
 constexpr int kTcTmemCols = 512;                 // S0/P0 [0,128) S1/P1 [128,256) S2/P2 [256,384) O [384,512)
 constexpr int kTcTmemO = kTcSBufs * 128;
 constexpr float kTcRescaleThreshold = 40.f;      // log2 units
+// fast pass ("precision modes" in the header comment)
+constexpr int kTcFastMinKeys = 1536;             // a block tries the fast pass only if its share of the keys is at least this long
+constexpr float kTcFastJump = 100.f;             // log2 units a logit may rise above the first tile's row maximum (P, l, O stay far inside fp32)
+constexpr float kTcFastCmax = 1.f / 64.f;        // bound on sum_i p_i^2 of a row for single-bf16 weights
+constexpr uint32_t kTcHintMagic = 0x45580000u;   // note word of a block: "EX" | failures in a row << 8 | launches still to start exact
+constexpr uint32_t kTcHintBackoff = 16;          // after two failed fast passes in a row a block starts exact for this many launches
 // merge buffers: received partial rows alias the K ring, the output staging rows alias the V ring (both dead once
 // every CTA of the cluster has left its main loop)
 constexpr int kTcRowFloats = kHeadDim + 4;       // 528-byte rows: 16-byte accesses of 8 consecutive rows hit 8 bank groups
@@ -99,13 +119,15 @@ struct AttnParams {
     int32_t ipt;        // block rows per M tile (ipt * G <= 128)
     int32_t pool_box;   // rows of the pool tensor-map box: min(cap, 128)
     float scale_log2;   // sm_scale * log2(e)
+    uint32_t* mode_hint; // [blocks of the grid] in the workspace, or NULL: see kTcHintExact
+    int32_t precision;   // 0 = automatic, 1 = exact only, 2 = every block tries the fast pass first (herald_tuning_t.attn_precision)
 #ifdef HERALD_ATTN_TRACE
     unsigned long long* trace;   // [CTAs][64] clock64 stamps (debug builds only)
 #endif
 };
 
 #ifdef HERALD_ATTN_TRACE
-#define HERALD_STAMP(slot) do { if (p.trace && (slot) < 64) p.trace[(((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * 64 + (slot)] = clock64(); } while (0)
+#define HERALD_STAMP(slot) do { if (p.trace && (slot) < 56) p.trace[(((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * 64 + (slot)] = clock64(); } while (0)
 #define HERALD_GSTAMP(slot) do { if (p.trace) { unsigned long long gt_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_)); p.trace[(((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * 64 + (slot)] = gt_; } } while (0)
 #else
 #define HERALD_GSTAMP(slot) do { } while (0)
@@ -296,6 +318,10 @@ __device__ __forceinline__ void ffma2v(float& d0, float& d1, float a0, float a1,
     asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %4};\n\tmov.b64 rc, {%5, %6};\n\t"
         "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}" : "=f"(d0), "=f"(d1) : "f"(a0), "f"(a1), "f"(b), "f"(c0), "f"(c1));
 }
+__device__ __forceinline__ void ffma2w(float& d0, float& d1, float a0, float a1, float b0, float b1, float c0, float c1) {   // d = a * b + c
+    asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tmov.b64 rc, {%6, %7};\n\t"
+        "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}" : "=f"(d0), "=f"(d1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1), "f"(c0), "f"(c1));
+}
 __device__ __forceinline__ void fadd2(float& d0, float& d1, float a0, float a1, float b0, float b1) {   // d = a + b
     asm("{\n\t.reg .b64 ra, rb, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\t"
         "add.rn.f32x2 rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}" : "=f"(d0), "=f"(d1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
@@ -314,6 +340,10 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* v) {
           "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]), "r"(taddr) : "memory");
 }
 
+// kTryFast = false: the exact pass only (every register of the softmax warps is spoken for: the block-uniform state of the
+// two-pass control costs the exact loop ~9 % when it is compiled in).  The launcher picks the instantiation from the
+// longest key share a block of the grid can have.
+template <bool kTryFast>
 __global__ void __launch_bounds__(kTcThreads, 1)
 attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
                const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_kb,
@@ -420,8 +450,28 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     const int row = quarter * 32 + lane;
     const uint32_t lane_base = tmem + ((uint32_t)(quarter * 32) << 16);
     float m_used = -INFINITY, l_run = 0.f;   // running max (log2 units) and the sum of this thread's quarter row
+    float q_run = 0.f;                       // fast pass: the sum of the squared weights of this thread's quarter row
+    bool jumped = false;                     // fast pass: this thread's rows fail its criteria
 
-    if (nt > 0) {
+    // One pass over the key tiles, or two (header comment, "precision modes"): blocks with a long share of the keys try the
+    // fast pass first; if its row statistics fail, every role goes through the same tiles once more the exact way.  Ring and
+    // TMEM barrier phases simply run on: tile j of the second pass is pipeline step jb + j.
+    int keys_here = 0;
+    if (kTryFast)
+        for (int j = 0; j < nt; ++j) keys_here += tile_valid(j);
+    const int cta_lin = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+    bool fast = false;                       // block-uniform
+    uint32_t hint = 0;
+    if (kTryFast && nt > 0 && p.precision != 1 && (p.precision == 2 || keys_here >= kTcFastMinKeys)) {
+        hint = p.mode_hint ? p.mode_hint[cta_lin] : 0u;
+        if ((hint & 0xffff0000u) != kTcHintMagic || (hint & 0xffu) > kTcHintBackoff) hint = kTcHintMagic;   // uninitialised workspace: no history
+        fast = p.precision == 2 || (hint & 0xffu) == 0;
+    }
+    const bool tried_fast = fast;
+    int n_fixed = 0;                         // V tiles whose tail rows were zeroed so far (phase of kBarVTail; V producer)
+    int jb_rt = 0;
+#define HERALD_JB (kTryFast ? jb_rt : 0)
+    for (int pass = 0; nt > 0; ++pass) {
         if (warp == kTcKWarp || warp == kTcVWarp) {
             // =========================== producers: one warp streams K tiles (and Q), one streams V tiles ===========================
             const bool is_k = warp == kTcKWarp;
@@ -430,7 +480,6 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
             const int bar_full = is_k ? kBarKFull : kBarVFull, bar_empty = is_k ? kBarKEmpty : kBarVEmpty;
             const uint32_t ring = sbase + (is_k ? kTcSmemK : kTcSmemV);
             uint8_t* ring_gen = sgen + (is_k ? kTcSmemK : kTcSmemV);
-            int n_fixed = 0;                                  // V tiles whose tail rows were zeroed so far (phase of kBarVTail)
             // dense mode: the page ids of a tile are fetched one tile ahead, so that their round trip does not sit between a
             // ring slot falling free and its TMA requests
             auto tile_phys = [&](int jj) -> int {
@@ -441,11 +490,11 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
             };
             int phys_next = tile_phys(0);
             for (int j = 0; j < nt; ++j) {
-                const int stage = j % kTcStages, t = t0 + j;
+                const int jg = HERALD_JB + j, stage = jg % kTcStages, t = t0 + j;
                 const int my_phys = phys_next;
                 phys_next = tile_phys(j + 1);
-                if (j >= kTcStages) mbar_wait(bar(bar_empty + stage), ((j / kTcStages) - 1) & 1);
-                if (!is_k && j == 0) named_bar_sync(9, 64);   // Q and K_0 are requested before any V tile
+                if (jg >= kTcStages) mbar_wait(bar(bar_empty + stage), ((jg / kTcStages) - 1) & 1);
+                if (!is_k && jg == 0) named_bar_sync(9, 64);   // Q and K_0 are requested before any V tile
                 const uint32_t dst = ring + stage * kTcTileBytes, full = bar(bar_full + stage);
                 const int valid = tile_valid(j), cols = (valid + 15) & ~15;
                 const bool fix = !is_k && cols != valid;      // V rows [valid, cols) must be zeros: land on kBarVTail first
@@ -474,7 +523,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                     }
                     __syncwarp();
                 }
-                if (is_k && j == 0) named_bar_sync(9, 64);
+                if (is_k && jg == 0) named_bar_sync(9, 64);
                 if (fix) {
                     mbar_wait(bar(kBarVTail), n_fixed & 1);
                     ++n_fixed;
@@ -493,10 +542,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
             constexpr uint32_t hi_k = umma_desc_hi(1024);
             const uint32_t q_lo = umma_desc_lo(sbase + kTcSmemQ, 16);
             auto issue_qk = [&](int j) {   // S_j = Q K_j^T into S buffer j % 3 (it held P_{j-3}: PV_{j-3} was issued before, the pipe runs in order)
-                const int stage = j % kTcStages, sb = j % kTcSBufs;
-                mbar_wait(bar(kBarKFull + stage), (j / kTcStages) & 1);
+                const int jg = HERALD_JB + j, stage = jg % kTcStages, sb = jg % kTcSBufs;
+                mbar_wait(bar(kBarKFull + stage), (jg / kTcStages) & 1);
                 tc_fence_after();
-                if (lane == 0) { HERALD_STAMP(8 + 4 * j); if (j == 0) HERALD_GSTAMP(58); }
+                if (lane == 0) { HERALD_STAMP(8 + 4 * jg); if (jg == 0) HERALD_GSTAMP(58); }
                 if (elect_one()) {
                     const uint32_t k_lo = umma_desc_lo(sbase + kTcSmemK + stage * kTcTileBytes, 16);
                     const uint32_t idesc_s = umma_idesc(1, 1, 0, 0, kTcBM, tile_cols(j));
@@ -509,21 +558,24 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                     }
                     umma_commit(bar(kBarSFull + sb));
                     umma_commit(bar(kBarKEmpty + stage));
-                    if (j == nt - 1) umma_commit(bar(kBarQkDone));   // the K ring is dead from here on (merge receive buffer)
+                    if (j == nt - 1) umma_commit(bar(kBarQkDone));   // every QK^T of this pass has read its K tile (phase = pass)
                 }
                 __syncwarp();
             };
             auto issue_pv = [&](int j) {   // O (+)= (P_hi + P_lo)_j V_j, P read from TMEM (it overlays S_j)
-                const int stage = j % kTcStages, sb = j % kTcSBufs;
-                mbar_wait(bar(kBarVFull + stage), (j / kTcStages) & 1);
-                mbar_wait(bar(kBarPFull + sb), (j / kTcSBufs) & 1);
+                const int jg = HERALD_JB + j, stage = jg % kTcStages, sb = jg % kTcSBufs;
+                mbar_wait(bar(kBarVFull + stage), (jg / kTcStages) & 1);
+                mbar_wait(bar(kBarPFull + sb), (jg / kTcSBufs) & 1);
                 tc_fence_after();
-                if (lane == 0) HERALD_STAMP(8 + 4 * j + 3);
+                if (lane == 0) HERALD_STAMP(8 + 4 * jg + 3);
                 if (elect_one()) {
                     const uint32_t v_lo = umma_desc_lo(sbase + kTcSmemV + stage * kTcTileBytes, kTcHalfBytes);
                     const uint32_t p_base = tmem + sb * 128, o_base = tmem + kTcTmemO;
                     const int ksteps = tile_cols(j) >> 4;
-                    if (ksteps == 8) {
+                    if (kTryFast && fast) {     // one bf16 per weight, at the head of each column quarter's own S columns
+                        for (int kk = 0; kk < ksteps; ++kk)
+                            umma_ts(o_base, p_base + (kk >> 1) * 32 + (kk & 1) * 8, v_lo + kk * 128, hi_k, idesc_pv, (j > 0 || kk > 0) ? 1u : 0u);
+                    } else if (ksteps == 8) {
 #pragma unroll
                         for (int kk = 0; kk < 8; ++kk) {
                             umma_ts(o_base, p_base + kk * 8, v_lo + kk * 128, hi_k, idesc_pv, (j > 0 || kk > 0) ? 1u : 0u);
@@ -542,20 +594,84 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 }
                 __syncwarp();
             };
-            mbar_wait(bar(kBarQFull), 0);
-            if (lane == 0) HERALD_GSTAMP(57);
+            if (pass == 0) {
+                mbar_wait(bar(kBarQFull), 0);
+                if (lane == 0) HERALD_GSTAMP(57);
+            }
 #pragma unroll 1
             for (int j = -2; j < nt; ++j) {   // QK^T runs two tiles ahead of PV
                 if (j + 2 < nt) issue_qk(j + 2);
                 if (j >= 0) issue_pv(j);
             }
-        } else {
-            // =========================== softmax warps ===========================
+        } else if (kTryFast && fast) {
+            // =========================== softmax warps, fast pass ===========================
+            m_used = -INFINITY, l_run = 0.f, q_run = 0.f, jumped = false;
             for (int j = 0; j < nt; ++j) {
-                const int sb = j % kTcSBufs, eb = j & 1;
-                mbar_wait(bar(kBarSFull + sb), (j / kTcSBufs) & 1);
+                const int jg = HERALD_JB + j, sb = jg % kTcSBufs;
+                mbar_wait(bar(kBarSFull + sb), (jg / kTcSBufs) & 1);
                 tc_fence_after();
-                if (tid == 0) { HERALD_STAMP(8 + 4 * j + 1); if (j == 0) HERALD_GSTAMP(62); }
+                if (tid == 0) { HERALD_STAMP(8 + 4 * jg + 1); if (jg == 0) HERALD_GSTAMP(62); }
+                float s[32];
+                tmem_ld32_async(lane_base + sb * 128 + cq * 32, s);
+                tmem_wait_ld();
+                const int valid = tile_valid(j);
+                if (valid < kTcBN) {
+#pragma unroll
+                    for (int i = 0; i < 32; ++i)
+                        if (cq * 32 + i >= valid) s[i] = -INFINITY;
+                }
+                float mx = fmax3(s[0], s[1], s[2]);
+#pragma unroll
+                for (int i = 3; i + 1 < 32; i += 2) mx = fmax3(mx, s[i], s[i + 1]);
+                mx = fmaxf(mx, s[31]);
+                if (j == 0) {   // the row reference: the maximum of the first tile, common to the four column quarters
+                    ex_max[cq * 128 + row] = __float2bfloat16_ru(mx);
+                    named_bar_sync(1 + quarter, 128);
+                    float mrow = __bfloat162float(ex_max[row]);
+#pragma unroll
+                    for (int c = 1; c < 4; ++c) mrow = fmaxf(mrow, __bfloat162float(ex_max[c * 128 + row]));
+                    m_used = mrow * p.scale_log2;
+                } else if (mx * p.scale_log2 > m_used + kTcFastJump) {
+                    jumped = true;        // the reference cannot move without the other quarters: the block goes through its tiles again
+                }
+                float sum0 = 0.f, sum1 = 0.f, sq0 = 0.f, sq1 = 0.f;
+                uint32_t hi[16];
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    float x0, x1;
+                    ffma2(x0, x1, s[2 * i], s[2 * i + 1], p.scale_log2, -m_used);
+                    const float e0 = fast_exp2(x0), e1 = fast_exp2(x1);
+                    fadd2(sum0, sum1, sum0, sum1, e0, e1);
+                    ffma2w(sq0, sq1, e0, e1, e0, e1, sq0, sq1);
+                    hi[i] = pack_bf16(e0, e1);
+                }
+                l_run += sum0 + sum1;
+                q_run += sq0 + sq1;
+                tmem_st16(lane_base + sb * 128 + cq * 32, hi);     // over the first 16 of this thread's own 32 S columns
+                tmem_wait_st();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(kBarPFull + sb));
+                if (tid == 0) HERALD_STAMP(8 + 4 * jg + 2);
+            }
+            // the verdict (the last PV is still running): row sums of e and e^2 over the four column quarters
+            ex_sum[cq * 128 + row] = l_run;
+            named_bar_sync(1 + quarter, 128);
+            const float l_row = (ex_sum[row] + ex_sum[128 + row]) + (ex_sum[256 + row] + ex_sum[384 + row]);
+            named_bar_sync(1 + quarter, 128);
+            ex_sum[cq * 128 + row] = q_run;
+            named_bar_sync(1 + quarter, 128);
+            const float q_row = (ex_sum[row] + ex_sum[128 + row]) + (ex_sum[256 + row] + ex_sum[384 + row]);
+            named_bar_sync(1 + quarter, 128);      // (the exact pass and the merge reuse this buffer)
+            if (!(q_row <= kTcFastCmax * l_row * l_row)) jumped = true;
+        } else {
+            // =========================== softmax warps, exact pass ===========================
+            m_used = -INFINITY, l_run = 0.f;
+            for (int j = 0; j < nt; ++j) {
+                const int jg = HERALD_JB + j, sb = jg % kTcSBufs, eb = jg & 1;
+                mbar_wait(bar(kBarSFull + sb), (jg / kTcSBufs) & 1);
+                tc_fence_after();
+                if (tid == 0) { HERALD_STAMP(8 + 4 * jg + 1); if (jg == 0) HERALD_GSTAMP(62); }
                 float s[32];
                 tmem_ld32_async(lane_base + sb * 128 + cq * 32, s);
                 tmem_wait_ld();
@@ -607,7 +723,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 }
                 l_run = l_run * alpha + (sum0 + sum1);
                 if (any) {   // rare: the running maximum of some row grew past the threshold -> rescale O in place
-                    mbar_wait(bar(kBarPvDone + ((j - 1) % kTcSBufs)), ((j - 1) / kTcSBufs) & 1);   // PV_{j-1} finished; PV_j waits for our arrive
+                    mbar_wait(bar(kBarPvDone + ((jg - 1) % kTcSBufs)), ((jg - 1) / kTcSBufs) & 1);   // PV_{j-1} finished; PV_j waits for our arrive
                     tc_fence_after();
                     float o[32];
                     tmem_ld32_async(lane_base + kTcTmemO + cq * 32, o);
@@ -626,14 +742,39 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar(kBarPFull + sb));
-                if (tid == 0) HERALD_STAMP(8 + 4 * j + 2);
+                if (tid == 0) HERALD_STAMP(8 + 4 * jg + 2);
             }
-            // A parity wait is only sound when the waiter is at most one phase behind: slot (nt-1) % 3 completes next for
-            // PV_{nt+2}, which does not exist.
-            mbar_wait(bar(kBarPvDone + ((nt - 1) % kTcSBufs)), ((nt - 1) / kTcSBufs) & 1);
-            tc_fence_after();
-            if (tid == 0) HERALD_STAMP(2);
         }
+        // ---- end of a fast pass: one block-wide vote (every warp is here shortly after the last P was handed over) ----
+        if (kTryFast && fast) {
+            fast = false;
+            if (__syncthreads_or(warp < kTcSoftmaxWarps && jumped ? 1 : 0)) {
+                jb_rt += nt;
+                continue;         // once more, the exact way: the first PV of the pass overwrites O
+            }
+        }
+        break;
+    }
+    const int n_passes = (kTryFast && jb_rt > 0) ? 2 : 1;
+    if (kTryFast && tid == 0 && p.mode_hint && nt > 0) {
+        // the note for this block's next launch.  One failed fast pass costs one redo and nothing more (on N(0,1)-like data a
+        // row with a 6-sigma logit turns up in some block now and then, and a block that starts exact holds up its whole
+        // launch); two in a row mean the data is peaked: exact for kTcHintBackoff launches, then one more try.
+        if (tried_fast) {
+            const uint32_t streak = n_passes == 2 ? min(((hint >> 8) & 0xffu) + 1u, 255u) : 0u;
+            p.mode_hint[cta_lin] = kTcHintMagic | (streak << 8) | (streak >= 2 ? kTcHintBackoff : 0u);
+        } else if (hint != 0 && (hint & 0xffu) != 0) {
+            p.mode_hint[cta_lin] = hint - 1;
+        }
+    }
+    if (warp < kTcSoftmaxWarps && nt > 0) {
+        // A parity wait is only sound when the waiter is at most one phase behind: the slot of the last PV completes next
+        // for a PV three pipeline steps later, which does not exist.
+        const int jl = HERALD_JB + nt - 1;
+#undef HERALD_JB
+        mbar_wait(bar(kBarPvDone + (jl % kTcSBufs)), (jl / kTcSBufs) & 1);
+        tc_fence_after();
+        if (tid == 0) HERALD_STAMP(2);
     }
 
     // ---- merge of the split-KV partials inside the cluster, normalisation, output -----------------------
@@ -642,7 +783,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     // this happens about a tile period before any partial exists, so no sender ever waits for it in practice.
     if (warp == kTcKWarp && nt == 0) mbar_wait(bar(kBarQFull), 0);   // the Q box was requested: it must have landed before the CTA exits
     if (warp == kTcKWarp && S > 1) {
-        if (nt > 0) mbar_wait(bar(kBarQkDone), 0);
+        if (nt > 0) mbar_wait(bar(kBarQkDone), (n_passes - 1) & 1);   // the last pass has read its last K tile
         cluster_wait_all();   // every CTA of the cluster has initialised its barriers (only this warp arrives on a peer's before it is told to)
         if (lane < S - 1) mbar_arrive_remote(map_to_cta(bar(kBarPeerReady), lane < split ? lane : lane + 1));
     }

@@ -44,7 +44,7 @@ static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 // launch-geometry overrides of this thread (herald_set_tuning); all zero = automatic
-static thread_local herald_tuning_t g_tune = {0, 0, 0, 0, 0, 0, 0};
+static thread_local herald_tuning_t g_tune = {0, 0, 0, 0, 0, 0, 0, 0};
 
 static int check_shape(const herald_shape_t* s) {
     if (!s) return fail(HERALD_ERR_INVALID_ARG, "shape is NULL");
@@ -159,7 +159,7 @@ static SelectWs select_ws_layout(const herald_shape_t* s) {
 // ---- attention launch geometry ----------------------------------------------------------------
 struct AttnGeom {
     int m_tiles, ipt, n_splits;
-    size_t total;
+    size_t hint_off, total;
 };
 
 static AttnGeom attn_geom(const herald_shape_t* s, bool dense = false) {
@@ -183,8 +183,10 @@ static AttnGeom attn_geom(const herald_shape_t* s, bool dense = false) {
     if (splits > kTcMaxSplits) splits = kTcMaxSplits;
     if (splits < 1) splits = 1;
     a.n_splits = splits;
-    // split-KV partials are merged on chip (DSMEM); the workspace only holds the longest-first unit order of a layer
-    a.total = align_up((size_t)(units > 0 ? units : 1) * sizeof(int32_t), 256);
+    // split-KV partials are merged on chip (DSMEM); the workspace holds the longest-first unit order of a layer and one
+    // precision note per block of the largest grid the shape can get (attn_tc.cuh, "precision modes")
+    a.hint_off = align_up((size_t)(units > 0 ? units : 1) * sizeof(int32_t), 256);
+    a.total = a.hint_off + align_up((size_t)(units > 0 ? units : 1) * 4 * kTcMaxSplits * sizeof(int32_t), 256);
     return a;
 }
 
@@ -673,9 +675,10 @@ static int sparse_attn_impl(const herald_shape_t* shape, const void* pool_k, con
     g_err[0] = 0;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
 
-    static bool attn_attr[kMaxDevices] = {false};
+    static bool attn_attr[kMaxDevices] = {false}, attn_fast_attr[kMaxDevices] = {false};
     {
-        const cudaError_t e = ensure_smem(attn_tc_kernel, kTcSmemBytes, attn_attr);
+        cudaError_t e = ensure_smem(attn_tc_kernel<false>, kTcSmemBytes, attn_attr);
+        if (e == cudaSuccess) e = ensure_smem(attn_tc_kernel<true>, kTcSmemBytes, attn_fast_attr);
         if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(attn)");
     }
     CUtensorMap tm_k, tm_v, tm_q, tm_kb, tm_vb;
@@ -707,6 +710,9 @@ static int sparse_attn_impl(const herald_shape_t* shape, const void* pool_k, con
     ap.ipt = a.ipt;
     ap.pool_box = shape->pool_capacity < kTcBN ? (shape->pool_capacity > 0 ? shape->pool_capacity : 1) : kTcBN;
     ap.scale_log2 = shape->sm_scale * 1.4426950408889634f;
+    ap.mode_hint = (size_t)a.n_splits * a.m_tiles * units * sizeof(int32_t) <= a.total - a.hint_off
+                       ? reinterpret_cast<uint32_t*>(static_cast<uint8_t*>(ws) + a.hint_off) : nullptr;
+    ap.precision = g_tune.attn_precision;
 #ifdef HERALD_ATTN_TRACE
     ap.trace = g_attn_trace;
 #endif
@@ -734,7 +740,14 @@ static int sparse_attn_impl(const herald_shape_t* shape, const void* pool_k, con
     }
     cfg.attrs = attr;
     cfg.numAttrs = n_attr;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, attn_tc_kernel, tm_k, tm_v, tm_q, tm_kb, tm_vb, ap);
+    // the instantiation with the fast first pass only where some block can have a key share long enough to try it
+    const int max_keys = (dense ? shape->max_seq_len : shape->pool_capacity) + shape->block_size;
+    // (and only for shapes whose step is bound by the tensor pipe / softmax issue: an M tile of 64 rows streams its pool at the HBM rate)
+    const bool try_fast = g_tune.attn_precision == HERALD_ATTN_FAST_FIRST ||
+                          (g_tune.attn_precision == HERALD_ATTN_AUTO && a.ipt * (shape->n_q_heads / shape->n_kv_heads) >= 96 &&
+                           (max_keys + a.n_splits - 1) / a.n_splits + kTcBN >= kTcFastMinKeys);
+    cudaError_t e = try_fast ? cudaLaunchKernelEx(&cfg, attn_tc_kernel<true>, tm_k, tm_v, tm_q, tm_kb, tm_vb, ap)
+                             : cudaLaunchKernelEx(&cfg, attn_tc_kernel<false>, tm_k, tm_v, tm_q, tm_kb, tm_vb, ap);
     if (e != cudaSuccess) return cuda_fail(e, "attention launch");
     return HERALD_OK;
 }
@@ -1198,11 +1211,12 @@ int herald_pipeline_tune(herald_pipeline_t* p, int32_t reps, herald_schedule_t* 
 
 int herald_set_tuning(const herald_tuning_t* t) {
     if (!t) {
-        g_tune = herald_tuning_t{0, 0, 0, 0, 0, 0, 0};
+        g_tune = herald_tuning_t{0, 0, 0, 0, 0, 0, 0, 0};
         return HERALD_OK;
     }
     if (t->attn_splits < 0 || t->attn_splits > kTcMaxSplits || t->attn_m_tiles < 0 || t->attn_total_ctas < 0 || t->scan_ctas < 0 ||
-        t->xq_path < HERALD_XQ_AUTO || t->xq_path > HERALD_XQ_TCGEN05)
+        t->xq_path < HERALD_XQ_AUTO || t->xq_path > HERALD_XQ_TCGEN05 || t->attn_precision < HERALD_ATTN_AUTO ||
+        t->attn_precision > HERALD_ATTN_FAST_FIRST)
         return fail(HERALD_ERR_INVALID_ARG, "herald_set_tuning: value out of range (attn_splits 0..%d, xq_path 0..2, the rest >= 0)", kTcMaxSplits);
     g_tune = *t;
     return HERALD_OK;

@@ -80,10 +80,11 @@ class HostIO(C.Structure):
 
 class Tuning(C.Structure):
     _fields_ = [("attn_splits", C.c_int32), ("attn_m_tiles", C.c_int32), ("attn_total_ctas", C.c_int32),
-                ("attn_no_pdl", C.c_int32), ("scan_ctas", C.c_int32), ("scan_head_major", C.c_int32), ("xq_path", C.c_int32)]
+                ("attn_no_pdl", C.c_int32), ("scan_ctas", C.c_int32), ("scan_head_major", C.c_int32), ("xq_path", C.c_int32), ("attn_precision", C.c_int32)]
 
 
 XQ_AUTO, XQ_MMA_SYNC, XQ_TCGEN05 = 0, 1, 2
+ATTN_AUTO, ATTN_EXACT, ATTN_FAST_FIRST = 0, 1, 2
 
 
 class Profile(C.Structure):
