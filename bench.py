@@ -502,7 +502,8 @@ def fig14_sweep(H, synth, torch, dev, seed, scan_ctas):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--steps", type=int, default=None,
+                    help="block steps per timed region (default: 200 for the CUDA arm, about 50 ms per region; 30 for --impl reference)")
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="herald", choices=["herald", "reference"])
     ap.add_argument("--workload", default=WORKLOAD)
@@ -518,6 +519,8 @@ def main():
     ap.add_argument("--no-graph", action="store_true", help="launch every kernel eagerly instead of replaying the captured block step")
     ap.add_argument("--quick", action="store_true", help="the C2 line only: no other workloads, no Fig. 14 sweep, no NEXT-row timings")
     args = ap.parse_args()
+    if args.steps is None:
+        args.steps = 30 if args.impl == "reference" else 200
     if args.impl == "reference":
         return run_reference(args)
 
@@ -638,7 +641,7 @@ def main():
     io = pipe.make_host_io(hosts)
     h2d = sum(h[n].numel() * h[n].element_size() for h in hosts for n in ("q_rep", "q_blk", "k_blk", "v_blk"))
     d2h = sum(h["out"].numel() * 4 for h in hosts)
-    e2e_steps = args.steps if n_layers == 1 else min(args.steps, 3)
+    e2e_steps = min(args.steps, 40) if n_layers == 1 else min(args.steps, 3)
     for _ in range(3 if n_layers == 1 else 1):
         pipe.step_host(io)
     torch.cuda.synchronize()
@@ -647,25 +650,37 @@ def main():
     a.record(pipe.main_stream)
     for _ in range(e2e_steps):
         pipe.step_host(io)
-    b.record(pipe.retrieval_stream)          # the last download of the outputs runs on the retrieval stream
+    b.record(pipe.copy_stream)               # the last download of the outputs runs on the pipeline's copy stream
     torch.cuda.synchronize()
     e2e_ms = max_over_ranks(a.elapsed_time(b), dev) / e2e_steps
     e2e_tokens = world * w.batch * w.block_size / (e2e_ms * 1e-3)
-    # the link floor of that step: its larger copy direction at the rate one pinned copy of the same size reaches here
+    # the link floor of that step: each direction alone, and both directions at once (what the step does: the upload of a block
+    # runs beside the download of the previous one), at the rates pinned copies of the output tensor reach on this box
     big = hosts[0]["out"]
-    dev_big = pipe.outs[0]
+    big2 = torch.empty_like(big).pin_memory()
+    dev_big, dev_big2 = pipe.outs[0], torch.empty_like(pipe.outs[0])
     link = {}
-    for name, src, dst in (("d2h", dev_big, big), ("h2d", big, dev_big)):
-        ca, cb = rig.ev(), rig.ev()
-        with torch.cuda.stream(side):
-            dst.copy_(src, non_blocking=True)
-            ca.record(side)
-            for _ in range(3):
+    side2 = torch.cuda.Stream(device=dev)
+    for name, pairs in (("d2h", [(side, dev_big, big)]), ("h2d", [(side, big, dev_big)]),
+                        ("both", [(side, dev_big, big), (side2, big2, dev_big2)])):
+        evs = []
+        for st, src, dst in pairs:
+            with torch.cuda.stream(st):
                 dst.copy_(src, non_blocking=True)
-            cb.record(side)
         torch.cuda.synchronize()
-        link[name + "_gbs"] = 3 * big.numel() * 4 / (ca.elapsed_time(cb) * 1e-3) / 1e9
+        for st, src, dst in pairs:
+            ca, cb = rig.ev(), rig.ev()
+            with torch.cuda.stream(st):
+                ca.record(st)
+                for _ in range(3):
+                    dst.copy_(src, non_blocking=True)
+                cb.record(st)
+            evs.append((ca, cb))
+        torch.cuda.synchronize()
+        link[name + "_gbs"] = sum(3 * big.numel() * 4 / (ca.elapsed_time(cb) * 1e-3) / 1e9 for ca, cb in evs)
     pcie_floor_ms = max(d2h / (link["d2h_gbs"] * 1e9), h2d / (link["h2d_gbs"] * 1e9)) * 1e3
+    pcie_floor_bidir_ms = (d2h + h2d) / (link["both_gbs"] * 1e9) * 1e3
+    del big2, dev_big2
 
     # ---- the other workloads and the Fig. 14 analogue (N = 1, default run only) ----
     other, fig14 = None, None
@@ -757,9 +772,12 @@ def main():
         "roofline": roofline, "roofline_scan": roofline_scan,
         "cpu_baseline": cpu_baseline,
         "e2e": {"value": e2e_tokens, "unit": "tokens/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "pcie_floor_ms": pcie_floor_ms, "link_gbs_measured": link,
-                "note": "uploads on the main stream, downloads on the retrieval stream (full duplex); the floor is the larger direction at the "
-                        "rate one pinned copy of the output tensor reaches on this box"},
+                "pcie_floor_ms": pcie_floor_ms, "pcie_floor_both_directions_ms": pcie_floor_bidir_ms, "link_gbs_measured": link,
+                "steps": e2e_steps,
+                "note": "uploads on the main stream, downloads on a copy stream (full duplex), two sets of device output buffers so that "
+                        "a block's attention runs beside the previous block's download; pcie_floor_ms = the larger direction alone, "
+                        "pcie_floor_both_directions_ms = all bytes of a step at the aggregate rate of an upload and a download running at once "
+                        "(both measured here with pinned copies of the output tensor)"},
         "gpu_launches": args.steps * ((n_layers - n_dense) * (3 + n_steps + (1 if int(pipe.c.scan_head_permille) > 0 else 0)) + n_dense * n_steps),   # per block step: scan (two launches with a head start), top-k, gather, T-1 x attention (first timed region only)
         "clocks": clock_info,
     }

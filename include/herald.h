@@ -335,14 +335,22 @@ int herald_pipeline_set_debug_delay(uint32_t main_us, uint32_t retrieval_us);
  * Each host_* is a host array of n_layers host pointers with the same extents as the device tensors.
  * The KV cache stays resident in HBM (it is the state, not a per-step input).  Uploads run on the main stream and
  * downloads on the retrieval stream, so that the upload of a block overlaps the download of the previous one; the next
- * call orders its attention after that download by itself.  The caller synchronises BOTH streams before reading
- * host_out (or before touching the host input buffers again). */
+ * call orders its attention after the download that last read its output buffer by itself (see dev_out_alt).  The caller synchronises BOTH streams before reading
+ * host_out (or before touching the host input buffers again) -- and copy_stream if one is given. */
 typedef struct herald_host_io {
     const void* const* host_q_rep;
     const void* const* host_q_blk;
     const void* const* host_k_blk;
     const void* const* host_v_blk;
     void* const* host_out;
+    /* optional double buffering of the device outputs: dev_out_alt[l] is a second fp32 [n_steps][batch][B][H_q][128] device buffer per
+     * layer.  Blocks then alternate between layers[l].out and dev_out_alt[l] (by pipe->active), so that the attention of a block
+     * runs beside the download of the previous block instead of behind it; ev_download[2] are caller-created events the library
+     * records after each download.  NULL = single buffering (the attention waits for the previous download). */
+    void* const* dev_out_alt;
+    herald_event_t ev_download[2];
+    herald_stream_t copy_stream; /* optional third stream for the downloads; NULL = the retrieval stream (the next block's selection
+                                    then queues behind the download of this block) */
 } herald_host_io_t;
 
 /* host_q_rep[l] may be NULL for a layer with `dense` set.  Every pointer is validated before anything is enqueued.

@@ -1239,8 +1239,10 @@ int herald_pipeline_step_host(herald_pipeline_t* p, const herald_host_io_t* io) 
     if (rc) return rc;
     if (!io || !io->host_q_rep || !io->host_q_blk || !io->host_k_blk || !io->host_v_blk || !io->host_out)
         return fail(HERALD_ERR_INVALID_ARG, "pipeline_step_host: NULL host io");
+    if (io->dev_out_alt && (p->n_layers > 64 || !io->ev_download[0] || !io->ev_download[1]))
+        return fail(HERALD_ERR_INVALID_ARG, "pipeline_step_host: dev_out_alt needs both ev_download events and at most 64 layers");
     for (int l = 0; l < p->n_layers; ++l)
-        if ((!p->layers[l].dense && !io->host_q_rep[l]) || !io->host_q_blk[l] || !io->host_k_blk[l] || !io->host_v_blk[l] || !io->host_out[l])
+        if ((io->dev_out_alt && !io->dev_out_alt[l]) || (!p->layers[l].dense && !io->host_q_rep[l]) || !io->host_q_blk[l] || !io->host_k_blk[l] || !io->host_v_blk[l] || !io->host_out[l])
             return fail(HERALD_ERR_INVALID_ARG, "pipeline_step_host: layer %d has a NULL host pointer", l);
     cudaStream_t s_main = static_cast<cudaStream_t>(p->main_stream);
     cudaStream_t s_ret = static_cast<cudaStream_t>(p->retrieval_stream);
@@ -1266,22 +1268,35 @@ int herald_pipeline_step_host(herald_pipeline_t* p, const herald_host_io_t* io) 
             e = cudaMemcpyAsync(const_cast<void*>(ly->v_blk), io->host_v_blk[l], kv_step * p->n_steps * 2, cudaMemcpyHostToDevice, s_main);
         if (e != cudaSuccess) return cuda_fail(e, "H2D copy");
     }
-    // this block's attention overwrites `out`: the previous call's download (last record of ev_join) must have read it
-    e = cudaStreamWaitEvent(s_main, ev_join, 0);
+    // This block's attention overwrites its output buffer: the download that last read that buffer must be done.  With a
+    // second set of device output buffers (dev_out_alt) the blocks alternate between the two sets, so the attention of this
+    // block only waits for the download issued TWO calls ago and runs beside the previous block's download.
+    const bool alternate = io->dev_out_alt != nullptr;
+    const int parity = p->active;
+    cudaEvent_t ev_done = alternate ? static_cast<cudaEvent_t>(io->ev_download[parity]) : ev_join;
+    e = cudaStreamWaitEvent(s_main, ev_done, 0);
     if (e != cudaSuccess) return cuda_fail(e, "wait previous download");
+    float* saved_out[64];
+    const bool swap = alternate && parity == 1;
+    if (swap)
+        for (int l = 0; l < p->n_layers; ++l) {
+            saved_out[l] = p->layers[l].out;
+            p->layers[l].out = static_cast<float*>(io->dev_out_alt[l]);
+        }
     rc = herald_pipeline_step(p);
-    if (rc) return rc;
-    e = cudaEventRecord(ev_fork, s_main);                    // outputs of this block are complete
-    if (e == cudaSuccess) e = cudaStreamWaitEvent(s_ret, ev_fork, 0);
-    if (e != cudaSuccess) return cuda_fail(e, "order download after the block");
-    for (int l = 0; l < p->n_layers; ++l) {
-        herald_layer_t* ly = &p->layers[l];
-        e = cudaMemcpyAsync(io->host_out[l], ly->out, q_step * p->n_steps * sizeof(float), cudaMemcpyDeviceToHost, s_ret);
-        if (e != cudaSuccess) return cuda_fail(e, "D2H copy");
+    if (rc == HERALD_OK) {
+        // downloads go to the copy stream if there is one: on the retrieval stream the NEXT block's selection would queue behind them
+        cudaStream_t s_copy = io->copy_stream ? static_cast<cudaStream_t>(io->copy_stream) : s_ret;
+        e = cudaEventRecord(ev_fork, s_main);                    // outputs of this block are complete
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s_copy, ev_fork, 0);
+        for (int l = 0; l < p->n_layers && e == cudaSuccess; ++l)
+            e = cudaMemcpyAsync(io->host_out[l], p->layers[l].out, q_step * p->n_steps * sizeof(float), cudaMemcpyDeviceToHost, s_copy);
+        if (e == cudaSuccess) e = cudaEventRecord(ev_done, s_copy);   // download done: a later call waits on it
+        if (e != cudaSuccess) rc = cuda_fail(e, "D2H copy");
     }
-    e = cudaEventRecord(ev_join, s_ret);                     // download done: the next call waits on it
-    if (e != cudaSuccess) return cuda_fail(e, "record download");
-    return HERALD_OK;
+    if (swap)
+        for (int l = 0; l < p->n_layers; ++l) p->layers[l].out = saved_out[l];
+    return rc;
 }
 
 }  // extern "C"

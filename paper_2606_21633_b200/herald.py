@@ -75,7 +75,7 @@ class Schedule(C.Structure):
 class HostIO(C.Structure):
     _fields_ = [("host_q_rep", C.POINTER(C.c_void_p)), ("host_q_blk", C.POINTER(C.c_void_p)),
                 ("host_k_blk", C.POINTER(C.c_void_p)), ("host_v_blk", C.POINTER(C.c_void_p)),
-                ("host_out", C.POINTER(C.c_void_p))]
+                ("host_out", C.POINTER(C.c_void_p)), ("dev_out_alt", C.POINTER(C.c_void_p)), ("ev_download", C.c_void_p * 2), ("copy_stream", C.c_void_p)]
 
 
 class Tuning(C.Structure):
@@ -374,11 +374,24 @@ class BlockPipeline:
     def step(self):
         herald_pipeline_step(self.c)
 
-    def make_host_io(self, host_layers) -> HostIO:
-        """host_layers: list of dicts of PINNED host tensors q_rep, q_blk, k_blk, v_blk, out."""
+    def make_host_io(self, host_layers, double_buffer=True) -> HostIO:
+        """host_layers: list of dicts of PINNED host tensors q_rep, q_blk, k_blk, v_blk, out.  double_buffer: a second set of
+        device output buffers, so that a block's attention runs beside the previous block's download."""
         n = len(host_layers)
         io = HostIO()
         self._io_arrays = []
+        if double_buffer:
+            self.outs_alt = [torch.empty_like(o) for o in self.outs]
+            alt = (C.c_void_p * n)(*[o.data_ptr() for o in self.outs_alt])
+            self._io_arrays.append(alt)
+            io.dev_out_alt = C.cast(alt, C.POINTER(C.c_void_p))
+            self._ev_download = [torch.cuda.Event(), torch.cuda.Event()]
+            with torch.cuda.device(self.device):
+                for i, e in enumerate(self._ev_download):
+                    e.record(self.retrieval_stream)          # materialises the cudaEvent_t handles
+                    io.ev_download[i] = e.cuda_event
+            self.copy_stream = torch.cuda.Stream(device=self.device)
+            io.copy_stream = self.copy_stream.cuda_stream
         for name in ("q_rep", "q_blk", "k_blk", "v_blk", "out"):
             arr = (C.c_void_p * n)(*[h[name].data_ptr() for h in host_layers])
             self._io_arrays.append(arr)

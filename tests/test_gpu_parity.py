@@ -642,7 +642,8 @@ def test_pipeline_with_a_dense_layer(H, cuda):
         assert np.abs(pipe.outs[1][s].cpu().numpy().astype(np.float64) - ref).max() <= ATTN_TOL
 
 
-def test_pipeline_host_io_roundtrip(H, cuda):
+@pytest.mark.parametrize("double_buffer", [False, True])
+def test_pipeline_host_io_roundtrip(H, cuda, double_buffer):
     w = synth.Workload("pipeh", 1, (1024,), 8, 2, 16, 3, 100, "plain")
     inp = synth.make_inputs(w, seed=9, device=cuda)
     ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
@@ -654,9 +655,10 @@ def test_pipeline_host_io_roundtrip(H, cuda):
         dev_layer[n] = torch.zeros_like(inp[n])
     pipe = H.BlockPipeline(shape, [dev_layer], w.n_attn_steps, 0, cuda)
     host["out"] = torch.zeros(pipe.outs[0].shape, dtype=torch.float32).pin_memory()
-    io = pipe.make_host_io([host])
+    io = pipe.make_host_io([host], double_buffer=double_buffer)
     pipe.step_host(io)
     pipe.step_host(io)       # second block attends over the pool selected by the first
+    pipe.step_host(io)       # (third: with two sets of device outputs this one reuses the first set)
     torch.cuda.synchronize()
     oi = oracle_inputs(inp)
     sel, _ = O.select(oi["q_rep"], oi["k_pages"], oi["page_table"], oi["seq_lens"], ks, 2, 128 ** -0.5)
