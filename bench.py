@@ -33,9 +33,9 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/r1_*), by workload
-NCU_ATTN_DRAM_BYTES = {"C2": 30.7e6}
-NCU_SCAN_DRAM_BYTES = {"C2": 275.5e6}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/r2_*), by workload
+NCU_ATTN_DRAM_BYTES = {"C2": 29.7e6}
+NCU_SCAN_DRAM_BYTES = {"C2": 273.8e6}
 METRIC = "selection-scan HBM GB/s (% of 8 TB/s); sparse-attn TFLOP/s; block tokens/s"
 WORKLOAD = "C2"
 SEED = 21633 + 1000 * 2
@@ -765,7 +765,7 @@ def main():
                          f"({rig.rows * 512 / 1e6:.0f} MB) is reused by all {n_steps} steps by design (L2-cold attention is reported in breakdown)",
                    "start_after_step": int(pipe.c.start_after_step), "scan_ctas": int(pipe.c.scan_ctas),
                    "scan_head_permille": int(pipe.c.scan_head_permille),
-                   "schedule_sweep_ms (scan_ctas/start_after_step/scan_head_permille, untimed calibration by herald_pipeline_tune, eager)": rs_sweep,
+                   "schedule_sweep_ms (scan_ctas/start_after_step/scan_head_permille, untimed calibration by herald_pipeline_tune, graph replay)": rs_sweep,
                    "attn_grid_ctas": H.herald_attn_grid_ctas(shape),
                    "launch": "eager" if rig.graphs is None else "one CUDA graph per pool parity, replayed"},
         "breakdown": breakdown,

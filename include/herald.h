@@ -297,10 +297,11 @@ typedef struct herald_pipeline {
 int herald_pipeline_step(herald_pipeline_t* pipe);
 
 /* Calibration of the schedule of a pipeline (how the retrieval stream shares the device with the denoising steps): runs
- * eager block steps -- each a complete, valid step, so the pools stay consistent -- for a handful of
- * (scan_ctas, start_after_step, scan_head_permille) candidates, `reps` timed steps each after two warm-up steps, timed with
- * CUDA events on the main stream, and leaves the fastest candidate in *pipe.  This is the ONE entry of the library that
- * creates (and destroys) two events and synchronises with the host; call it once outside any timed region or graph
+ * block steps -- each a complete, valid step, so the pools stay consistent -- for a handful of
+ * (scan_ctas, start_after_step, scan_head_permille) candidates: two eager warm-up steps, then the step captured into a CUDA
+ * graph and replayed `reps` times between two CUDA events on the main stream (eager steps if the capture fails), and leaves
+ * the fastest candidate in *pipe.  This is the ONE entry of the library that creates (and destroys) events and graphs and
+ * synchronises with the host; call it once outside any timed region or graph
  * capture.  table (optional, host): receives up to table_cap measured candidates, *n_table how many.  Host only. */
 typedef struct herald_schedule {
     int32_t scan_ctas, start_after_step, scan_head_permille;

@@ -1167,18 +1167,44 @@ int herald_pipeline_tune(herald_pipeline_t* p, int32_t reps, herald_schedule_t* 
     int n = 0;
     float best_ms = 0.f;
     herald_schedule_t best{p->scan_ctas, p->start_after_step, p->scan_head_permille, 0.f};
+    // a candidate is timed the way a serving loop runs it: the block step captured once into a CUDA graph and replayed (cross-stream
+    // event waits cost several microseconds more between eagerly launched kernels than between graph nodes, which would
+    // bias the choice against schedules with an extra dependency); the replays use the same pool parity, which changes nothing
+    // in the work done.  If the capture fails (streams already capturing) the candidate is timed with eager steps.
     auto time_one = [&](int ctas, int start, int head) -> int {
         p->scan_ctas = ctas; p->start_after_step = start; p->scan_head_permille = head;
         int r = HERALD_OK;
-        for (int i = 0; i < 2 && r == HERALD_OK; ++i) r = herald_pipeline_step(p);
+        for (int i = 0; i < 2 && r == HERALD_OK; ++i) r = herald_pipeline_step(p);    // eager warm-up: one-time setup, both parities
         if (r) return r;
         cudaStreamSynchronize(s_main); cudaStreamSynchronize(s_ret);
-        cudaEventRecord(a, s_main);
-        for (int i = 0; i < reps && r == HERALD_OK; ++i) r = herald_pipeline_step(p);
+        cudaGraph_t graph = nullptr;
+        cudaGraphExec_t exec = nullptr;
+        const int act0 = p->active;
+        if (cudaStreamBeginCapture(s_main, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            r = herald_pipeline_step(p);
+            const cudaError_t ce = cudaStreamEndCapture(s_main, &graph);
+            p->active = act0;                                   // the capture enqueued nothing
+            if (r != HERALD_OK || ce != cudaSuccess || cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) exec = nullptr;
+            if (r != HERALD_OK) { if (graph) cudaGraphDestroy(graph); return r; }
+        }
+        (void)cudaGetLastError();
+        auto run = [&]() -> int {
+            if (exec) return cudaGraphLaunch(exec, s_main) == cudaSuccess ? HERALD_OK : fail(HERALD_ERR_CUDA, "herald_pipeline_tune: graph launch failed");
+            return herald_pipeline_step(p);
+        };
+        for (int i = 0; i < 2 && r == HERALD_OK; ++i) r = run();
+        if (r == HERALD_OK) {
+            cudaStreamSynchronize(s_main); cudaStreamSynchronize(s_ret);
+            cudaEventRecord(a, s_main);
+            for (int i = 0; i < reps && r == HERALD_OK; ++i) r = run();
+            cudaEventRecord(b, s_main);
+            const cudaError_t ee = cudaEventSynchronize(b);
+            if (r == HERALD_OK && ee != cudaSuccess) r = cuda_fail(ee, "herald_pipeline_tune: step failed");
+        }
+        cudaStreamSynchronize(s_ret);
+        if (exec) cudaGraphExecDestroy(exec);
+        if (graph) cudaGraphDestroy(graph);
         if (r) return r;
-        cudaEventRecord(b, s_main);
-        cudaError_t ee = cudaEventSynchronize(b);
-        if (ee != cudaSuccess) return cuda_fail(ee, "herald_pipeline_tune: step failed");
         float ms = 0.f;
         cudaEventElapsedTime(&ms, a, b);
         ms /= (float)reps;
@@ -1199,8 +1225,8 @@ int herald_pipeline_tune(herald_pipeline_t* p, int32_t reps, herald_schedule_t* 
     // 2. with the best overlapped grid: how much of the scan runs on every SM before the denoising steps start
     if (rc == HERALD_OK && best.scan_ctas < n_sm && p->shape.agg_mode == HERALD_AGG_MAX_LOGIT) {
         const int ctas = best.scan_ctas, start = best.start_after_step;
-        const int heads[5] = {100, 200, 300, 450, 600};
-        for (int i = 0; i < 5 && rc == HERALD_OK; ++i) rc = time_one(ctas, start, heads[i]);
+        const int heads[6] = {50, 100, 200, 300, 450, 600};
+        for (int i = 0; i < 6 && rc == HERALD_OK; ++i) rc = time_one(ctas, start, heads[i]);
     }
     cudaEventDestroy(a);
     cudaEventDestroy(b);
