@@ -682,6 +682,23 @@ def main():
     pcie_floor_bidir_ms = (d2h + h2d) / (link["both_gbs"] * 1e9) * 1e3
     del big2, dev_big2
 
+    # ---- read-only streaming probe: a library reduction over 1 GiB, the ceiling a read-only stream like the scan has ----
+    read_probe_gbs = None
+    if full:
+        probe = torch.empty(1 << 29, dtype=torch.bfloat16, device=dev).normal_()
+        best = None
+        for i in range(6):
+            pa, pb = rig.ev(), rig.ev()
+            pa.record()
+            probe.sum(dtype=torch.float32)
+            pb.record()
+            torch.cuda.synchronize()
+            if i:
+                best = min(best or 1e9, pa.elapsed_time(pb))
+        read_probe_gbs = probe.numel() * 2 / (best * 1e-3) / 1e9
+        del probe
+        torch.cuda.empty_cache()
+
     # ---- the other workloads and the Fig. 14 analogue (N = 1, default run only) ----
     other, fig14 = None, None
     if full:
@@ -734,6 +751,8 @@ def main():
         "block_latency_ms": ms_step, "block_latency_median_ms": statistics.median(regions), "block_latency_min_ms": regions_sorted[0],
         "timed_regions": len(regions), "steps_per_region": args.steps,
         "scan_gbs_alone": scan_gbs_alone, "scan_pct_of_8TBs_alone": 100.0 * scan_gbs_alone / 8000.0,
+        "hbm_read_probe_gbs (torch sum over 1 GiB bf16, best of 5)": read_probe_gbs,
+        "scan_frac_of_read_probe": scan_gbs_alone / read_probe_gbs if read_probe_gbs else None,
         "scan_kernel_ms": iso["scan_kernel_ms"], "scan_with_memset_and_empty_topk_ms": iso["scan_with_memset_and_empty_topk_ms"],
         "scan_kernel_eager_events_ms": iso["scan_kernel_eager_events_ms"], "scan_kernel_eager_events_min_ms": iso["scan_kernel_eager_events_min_ms"],
         "scan_gbs_eager_events": rig.scan_bytes / (iso["scan_kernel_eager_events_ms"] * 1e-3) / 1e9,
