@@ -579,9 +579,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
 #pragma unroll
                         for (int kk = 0; kk < 8; ++kk) {
                             umma_ts(o_base, p_base + kk * 8, v_lo + kk * 128, hi_k, idesc_pv, (j > 0 || kk > 0) ? 1u : 0u);
-#ifndef HERALD_EXP_NOLO
                             umma_ts(o_base, p_base + 64 + kk * 8, v_lo + kk * 128, hi_k, idesc_pv, 1u);
-#endif
                         }
                     } else {
                         for (int kk = 0; kk < ksteps; ++kk) {
@@ -715,11 +713,9 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                     const float e0 = fast_exp2(x0), e1 = fast_exp2(x1);
                     fadd2(sum0, sum1, sum0, sum1, e0, e1);
                     hi[i] = pack_bf16(e0, e1);
-#ifndef HERALD_EXP_NOLO
                     float r0, r1;
                     ffma2v(r0, r1, __uint_as_float(hi[i] << 16), __uint_as_float(hi[i] & 0xffff0000u), -1.f, e0, e1);   // e - hi, exact
                     lo[i] = pack_bf16(r0, r1);
-#endif
                 }
                 l_run = l_run * alpha + (sum0 + sum1);
                 if (any) {   // rare: the running maximum of some row grew past the threshold -> rescale O in place
@@ -735,9 +731,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 // Both halves go to TMEM as the A operand of the PV MMA: row = lane, two keys per 32-bit column; P_hi in
                 // columns [0,64) of the S buffer, P_lo in [64,128), this thread's quarter row at [cq*16, cq*16+16) of each.
                 tmem_st16(lane_base + sb * 128 + cq * 16, hi);
-#ifndef HERALD_EXP_NOLO
                 tmem_st16(lane_base + sb * 128 + 64 + cq * 16, lo);
-#endif
                 tmem_wait_st();
                 tc_fence_before();
                 __syncwarp();
