@@ -793,8 +793,8 @@ def main():
         "e2e": {"value": e2e_tokens, "unit": "tokens/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "pcie_floor_ms": pcie_floor_ms, "pcie_floor_both_directions_ms": pcie_floor_bidir_ms, "link_gbs_measured": link,
                 "steps": e2e_steps,
-                "note": "uploads on the main stream, downloads on a copy stream (full duplex), two sets of device output buffers so that "
-                        "a block's attention runs beside the previous block's download; pcie_floor_ms = the larger direction alone, "
+                "note": "uploads on an upload stream, downloads on a copy stream (full duplex), two sets of device input and output buffers so "
+                        "that the transfers of neighbouring blocks run beside a block's attention; pcie_floor_ms = the larger direction alone, "
                         "pcie_floor_both_directions_ms = all bytes of a step at the aggregate rate of an upload and a download running at once "
                         "(both measured here with pinned copies of the output tensor)"},
         "gpu_launches": args.steps * ((n_layers - n_dense) * (3 + n_steps + (1 if int(pipe.c.scan_head_permille) > 0 else 0)) + n_dense * n_steps),   # per block step: scan (two launches with a head start), top-k, gather, T-1 x attention (first timed region only)

@@ -337,7 +337,7 @@ int herald_pipeline_set_debug_delay(uint32_t main_us, uint32_t retrieval_us);
  * The KV cache stays resident in HBM (it is the state, not a per-step input).  Uploads run on the main stream and
  * downloads on the retrieval stream, so that the upload of a block overlaps the download of the previous one; the next
  * call orders its attention after the download that last read its output buffer by itself (see dev_out_alt).  The caller synchronises BOTH streams before reading
- * host_out (or before touching the host input buffers again) -- and copy_stream if one is given. */
+ * host_out (or before touching the host input buffers again) -- and copy_stream / upload_stream if given. */
 typedef struct herald_host_io {
     const void* const* host_q_rep;
     const void* const* host_q_blk;
@@ -352,6 +352,18 @@ typedef struct herald_host_io {
     herald_event_t ev_download[2];
     herald_stream_t copy_stream; /* optional third stream for the downloads; NULL = the retrieval stream (the next block's selection
                                     then queues behind the download of this block) */
+    /* optional double buffering of the device INPUTS: dev_*_alt[l] are second device buffers with the extents of layers[l].q_rep /
+     * q_blk / k_blk / v_blk (dev_q_rep_alt[l] may be NULL for a dense layer).  Blocks alternate between the two sets; the uploads of
+     * a block then run on upload_stream beside the previous block's attention instead of in front of their own.  ev_upload[2]
+     * (recorded on upload_stream after a block's uploads) and ev_compute[2] (recorded on the main stream after a block step: its
+     * input set may be overwritten) are caller-created.  dev_q_blk_alt == NULL = single buffering, uploads on the main stream. */
+    void* const* dev_q_rep_alt;
+    void* const* dev_q_blk_alt;
+    void* const* dev_k_blk_alt;
+    void* const* dev_v_blk_alt;
+    herald_stream_t upload_stream;
+    herald_event_t ev_upload[2];
+    herald_event_t ev_compute[2];
 } herald_host_io_t;
 
 /* host_q_rep[l] may be NULL for a layer with `dense` set.  Every pointer is validated before anything is enqueued.

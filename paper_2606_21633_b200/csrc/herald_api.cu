@@ -1265,11 +1265,20 @@ int herald_pipeline_step_host(herald_pipeline_t* p, const herald_host_io_t* io) 
     if (rc) return rc;
     if (!io || !io->host_q_rep || !io->host_q_blk || !io->host_k_blk || !io->host_v_blk || !io->host_out)
         return fail(HERALD_ERR_INVALID_ARG, "pipeline_step_host: NULL host io");
-    if (io->dev_out_alt && (p->n_layers > 64 || !io->ev_download[0] || !io->ev_download[1]))
-        return fail(HERALD_ERR_INVALID_ARG, "pipeline_step_host: dev_out_alt needs both ev_download events and at most 64 layers");
-    for (int l = 0; l < p->n_layers; ++l)
-        if ((io->dev_out_alt && !io->dev_out_alt[l]) || (!p->layers[l].dense && !io->host_q_rep[l]) || !io->host_q_blk[l] || !io->host_k_blk[l] || !io->host_v_blk[l] || !io->host_out[l])
+    const bool out_alt = io->dev_out_alt != nullptr, in_alt = io->dev_q_blk_alt != nullptr;
+    if ((out_alt || in_alt) && p->n_layers > 64) return fail(HERALD_ERR_INVALID_ARG, "pipeline_step_host: double buffering supports at most 64 layers");
+    if (out_alt && (!io->ev_download[0] || !io->ev_download[1]))
+        return fail(HERALD_ERR_INVALID_ARG, "pipeline_step_host: dev_out_alt needs both ev_download events");
+    if (in_alt && (!io->dev_q_rep_alt || !io->dev_k_blk_alt || !io->dev_v_blk_alt || !io->upload_stream || !io->ev_upload[0] || !io->ev_upload[1] ||
+                   !io->ev_compute[0] || !io->ev_compute[1]))
+        return fail(HERALD_ERR_INVALID_ARG, "pipeline_step_host: the second input set needs all four dev_*_alt arrays, upload_stream, ev_upload[2] and ev_compute[2]");
+    for (int l = 0; l < p->n_layers; ++l) {
+        const bool dense = p->layers[l].dense != 0;
+        if ((out_alt && !io->dev_out_alt[l]) || (!dense && !io->host_q_rep[l]) || !io->host_q_blk[l] || !io->host_k_blk[l] || !io->host_v_blk[l] || !io->host_out[l])
             return fail(HERALD_ERR_INVALID_ARG, "pipeline_step_host: layer %d has a NULL host pointer", l);
+        if (in_alt && ((!dense && !io->dev_q_rep_alt[l]) || !io->dev_q_blk_alt[l] || !io->dev_k_blk_alt[l] || !io->dev_v_blk_alt[l]))
+            return fail(HERALD_ERR_INVALID_ARG, "pipeline_step_host: layer %d has a NULL pointer in the second input set", l);
+    }
     cudaStream_t s_main = static_cast<cudaStream_t>(p->main_stream);
     cudaStream_t s_ret = static_cast<cudaStream_t>(p->retrieval_stream);
     cudaEvent_t ev_fork = static_cast<cudaEvent_t>(p->ev_fork), ev_join = static_cast<cudaEvent_t>(p->ev_join);
@@ -1277,51 +1286,71 @@ int herald_pipeline_step_host(herald_pipeline_t* p, const herald_host_io_t* io) 
     const size_t q_step = (size_t)sh->batch * sh->block_size * sh->n_q_heads * kHeadDim;
     const size_t kv_step = (size_t)sh->batch * sh->block_size * sh->n_kv_heads * kHeadDim;
     const size_t q_rep_bytes = (size_t)sh->batch * sh->n_q_heads * kHeadDim * 2;
-    cudaError_t e;
-    // The two copy directions run on the two streams so that the upload of this block overlaps the download of the
-    // previous one (full-duplex link, two copy engines): uploads on the main stream, downloads on the retrieval stream.
-    for (int l = 0; l < p->n_layers; ++l) {
-        herald_layer_t* ly = &p->layers[l];
-        // inputs are enqueued on the main stream; the fork event orders the retrieval stream after them
-        e = cudaSuccess;
-        if (!ly->dense)                       // a dense layer has no representative query (host_q_rep[l] may be NULL)
-            e = cudaMemcpyAsync(const_cast<void*>(ly->q_rep), io->host_q_rep[l], q_rep_bytes, cudaMemcpyHostToDevice, s_main);
-        if (e == cudaSuccess)
-            e = cudaMemcpyAsync(const_cast<void*>(ly->q_blk), io->host_q_blk[l], q_step * p->n_steps * 2, cudaMemcpyHostToDevice, s_main);
-        if (e == cudaSuccess)
-            e = cudaMemcpyAsync(const_cast<void*>(ly->k_blk), io->host_k_blk[l], kv_step * p->n_steps * 2, cudaMemcpyHostToDevice, s_main);
-        if (e == cudaSuccess)
-            e = cudaMemcpyAsync(const_cast<void*>(ly->v_blk), io->host_v_blk[l], kv_step * p->n_steps * 2, cudaMemcpyHostToDevice, s_main);
-        if (e != cudaSuccess) return cuda_fail(e, "H2D copy");
-    }
-    // This block's attention overwrites its output buffer: the download that last read that buffer must be done.  With a
-    // second set of device output buffers (dev_out_alt) the blocks alternate between the two sets, so the attention of this
-    // block only waits for the download issued TWO calls ago and runs beside the previous block's download.
-    const bool alternate = io->dev_out_alt != nullptr;
+    cudaError_t e = cudaSuccess;
+    // Blocks alternate (by pipe->active) between the caller's device buffers and the optional second sets: with a second
+    // OUTPUT set the attention of this block waits only for the download issued two calls ago, with a second INPUT set the
+    // uploads of this block run on their own stream beside the previous block's attention -- the link is then busy in both
+    // directions all the time and a block costs what its larger direction costs.
     const int parity = p->active;
-    cudaEvent_t ev_done = alternate ? static_cast<cudaEvent_t>(io->ev_download[parity]) : ev_join;
-    e = cudaStreamWaitEvent(s_main, ev_done, 0);
-    if (e != cudaSuccess) return cuda_fail(e, "wait previous download");
-    float* saved_out[64];
-    const bool swap = alternate && parity == 1;
-    if (swap)
+    struct Saved { const void *q_rep, *q_blk, *k_blk, *v_blk; float* out; } saved[64];
+    const bool swap_out = out_alt && parity == 1, swap_in = in_alt && parity == 1;
+    if (swap_out || swap_in)
         for (int l = 0; l < p->n_layers; ++l) {
-            saved_out[l] = p->layers[l].out;
-            p->layers[l].out = static_cast<float*>(io->dev_out_alt[l]);
+            herald_layer_t* ly = &p->layers[l];
+            saved[l] = Saved{ly->q_rep, ly->q_blk, ly->k_blk, ly->v_blk, ly->out};
+            if (swap_out) ly->out = static_cast<float*>(io->dev_out_alt[l]);
+            if (swap_in) {
+                ly->q_rep = io->dev_q_rep_alt[l];
+                ly->q_blk = io->dev_q_blk_alt[l];
+                ly->k_blk = io->dev_k_blk_alt[l];
+                ly->v_blk = io->dev_v_blk_alt[l];
+            }
         }
+    auto restore = [&]() {
+        if (swap_out || swap_in)
+            for (int l = 0; l < p->n_layers; ++l) {
+                herald_layer_t* ly = &p->layers[l];
+                ly->q_rep = saved[l].q_rep; ly->q_blk = saved[l].q_blk; ly->k_blk = saved[l].k_blk; ly->v_blk = saved[l].v_blk; ly->out = saved[l].out;
+            }
+    };
+    // uploads: on the main stream, or on the upload stream once the block that last read this input set has finished
+    cudaStream_t s_up = in_alt ? static_cast<cudaStream_t>(io->upload_stream) : s_main;
+    if (in_alt) e = cudaStreamWaitEvent(s_up, static_cast<cudaEvent_t>(io->ev_compute[parity]), 0);
+    for (int l = 0; l < p->n_layers && e == cudaSuccess; ++l) {
+        herald_layer_t* ly = &p->layers[l];
+        if (!ly->dense)                       // a dense layer has no representative query (host_q_rep[l] may be NULL)
+            e = cudaMemcpyAsync(const_cast<void*>(ly->q_rep), io->host_q_rep[l], q_rep_bytes, cudaMemcpyHostToDevice, s_up);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(const_cast<void*>(ly->q_blk), io->host_q_blk[l], q_step * p->n_steps * 2, cudaMemcpyHostToDevice, s_up);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(const_cast<void*>(ly->k_blk), io->host_k_blk[l], kv_step * p->n_steps * 2, cudaMemcpyHostToDevice, s_up);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(const_cast<void*>(ly->v_blk), io->host_v_blk[l], kv_step * p->n_steps * 2, cudaMemcpyHostToDevice, s_up);
+    }
+    if (e == cudaSuccess && in_alt) {
+        e = cudaEventRecord(static_cast<cudaEvent_t>(io->ev_upload[parity]), s_up);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s_main, static_cast<cudaEvent_t>(io->ev_upload[parity]), 0);
+    }
+    // this block's attention overwrites its output buffer: the download that last read that buffer must be done
+    cudaEvent_t ev_done = out_alt ? static_cast<cudaEvent_t>(io->ev_download[parity]) : ev_join;
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s_main, ev_done, 0);
+    if (e != cudaSuccess) {
+        restore();
+        return cuda_fail(e, "H2D copy / ordering");
+    }
     rc = herald_pipeline_step(p);
     if (rc == HERALD_OK) {
         // downloads go to the copy stream if there is one: on the retrieval stream the NEXT block's selection would queue behind them
         cudaStream_t s_copy = io->copy_stream ? static_cast<cudaStream_t>(io->copy_stream) : s_ret;
-        e = cudaEventRecord(ev_fork, s_main);                    // outputs of this block are complete
+        e = cudaEventRecord(ev_fork, s_main);                    // this block is complete (the step joined the retrieval stream)
+        if (e == cudaSuccess && in_alt) e = cudaEventRecord(static_cast<cudaEvent_t>(io->ev_compute[parity]), s_main);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(s_copy, ev_fork, 0);
         for (int l = 0; l < p->n_layers && e == cudaSuccess; ++l)
             e = cudaMemcpyAsync(io->host_out[l], p->layers[l].out, q_step * p->n_steps * sizeof(float), cudaMemcpyDeviceToHost, s_copy);
         if (e == cudaSuccess) e = cudaEventRecord(ev_done, s_copy);   // download done: a later call waits on it
         if (e != cudaSuccess) rc = cuda_fail(e, "D2H copy");
     }
-    if (swap)
-        for (int l = 0; l < p->n_layers; ++l) p->layers[l].out = saved_out[l];
+    restore();
     return rc;
 }
 

@@ -75,7 +75,10 @@ class Schedule(C.Structure):
 class HostIO(C.Structure):
     _fields_ = [("host_q_rep", C.POINTER(C.c_void_p)), ("host_q_blk", C.POINTER(C.c_void_p)),
                 ("host_k_blk", C.POINTER(C.c_void_p)), ("host_v_blk", C.POINTER(C.c_void_p)),
-                ("host_out", C.POINTER(C.c_void_p)), ("dev_out_alt", C.POINTER(C.c_void_p)), ("ev_download", C.c_void_p * 2), ("copy_stream", C.c_void_p)]
+                ("host_out", C.POINTER(C.c_void_p)), ("dev_out_alt", C.POINTER(C.c_void_p)), ("ev_download", C.c_void_p * 2), ("copy_stream", C.c_void_p),
+                ("dev_q_rep_alt", C.POINTER(C.c_void_p)), ("dev_q_blk_alt", C.POINTER(C.c_void_p)),
+                ("dev_k_blk_alt", C.POINTER(C.c_void_p)), ("dev_v_blk_alt", C.POINTER(C.c_void_p)),
+                ("upload_stream", C.c_void_p), ("ev_upload", C.c_void_p * 2), ("ev_compute", C.c_void_p * 2)]
 
 
 class Tuning(C.Structure):
@@ -392,6 +395,21 @@ class BlockPipeline:
                     io.ev_download[i] = e.cuda_event
             self.copy_stream = torch.cuda.Stream(device=self.device)
             io.copy_stream = self.copy_stream.cuda_stream
+            # second set of device inputs + an upload stream: the uploads of a block run beside the previous block's attention
+            self.ins_alt = {}
+            for name in ("q_rep", "q_blk", "k_blk", "v_blk"):
+                bufs = [torch.empty_like(ly[name]) if not (name == "q_rep" and ly.get("dense")) else None for ly in self.keep]
+                self.ins_alt[name] = bufs
+                arr = (C.c_void_p * n)(*[b.data_ptr() if b is not None else None for b in bufs])
+                self._io_arrays.append(arr)
+                setattr(io, f"dev_{name}_alt", C.cast(arr, C.POINTER(C.c_void_p)))
+            self.upload_stream = torch.cuda.Stream(device=self.device)
+            io.upload_stream = self.upload_stream.cuda_stream
+            self._ev_io = [torch.cuda.Event() for _ in range(4)]
+            with torch.cuda.device(self.device):
+                for i, e in enumerate(self._ev_io):
+                    e.record(self.main_stream)
+                    (io.ev_upload if i < 2 else io.ev_compute)[i % 2] = e.cuda_event
         for name in ("q_rep", "q_blk", "k_blk", "v_blk", "out"):
             arr = (C.c_void_p * n)(*[h[name].data_ptr() for h in host_layers])
             self._io_arrays.append(arr)
