@@ -98,6 +98,7 @@ enum { kBarKFull = 0, kBarKEmpty = kBarKFull + kTcStages, kBarVFull = kBarKEmpty
        kBarSFull = kBarVEmpty + kTcStages, kBarPFull = kBarSFull + kTcSBufs, kBarPvDone = kBarPFull + kTcSBufs,
        kBarQFull = kBarPvDone + kTcSBufs, kBarVTail, kBarMerge, kBarPeerReady, kBarQkDone, kBarCount };
 constexpr int kTcMiscTmemPtr = 240;              // uint32
+constexpr int kTcMiscReady = 244;                // uint32: the word the peers' "receive buffer ready" signals land on
 constexpr int kTcMiscMax = 256;                  // bf16 [2 buffers][4 column quarters][128 rows]; float [4][128] for the row sums
 static_assert(kBarCount <= 32, "one barrier per lane of the initialising warp");
 static_assert(kBarCount * 8 <= kTcMiscTmemPtr, "barriers overlap the TMEM pointer slot");
@@ -204,6 +205,9 @@ __device__ __forceinline__ uint32_t map_to_cta(uint32_t smem_addr, uint32_t cta_
 __device__ __forceinline__ void st_async_f4(uint32_t addr, float a, float b, float c, float d, uint32_t bar_cluster) {
     asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1, %2, %3, %4}, [%5];"
                  ::"r"(addr), "f"(a), "f"(b), "f"(c), "f"(d), "r"(bar_cluster) : "memory");
+}
+__device__ __forceinline__ void st_async_u32(uint32_t addr, uint32_t v, uint32_t bar_cluster) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];" ::"r"(addr), "r"(v), "r"(bar_cluster) : "memory");
 }
 __device__ __forceinline__ void st_async_f2(uint32_t addr, float a, float b, uint32_t bar_cluster) {
     asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];"
@@ -378,16 +382,19 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(misc + kTcMiscTmemPtr), "n"(kTcTmemCols));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     } else if (warp == kTcKWarp) {
-        // one barrier per lane: every count is 1 except P-full (one arrive per softmax warp) and peer-ready (one per peer)
+        // one barrier per lane: every count is 1 except P-full (one arrive per softmax warp)
         if (lane < kBarCount) {
             const bool is_p = lane >= kBarPFull && lane < kBarPFull + kTcSBufs;
-            mbar_init(bar(lane), is_p ? kTcSoftmaxWarps : (lane == kBarPeerReady && S > 1 ? S - 1 : 1));
+            mbar_init(bar(lane), is_p ? kTcSoftmaxWarps : 1);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
         __syncwarp();
         if (lane == 0) {
             // the partial rows the other CTAs of the cluster will send (st.async, counted in bytes)
             if (merge_bytes > 0) mbar_arrive_expect_tx(bar(kBarMerge), (uint32_t)merge_bytes);
+            // ... and the 4-byte "my receive buffer is ready" signals of the S - 1 peers (asynchronous stores as well: a remote
+            // mbarrier arrive with release semantics compiles to a device-wide memory barrier)
+            if (S > 1) mbar_arrive_expect_tx(bar(kBarPeerReady), (uint32_t)(S - 1) * 4u);
         }
         if (lane < 5) {
             const CUtensorMap* tm = lane == 0 ? &tm_q : lane == 1 ? &tm_k : lane == 2 ? &tm_v : lane == 3 ? &tm_kb : &tm_vb;
@@ -652,16 +659,22 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 if (lane == 0) mbar_arrive(bar(kBarPFull + sb));
                 if (tid == 0) HERALD_STAMP(8 + 4 * jg + 2);
             }
-            // the verdict (the last PV is still running): row sums of e and e^2 over the four column quarters
-            ex_sum[cq * 128 + row] = l_run;
-            named_bar_sync(1 + quarter, 128);
-            const float l_row = (ex_sum[row] + ex_sum[128 + row]) + (ex_sum[256 + row] + ex_sum[384 + row]);
-            named_bar_sync(1 + quarter, 128);
-            ex_sum[cq * 128 + row] = q_run;
-            named_bar_sync(1 + quarter, 128);
-            const float q_row = (ex_sum[row] + ex_sum[128 + row]) + (ex_sum[256 + row] + ex_sum[384 + row]);
-            named_bar_sync(1 + quarter, 128);      // (the exact pass and the merge reuse this buffer)
-            if (!(q_row <= kTcFastCmax * l_row * l_row)) jumped = true;
+            // the verdict (the last PV is still running): row sums of e and e^2 over the four column quarters, exchanged as one
+            // bf16 pair per thread (the sum rounded down, the sum of squares rounded up: the test stays on the safe side)
+            {
+                uint32_t* ex_pair = reinterpret_cast<uint32_t*>(ex_max);
+                const __nv_bfloat16 lb = __float2bfloat16_rd(l_run), qb = __float2bfloat16_ru(q_run);
+                ex_pair[cq * 128 + row] = (uint32_t)__bfloat16_as_ushort(lb) | ((uint32_t)__bfloat16_as_ushort(qb) << 16);
+                named_bar_sync(1 + quarter, 128);
+                float l_row = 0.f, q_row = 0.f;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const uint32_t v = ex_pair[c * 128 + row];
+                    l_row += __uint_as_float(v << 16);
+                    q_row += __uint_as_float(v & 0xffff0000u);
+                }
+                if (!(q_row <= kTcFastCmax * l_row * l_row)) jumped = true;
+            }
         } else {
             // =========================== softmax warps, exact pass ===========================
             m_used = -INFINITY, l_run = 0.f;
@@ -779,7 +792,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     if (warp == kTcKWarp && S > 1) {
         if (nt > 0) mbar_wait(bar(kBarQkDone), (n_passes - 1) & 1);   // the last pass has read its last K tile
         cluster_wait_all();   // every CTA of the cluster has initialised its barriers (only this warp arrives on a peer's before it is told to)
-        if (lane < S - 1) mbar_arrive_remote(map_to_cta(bar(kBarPeerReady), lane < split ? lane : lane + 1));
+        if (lane < S - 1) {
+            const uint32_t peer = lane < split ? lane : lane + 1;
+            st_async_u32(map_to_cta(misc + kTcMiscReady, peer), 1u, map_to_cta(bar(kBarPeerReady), peer));
+        }
     }
     // the next kernel of the stream may be scheduled from here on: its blocks take the SMs as this grid's blocks exit
     asm volatile("griddepcontrol.launch_dependents;");
