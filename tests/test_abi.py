@@ -187,3 +187,40 @@ def test_pipeline_arguments_are_validated_before_anything_is_enqueued(H):
     expect(H.ERR_INVALID_ARG)
     p.retrieval_stream = 1
     expect(H.ERR_INVALID_ARG)
+
+
+def test_host_io_double_buffering_is_validated(H):
+    """herald_pipeline_step_host: the optional second buffer sets need their streams and events; nothing is enqueued otherwise."""
+    shape = H.make_shape(2, 8, 4, 16, 1024, 64, 64)
+    layers = (H.Layer * 1)()
+    ly = layers[0]
+    ly.cache = H.Cache(256, 256, 16 * 4 * 128, 4 * 128, 128, 256, 256)
+    ly.q_rep = ly.k_per_seq = ly.q_blk = ly.k_blk = ly.v_blk = ly.out = 256
+    for j in range(2):
+        ly.pool_k[j] = ly.pool_v[j] = ly.pool_len[j] = 256
+    p = H.Pipeline()
+    p.shape, p.n_layers, p.n_steps, p.start_after_step, p.active = shape, 1, 3, 0, 0
+    p.layers = C.cast(layers, C.POINTER(H.Layer))
+    p.sel_idx = p.ws_select = p.ws_attn = 256
+    p.ws_select_bytes = p.ws_attn_bytes = 1 << 30
+    p.main_stream, p.retrieval_stream, p.ev_fork, p.ev_join = 1, 2, 256, 256
+    one = (C.c_void_p * 1)(256)
+    ptrs = C.cast(one, C.POINTER(C.c_void_p))
+    io = H.HostIO()
+    io.host_q_rep = io.host_q_blk = io.host_k_blk = io.host_v_blk = io.host_out = ptrs
+    def expect_invalid():
+        with pytest.raises(H.HeraldError) as ei:
+            H.herald_pipeline_step_host(p, io)
+        assert ei.value.code == H.ERR_INVALID_ARG, str(ei.value)
+        assert p.active == 0
+    io.dev_out_alt = ptrs                    # a second output set without its events
+    expect_invalid()
+    io.ev_download[0] = io.ev_download[1] = 256
+    io.dev_q_blk_alt = ptrs                  # a second input set without the other arrays / the upload stream
+    expect_invalid()
+    io.dev_q_rep_alt = io.dev_k_blk_alt = io.dev_v_blk_alt = ptrs
+    expect_invalid()                         # ... still no upload stream and events
+    io.host_out = C.cast((C.c_void_p * 1)(None), C.POINTER(C.c_void_p))
+    io.dev_out_alt = None
+    io.dev_q_blk_alt = None
+    expect_invalid()                         # a NULL host pointer for layer 0

@@ -313,3 +313,31 @@ def test_fused_retrieval_chained_in_one_graph(H, cuda):
                 assert np.array_equal(synth.to_u16(pools_v[r][b])[:, :n], pv_o[0][:, :n]), (it, r, b)
                 if it == 0:
                     _check_attn("chain", {k: v for k, v in inp.items()}, b, r, pools_k[r], pools_v[r], pl_o, outs[r])
+
+
+def test_pipeline_tune_keeps_results_and_reports_its_table(H, cuda):
+    """herald_pipeline_tune (C ABI): times a handful of schedules with complete block steps, leaves the fastest one set, and
+    changes nothing in what the pipeline computes -- the block after the calibration attends over exactly the oracle's pool."""
+    w = synth.Workload("tune", 4, (20000, 12345, 8000, 16384), 28, 4, 32, 6, 50, "planted", 16)
+    inp = synth.make_inputs(w, seed=4242, device=cuda)
+    ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
+    cap = max(ks) + w.block_size
+    pipe = H.BlockPipeline(_shape(H, w, inp, cap), [_layer(w, inp, ks, cuda)], w.n_attn_steps, 0, cuda)
+    pipe.step()
+    table = pipe.tune_schedule(reps=2)
+    assert len(table) >= 4
+    chosen = f"{pipe.c.scan_ctas}/{pipe.c.start_after_step}/{pipe.c.scan_head_permille}"
+    assert chosen in table and table[chosen] == min(table.values())
+    assert any(k.split("/")[2] != "0" for k in table), "the head start of the scan was not among the candidates"
+    # a head start forced on: the scan runs in two launches, the histogram accumulates over both
+    pipe.c.scan_ctas, pipe.c.start_after_step, pipe.c.scan_head_permille = 20, 0, 350
+    pipe.step()
+    act = pipe.active
+    pipe.step()
+    torch.cuda.synchronize()
+    differing = 0
+    for b in range(w.batch):
+        pl_o, d = _check_unit_pools("tune", w, inp, b, ks, cap, pipe.pools_k[0][act], pipe.pools_v[0][act], pipe.pool_lens[0][act], cuda)
+        differing += d
+        _check_attn("tune", inp, b, 1, pipe.pools_k[0][act], pipe.pools_v[0][act], pl_o, pipe.outs[0][1])
+    assert differing <= 2
