@@ -346,6 +346,23 @@ class Rig:
         return (mean(e4[0].elapsed_time(e4[1]) for e4 in prof_events), mean(e4[1].elapsed_time(e4[2]) for e4 in prof_events),
                 mean(e4[2].elapsed_time(e4[3]) for e4 in prof_events))
 
+    def retrieval_time(self, n_sets=8):
+        """The retrieval stream of a block step from its first kernel to the end of its last (two events, eager steps)."""
+        H = self.H
+        evs, profs = [], []
+        for _ in range(n_sets):
+            e2 = [self.ev(), self.ev()]
+            for e in e2:
+                e.record(self.pipe.retrieval_stream)
+            evs.append(e2)
+            profs.append(H.Profile(e2[0].cuda_event, None, None, e2[1].cuda_event))
+        for i in range(n_sets):
+            H.herald_pipeline_set_profile(profs[i])
+            self.pipe.step()
+        self.torch.cuda.synchronize()
+        H.herald_pipeline_set_profile(None)
+        return statistics.mean(a.elapsed_time(b) for a, b in evs)
+
     def time_isolated(self, fn, reps=20, warm=3, timed=5):
         """ms per call of `fn`: `reps` calls captured in one CUDA graph (no host launch cost between them), replayed."""
         torch, side = self.torch, self.side
@@ -484,14 +501,14 @@ def fig14_sweep(H, synth, torch, dev, seed, scan_ctas):
             rig.pipe.c.start_after_step = start
             rig.graphs = None
             rig.warm(2)
-            scan_ms, topk_ms, gather_ms = rig.stage_times(4)
+            retr_ms = rig.retrieval_time(4)
             rig.capture()
             reg = sorted(rig.time_block(6) for _ in range(3))
             if iso_attn is None:
                 iso_attn = rig.isolated_stages()["attn_step_alone_ms"]
             main_ms = iso_attn * rig.n_steps
             rows.append({"T": T, "start_after_step": start, "block_latency_ms": statistics.median(reg),
-                         "main_stream_alone_ms": main_ms, "retrieval_stream_ms": scan_ms + topk_ms + gather_ms,
+                         "main_stream_alone_ms": main_ms, "retrieval_stream_ms": retr_ms,
                          "exposed_ms": statistics.median(reg) - main_ms,
                          "bound": "retrieval" if statistics.median(reg) - main_ms > 0.05 * statistics.median(reg) else "main"})
         del rig
@@ -571,6 +588,7 @@ def main():
     regions_sorted = sorted(regions)
 
     scan_ms, topk_ms, gather_ms = rig.stage_times(8)
+    retrieval_ms = rig.retrieval_time(8)
     iso = rig.isolated_stages(cold_attention=True)
     cache, sel_idx, sel_cnt, ws_sel, ws_att, out1, side = rig.cache, rig.sel_idx, rig.sel_cnt, rig.ws_sel, rig.ws_att, rig.out1, rig.side
     k_per_seq = rig.k_per_seq
@@ -758,7 +776,9 @@ def main():
         "scan_gbs_eager_events": rig.scan_bytes / (iso["scan_kernel_eager_events_ms"] * 1e-3) / 1e9,
         "topk_kernel_eager_events_ms": iso["topk_kernel_eager_events_ms"],
         "scan_gbs_in_pipeline": scan_gbs_live, "scan_ms_in_pipeline": scan_ms, "topk_ms_in_pipeline": topk_ms,
-        "gather_ms_in_pipeline": gather_ms, "select_alone_ms": select_alone_block_ms,
+        "gather_ms_in_pipeline": gather_ms,
+        "retrieval_stream_ms_in_pipeline": retrieval_ms,
+        "select_alone_ms": select_alone_block_ms,
         "gather_alone_ms": gather_alone_ms, "gather_gbs_alone": rig.gather_bytes / (gather_alone_ms * 1e-3) / 1e9,
         "attn_step_alone_ms": attn_alone_ms, "attn_tflops_alone": attn_tflops_step,
         "attn_step_l2_cold_ms": iso.get("attn_step_l2_cold_ms"), "attn_step_l2_cold_min_ms": iso.get("attn_step_l2_cold_min_ms"),
