@@ -12,39 +12,41 @@
 //   grid    = (KV splits S, M tiles, units); the S CTAs of one (unit, M tile) form a thread-block cluster
 //   M tile  = `ipt` block rows x G heads (row r = block row r/G, head r%G; at most 128 rows), so the Q tile
 //             is one TMA box of q_blk; rows past ipt*G are zeros
-//   TMEM    = three S/P tiles of 128 columns + O (128 columns): QK^T runs two tiles ahead of PV, so the softmax
+//   TMEM    = three S/P tiles of 128 columns + O (128 columns): QK^T runs up to three tiles ahead of PV, so the softmax
 //             warps never wait for the tensor pipe and the pipe never waits for one softmax
-//   keys    = key tile 0 holds the B in-block rows (one TMA box of k_blk / v_blk), key tile t >= 1 holds pool rows
-//             [128(t-1), 128t) (one TMA box of the pool; softmax is invariant to the key order)
-//             (dense mode, herald_dense_attn: tile t >= 1 holds tokens [128(t-1), 128t) of the paged cache itself, one
+//   keys    = key tile t < n_pool_tiles holds pool rows [128t, 128t+128) (one TMA box of the pool), the last tile the B
+//             in-block rows (one TMA box of k_blk / v_blk); softmax is invariant to the key order
+//             (dense mode, herald_dense_attn: tile t holds tokens [128t, 128t+128) of the paged cache itself, one
 //             TMA box per 16-token page)
 //   warp 16   K producer (+ Q): tiles arrive by TMA (cp.async.bulk.tensor, 128B swizzle) into a 3-stage ring; a
-//             stage is released as soon as QK^T has read it.  Rows past the valid keys of a tile (stale pool rows,
-//             zero fill) give logits that the softmax masks.
-//   warp 17   V producer, same, released after PV.  Where the valid keys of a tile are not a multiple of the MMA
-//             k-step (16), it zeroes the few V rows up to the next multiple after the box has landed (P is 0 there,
-//             but 0 x NaN would poison O).
-//   warp 18   issues the MMAs (one elected lane, descriptors precomputed so the issue keeps up with the
-//             tensor pipe): S[j%3] = Q K_j^T, then O += P_{j-2} V_{j-2} with P read from TMEM; tcgen05.commit -> mbarrier
-//   warps 0-15 softmax: thread (row, column quarter) reads 32 logits of its row from TMEM (tcgen05.ld),
-//             exchanges the row maximum with the three warps that hold the rest of the row, exponentiates (ex2),
-//             accumulates the row sum, and writes P back over S_j in TMEM (tcgen05.st).  The running maximum
-//             is only raised when it grows by more than 2^kTcRescaleThreshold ("lazy rescale"; P, l and O are
-//             fp32/bf16-ranged, so the threshold only guards overflow): O in TMEM is then rescaled in place.
-//   precision modes.  EXACT: as above (P = bf16 hi + lo, the row maximum exchanged at every tile, O rescaled in place when
-//             it moves by more than 2^40).  FAST, tried first by blocks whose share of the keys is >= 1536 long: P is ONE bf16
-//             (8 PV MMAs per tile instead of 16; the TMEM-operand MMAs are the slower kind) and the row keeps the reference of
-//             its first tile without another exchange (any logit up to 2^100 above it is still far inside fp32), so the softmax
-//             warps run free of each other.  Because they no longer meet, a thread may only overwrite S columns it has read
-//             itself: P_hi goes to the first 16 of its own 32 S columns.
+//             stage is free as soon as QK^T has read it (the S-full barrier of that tile).  Rows past the valid keys of a
+//             tile (stale pool rows, zero fill) give logits that the softmax masks.
+//   warp 17   V producer, same, a stage is free after PV (its PV-done barrier).  Where the valid keys of a tile are not a
+//             multiple of the MMA k-step (16), it zeroes the few V rows up to the next multiple after the box has landed
+//             (P is 0 there, but 0 x NaN would poison O).
+//   warp 18   issues S[j%3] = Q K_j^T (one elected lane; tcgen05.commit -> mbarrier) once PV_{j-3} has finished with those
+//             TMEM columns; owns the TMEM allocation
+//   warp 19   issues O += P_j V_j with P read from TMEM.  One warp per product: a tcgen05.mma costs its issuing warp ~45
+//             cycles and every barrier poll or commit ~100, which for one warp doing both products (24 MMAs, 4 commits, 3
+//             polls per tile) came to 2.25k cycles per tile against 1.56k of tensor-pipe time.
+//   warps 0-15 softmax: thread (row, column quarter) reads 32 logits of its row from TMEM (tcgen05.ld), exponentiates
+//             (ex2) against the row reference of the pass, accumulates the row sum, and writes P back over its own 32 S
+//             columns (tcgen05.st).  The reference is fixed before the first exponential of a pass -- the maximum of the
+//             pass's first tile, exchanged once among the four warps that hold the row -- so inside the loop no warp waits
+//             for another and the four warps of a scheduler hide each other's TMEM and barrier round trips.  A logit may
+//             rise 2^64 above the reference before P, l or O leave fp32; if one does (or if the fast pass's row statistics
+//             fail, below), the block votes, takes the row maximum it has seen as the reference and goes through its tiles a
+//             second time, which cannot fail.
+//   precision modes.  EXACT: P = bf16 hi + lo (two MMAs per k-step).  FAST, tried first by blocks whose share of the keys is
+//             >= 1536 long: P is ONE bf16 (8 PV MMAs per tile instead of 16).
 //             Rounding a weight to 8 significant bits moves an output element by sum_i eps_i p_i v_i with |eps_i| <= 2^-8,
 //             pseudo-random: standard deviation <= 2^-8 sqrt(sum_i p_i^2) rms(v) / sqrt(3).  The fast pass accumulates
 //             sum_i e_i^2 per row next to the row sum and is ACCEPTED only if every row of the block has sum_i p_i^2 <= 1/64
 //             (<= 2.8e-4 rms(v) per element, 7 sigma inside the 2e-3 bar; one key alone may then weigh at most 1/8; flat rows
-//             over n keys have sum p^2 ~ e/n) and no logit rose past the 2^100 margin.  Otherwise the block goes through its
-//             tiles once more the exact way (a block-wide vote, taken while the last PV is still running) and leaves a note
-//             in the workspace that makes it start exact for its next 16 launches.  Blocks with short key shares never try:
-//             among a few hundred keys a 5-sigma logit already breaks the criterion, and one redone block delays its launch.
+//             over n keys have sum p^2 ~ e/n) and no logit rose past its 2^30 margin.  Otherwise the block goes through its
+//             tiles once more with the pair and leaves a note in the workspace: two failures in a row make it start with
+//             the pair for its next 16 launches.  Blocks with short key shares never try: among a few hundred keys a
+//             5-sigma logit already breaks the criterion, and one redone block delays its launch.
 //   merge     split-KV partials never leave the chip: tile row r is owned by CTA r / rows_own of the cluster; the
 //             other CTAs write their unnormalised O rows and (max, sum) straight from registers into the owner's
 //             shared memory (st.shared::cluster into the owner's K ring, which its last QK^T has released: every CTA
@@ -55,6 +57,8 @@
 #pragma once
 #include <cuda.h>
 
+#include <type_traits>
+
 #include "common.cuh"
 
 namespace herald {
@@ -64,8 +68,9 @@ constexpr int kTcBN = 128;                       // keys per tile (UMMA N of QK^
 constexpr int kTcStages = 3;                     // depth of the K ring and of the V ring
 constexpr int kTcSBufs = 3;                      // S/P tiles in TMEM
 constexpr int kTcSoftmaxWarps = 16;              // 4 row quarters (TMEM lane quarters) x 4 column quarters
-constexpr int kTcKWarp = 16, kTcVWarp = 17, kTcMmaWarp = 18;
-constexpr int kTcThreads = 19 * 32;
+constexpr int kTcKWarp = 16, kTcVWarp = 17, kTcMmaWarp = 18, kTcPvWarp = 19;   // warp 18 issues QK^T (and owns TMEM), warp 19 issues PV
+constexpr int kTcThreads = 20 * 32;
+static_assert(kTcStages == kTcSBufs, "a ring stage falls free on the S-full / PV-done barrier of the same index");
 constexpr int kTcMaxSplits = 8;                  // portable cluster size
 constexpr int kTcHalfBytes = kTcBN * 128;        // one [128 rows x 64 el] swizzled half tile (16 KB)
 constexpr int kTcTileBytes = 2 * kTcHalfBytes;   // a [128 x 128] bf16 tile = two halves (32 KB)
@@ -77,10 +82,10 @@ constexpr int kTcMiscBytes = 2304;
 constexpr int kTcSmemBytes = kTcSmemMisc + kTcMiscBytes;                 // 231,680 B of the 232,448 B a CTA may own
 constexpr int kTcTmemCols = 512;                 // S0/P0 [0,128) S1/P1 [128,256) S2/P2 [256,384) O [384,512)
 constexpr int kTcTmemO = kTcSBufs * 128;
-constexpr float kTcRescaleThreshold = 40.f;      // log2 units
+constexpr float kTcExactJump = 64.f;             // log2 units a logit may rise above the reference of a pass with the hi + lo pair (P, l, O stay inside fp32)
 // fast pass ("precision modes" in the header comment)
 constexpr int kTcFastMinKeys = 1536;             // a block tries the fast pass only if its share of the keys is at least this long
-constexpr float kTcFastJump = 100.f;             // log2 units a logit may rise above the first tile's row maximum (P, l, O stay far inside fp32)
+constexpr float kTcFastJump = 30.f;              // the same for the fast pass, which also sums squares of the weights
 constexpr float kTcFastCmax = 1.f / 64.f;        // bound on sum_i p_i^2 of a row for single-bf16 weights
 constexpr uint32_t kTcHintMagic = 0x45580000u;   // note word of a block: "EX" | failures in a row << 8 | launches still to start exact
 constexpr uint32_t kTcHintBackoff = 16;          // after two failed fast passes in a row a block starts exact for this many launches
@@ -94,8 +99,8 @@ static_assert(kTcRecvML + (kTcBM + 2 * kTcMaxSplits) * 8 <= kTcSmemV, "receive b
 static_assert(kTcBM * kTcRowFloats * 4 <= kTcStages * kTcTileBytes, "output staging must fit in the V ring");
 
 // barrier slots (8 bytes each) inside the misc area
-enum { kBarKFull = 0, kBarKEmpty = kBarKFull + kTcStages, kBarVFull = kBarKEmpty + kTcStages, kBarVEmpty = kBarVFull + kTcStages,
-       kBarSFull = kBarVEmpty + kTcStages, kBarPFull = kBarSFull + kTcSBufs, kBarPvDone = kBarPFull + kTcSBufs,
+enum { kBarKFull = 0, kBarVFull = kBarKFull + kTcStages,
+       kBarSFull = kBarVFull + kTcStages, kBarPFull = kBarSFull + kTcSBufs, kBarPvDone = kBarPFull + kTcSBufs,
        kBarQFull = kBarPvDone + kTcSBufs, kBarVTail, kBarMerge, kBarPeerReady, kBarQkDone, kBarCount };
 constexpr int kTcMiscTmemPtr = 240;              // uint32
 constexpr int kTcMiscReady = 244;                // uint32: the word the peers' "receive buffer ready" signals land on
@@ -458,11 +463,12 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     const uint32_t lane_base = tmem + ((uint32_t)(quarter * 32) << 16);
     float m_used = -INFINITY, l_run = 0.f;   // running max (log2 units) and the sum of this thread's quarter row
     float q_run = 0.f;                       // fast pass: the sum of the squared weights of this thread's quarter row
-    bool jumped = false;                     // fast pass: this thread's rows fail its criteria
+    bool jumped = false;                     // this thread's rows fail the criteria of the pass
+    float mx_all = -INFINITY;                // the largest logit this thread has seen (raw, before the scale)
 
-    // One pass over the key tiles, or two (header comment, "precision modes"): blocks with a long share of the keys try the
-    // fast pass first; if its row statistics fail, every role goes through the same tiles once more the exact way.  Ring and
-    // TMEM barrier phases simply run on: tile j of the second pass is pipeline step jb + j.
+    // One pass over the key tiles, or two (header comment, "softmax" and "precision modes"): if the pass fails its criteria,
+    // every role goes through the same tiles once more.  Ring and TMEM barrier phases simply run on: tile j of the second pass
+    // is pipeline step jb + j.
     int keys_here = 0;
     if (kTryFast)
         for (int j = 0; j < nt; ++j) keys_here += tile_valid(j);
@@ -477,14 +483,15 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     const bool tried_fast = fast;
     int n_fixed = 0;                         // V tiles whose tail rows were zeroed so far (phase of kBarVTail; V producer)
     int jb_rt = 0;
-#define HERALD_JB (kTryFast ? jb_rt : 0)
+#define HERALD_JB jb_rt
     for (int pass = 0; nt > 0; ++pass) {
         if (warp == kTcKWarp || warp == kTcVWarp) {
             // =========================== producers: one warp streams K tiles (and Q), one streams V tiles ===========================
             const bool is_k = warp == kTcKWarp;
             const CUtensorMap* map = is_k ? &tm_k : &tm_v;
             const CUtensorMap* map_blk = is_k ? &tm_kb : &tm_vb;
-            const int bar_full = is_k ? kBarKFull : kBarVFull, bar_empty = is_k ? kBarKEmpty : kBarVEmpty;
+            // a K stage is free once QK^T has read it (= S of that tile is full), a V stage once PV has (= PV done): same index, same phase
+            const int bar_full = is_k ? kBarKFull : kBarVFull, bar_empty = is_k ? kBarSFull : kBarPvDone;
             const uint32_t ring = sbase + (is_k ? kTcSmemK : kTcSmemV);
             uint8_t* ring_gen = sgen + (is_k ? kTcSmemK : kTcSmemV);
             // dense mode: the page ids of a tile are fetched one tile ahead, so that their round trip does not sit between a
@@ -544,12 +551,21 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                 }
             }
         } else if (warp == kTcMmaWarp) {
-            // =========================== MMA issuer ===========================
-            constexpr uint32_t idesc_pv = umma_idesc(/*A bf16*/ 1, /*B bf16*/ 1, /*A K-major*/ 0, /*B MN-major*/ 1, kTcBM, kHeadDim);
+            // =========================== QK^T issuer ===========================
+            // Two warps feed the tensor pipe, one per product: what an issuing warp does between its MMAs (barrier polls,
+            // commits, descriptor set-up: about 1.1k cycles per tile next to 1.1k of issue) was longer than the pipe's own
+            // 1.56k per tile while one warp did both.  The pipe no longer orders S_j after the PV that read the same TMEM
+            // columns three tiles earlier, so this warp waits for that PV's completion barrier.
             constexpr uint32_t hi_k = umma_desc_hi(1024);
             const uint32_t q_lo = umma_desc_lo(sbase + kTcSmemQ, 16);
-            auto issue_qk = [&](int j) {   // S_j = Q K_j^T into S buffer j % 3 (it held P_{j-3}: PV_{j-3} was issued before, the pipe runs in order)
+            if (pass == 0) {
+                mbar_wait(bar(kBarQFull), 0);
+                if (lane == 0) HERALD_GSTAMP(57);
+            }
+#pragma unroll 1
+            for (int j = 0; j < nt; ++j) {   // S_j = Q K_j^T into S buffer j % 3, which held P_{j-3}
                 const int jg = HERALD_JB + j, stage = jg % kTcStages, sb = jg % kTcSBufs;
+                if (jg >= kTcSBufs) mbar_wait(bar(kBarPvDone + sb), ((jg / kTcSBufs) - 1) & 1);
                 mbar_wait(bar(kBarKFull + stage), (jg / kTcStages) & 1);
                 tc_fence_after();
                 if (lane == 0) { HERALD_STAMP(8 + 4 * jg); if (jg == 0) HERALD_GSTAMP(58); }
@@ -563,13 +579,17 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                         if (ks == 0) umma_ss<false>(s_base, q_lo + off, hi_k, k_lo + off, hi_k, idesc_s);
                         else umma_ss<true>(s_base, q_lo + off, hi_k, k_lo + off, hi_k, idesc_s);
                     }
-                    umma_commit(bar(kBarSFull + sb));
-                    umma_commit(bar(kBarKEmpty + stage));
+                    umma_commit(bar(kBarSFull + sb));                // S_j is complete; K stage j % 3 has been read
                     if (j == nt - 1) umma_commit(bar(kBarQkDone));   // every QK^T of this pass has read its K tile (phase = pass)
                 }
                 __syncwarp();
-            };
-            auto issue_pv = [&](int j) {   // O (+)= (P_hi + P_lo)_j V_j, P read from TMEM (it overlays S_j)
+            }
+        } else if (warp == kTcPvWarp) {
+            // =========================== PV issuer ===========================
+            constexpr uint32_t idesc_pv = umma_idesc(/*A bf16*/ 1, /*B bf16*/ 1, /*A K-major*/ 0, /*B MN-major*/ 1, kTcBM, kHeadDim);
+            constexpr uint32_t hi_k = umma_desc_hi(1024);
+#pragma unroll 1
+            for (int j = 0; j < nt; ++j) {   // O (+)= (P_hi + P_lo)_j V_j, P read from TMEM (it overlays S_j)
                 const int jg = HERALD_JB + j, stage = jg % kTcStages, sb = jg % kTcSBufs;
                 mbar_wait(bar(kBarVFull + stage), (jg / kTcStages) & 1);
                 mbar_wait(bar(kBarPFull + sb), (jg / kTcSBufs) & 1);
@@ -579,89 +599,108 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                     const uint32_t v_lo = umma_desc_lo(sbase + kTcSmemV + stage * kTcTileBytes, kTcHalfBytes);
                     const uint32_t p_base = tmem + sb * 128, o_base = tmem + kTcTmemO;
                     const int ksteps = tile_cols(j) >> 4;
+                    const uint32_t acc0 = j > 0 ? 1u : 0u;
                     if (kTryFast && fast) {     // one bf16 per weight, at the head of each column quarter's own S columns
-                        for (int kk = 0; kk < ksteps; ++kk)
-                            umma_ts(o_base, p_base + (kk >> 1) * 32 + (kk & 1) * 8, v_lo + kk * 128, hi_k, idesc_pv, (j > 0 || kk > 0) ? 1u : 0u);
+                        if (ksteps == 8) {
+#pragma unroll
+                            for (int kk = 0; kk < 8; ++kk)
+                                umma_ts(o_base, p_base + (kk >> 1) * 32 + (kk & 1) * 8, v_lo + kk * 128, hi_k, idesc_pv, kk > 0 ? 1u : acc0);
+                        } else {
+                            for (int kk = 0; kk < ksteps; ++kk)
+                                umma_ts(o_base, p_base + (kk >> 1) * 32 + (kk & 1) * 8, v_lo + kk * 128, hi_k, idesc_pv, kk > 0 ? 1u : acc0);
+                        }
                     } else if (ksteps == 8) {
 #pragma unroll
                         for (int kk = 0; kk < 8; ++kk) {
-                            umma_ts(o_base, p_base + kk * 8, v_lo + kk * 128, hi_k, idesc_pv, (j > 0 || kk > 0) ? 1u : 0u);
-                            umma_ts(o_base, p_base + 64 + kk * 8, v_lo + kk * 128, hi_k, idesc_pv, 1u);
+                            umma_ts(o_base, p_base + (kk >> 1) * 32 + (kk & 1) * 8, v_lo + kk * 128, hi_k, idesc_pv, kk > 0 ? 1u : acc0);
+                            umma_ts(o_base, p_base + (kk >> 1) * 32 + (kk & 1) * 8 + 16, v_lo + kk * 128, hi_k, idesc_pv, 1u);
                         }
                     } else {
                         for (int kk = 0; kk < ksteps; ++kk) {
-                            umma_ts(o_base, p_base + kk * 8, v_lo + kk * 128, hi_k, idesc_pv, (j > 0 || kk > 0) ? 1u : 0u);
-                            umma_ts(o_base, p_base + 64 + kk * 8, v_lo + kk * 128, hi_k, idesc_pv, 1u);
+                            umma_ts(o_base, p_base + (kk >> 1) * 32 + (kk & 1) * 8, v_lo + kk * 128, hi_k, idesc_pv, kk > 0 ? 1u : acc0);
+                            umma_ts(o_base, p_base + (kk >> 1) * 32 + (kk & 1) * 8 + 16, v_lo + kk * 128, hi_k, idesc_pv, 1u);
                         }
                     }
-                    umma_commit(bar(kBarPvDone + sb));
-                    umma_commit(bar(kBarVEmpty + stage));
+                    umma_commit(bar(kBarPvDone + sb));               // P_j and V stage j % 3 have been read
                 }
                 __syncwarp();
+            }
+        } else {
+            // =========================== softmax warps ===========================
+            // The warps run free of each other: the row reference is fixed before the first exponential of a pass (pass 0:
+            // the maximum of the first tile, exchanged once among the four column quarters; pass 1: the row maximum that
+            // pass 0 saw), so no thread waits for another one inside the loop and the four warps of a scheduler hide each
+            // other's TMEM and barrier round trips.  Because they no longer meet, a thread may only overwrite S columns it
+            // has read itself: its 32 weights go to its own 32 S columns, P_hi in the first 16, P_lo in the last 16.
+            auto softmax_pass = [&](auto single_tag) {
+                constexpr bool kSingle = decltype(single_tag)::value;   // one bf16 per weight (fast pass) or the hi + lo pair
+                constexpr float kJump = kSingle ? kTcFastJump : kTcExactJump;
+                for (int j = 0; j < nt; ++j) {
+                    const int jg = jb_rt + j, sb = jg % kTcSBufs;
+                    mbar_wait(bar(kBarSFull + sb), (jg / kTcSBufs) & 1);
+                    tc_fence_after();
+                    if (tid == 0) { HERALD_STAMP(8 + 4 * jg + 1); if (jg == 0) HERALD_GSTAMP(62); }
+                    float s[32];
+                    tmem_ld32_async(lane_base + sb * 128 + cq * 32, s);
+                    tmem_wait_ld();
+                    const int valid = tile_valid(j);
+                    if (valid < kTcBN) {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i)
+                            if (cq * 32 + i >= valid) s[i] = -INFINITY;
+                    }
+                    float mx = fmax3(s[0], s[1], s[2]);
+#pragma unroll
+                    for (int i = 3; i + 1 < 32; i += 2) mx = fmax3(mx, s[i], s[i + 1]);
+                    mx = fmaxf(mx, s[31]);
+                    mx_all = fmaxf(mx_all, mx);
+                    if (j == 0 && pass == 0) {
+                        // the reference only has to be common to the four column quarters: it is exchanged rounded up to bf16
+                        ex_max[cq * 128 + row] = __float2bfloat16_ru(mx);
+                        named_bar_sync(1 + quarter, 128);             // the four warps that hold these 32 rows
+                        float mrow = __bfloat162float(ex_max[row]);
+#pragma unroll
+                        for (int c = 1; c < 4; ++c) mrow = fmaxf(mrow, __bfloat162float(ex_max[c * 128 + row]));
+                        m_used = mrow * p.scale_log2;
+                    } else if (mx * p.scale_log2 > m_used + kJump) {
+                        jumped = true;    // the reference cannot move without the other quarters: the block goes through its tiles again
+                    }
+                    // The exponentials (MUFU, 16 per clock and SM: the scarce unit) and the splitting arithmetic of earlier
+                    // pairs share one unrolled loop so that the scheduler interleaves them.
+                    float sum0 = 0.f, sum1 = 0.f, sq0 = 0.f, sq1 = 0.f;
+                    uint32_t hi[16], lo[kSingle ? 1 : 16];
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) {
+                        float x0, x1;
+                        ffma2(x0, x1, s[2 * i], s[2 * i + 1], p.scale_log2, -m_used);
+                        const float e0 = fast_exp2(x0), e1 = fast_exp2(x1);
+                        fadd2(sum0, sum1, sum0, sum1, e0, e1);
+                        hi[i] = pack_bf16(e0, e1);
+                        if (kSingle) {
+                            ffma2w(sq0, sq1, e0, e1, e0, e1, sq0, sq1);
+                        } else {
+                            float r0, r1;
+                            ffma2v(r0, r1, __uint_as_float(hi[i] << 16), __uint_as_float(hi[i] & 0xffff0000u), -1.f, e0, e1);   // e - hi, exact
+                            lo[i] = pack_bf16(r0, r1);
+                        }
+                    }
+                    l_run += sum0 + sum1;
+                    if (kSingle) q_run += sq0 + sq1;
+                    // A operand of the PV MMA: row = lane, two keys per 32-bit column
+                    tmem_st16(lane_base + sb * 128 + cq * 32, hi);
+                    if (!kSingle) tmem_st16(lane_base + sb * 128 + cq * 32 + 16, lo);
+                    tmem_wait_st();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar(kBarPFull + sb));
+                    if (tid == 0) HERALD_STAMP(8 + 4 * jg + 2);
+                }
             };
-            if (pass == 0) {
-                mbar_wait(bar(kBarQFull), 0);
-                if (lane == 0) HERALD_GSTAMP(57);
-            }
-#pragma unroll 1
-            for (int j = -2; j < nt; ++j) {   // QK^T runs two tiles ahead of PV
-                if (j + 2 < nt) issue_qk(j + 2);
-                if (j >= 0) issue_pv(j);
-            }
-        } else if (kTryFast && fast) {
-            // =========================== softmax warps, fast pass ===========================
-            m_used = -INFINITY, l_run = 0.f, q_run = 0.f, jumped = false;
-            for (int j = 0; j < nt; ++j) {
-                const int jg = HERALD_JB + j, sb = jg % kTcSBufs;
-                mbar_wait(bar(kBarSFull + sb), (jg / kTcSBufs) & 1);
-                tc_fence_after();
-                if (tid == 0) { HERALD_STAMP(8 + 4 * jg + 1); if (jg == 0) HERALD_GSTAMP(62); }
-                float s[32];
-                tmem_ld32_async(lane_base + sb * 128 + cq * 32, s);
-                tmem_wait_ld();
-                const int valid = tile_valid(j);
-                if (valid < kTcBN) {
-#pragma unroll
-                    for (int i = 0; i < 32; ++i)
-                        if (cq * 32 + i >= valid) s[i] = -INFINITY;
-                }
-                float mx = fmax3(s[0], s[1], s[2]);
-#pragma unroll
-                for (int i = 3; i + 1 < 32; i += 2) mx = fmax3(mx, s[i], s[i + 1]);
-                mx = fmaxf(mx, s[31]);
-                if (j == 0) {   // the row reference: the maximum of the first tile, common to the four column quarters
-                    ex_max[cq * 128 + row] = __float2bfloat16_ru(mx);
-                    named_bar_sync(1 + quarter, 128);
-                    float mrow = __bfloat162float(ex_max[row]);
-#pragma unroll
-                    for (int c = 1; c < 4; ++c) mrow = fmaxf(mrow, __bfloat162float(ex_max[c * 128 + row]));
-                    m_used = mrow * p.scale_log2;
-                } else if (mx * p.scale_log2 > m_used + kTcFastJump) {
-                    jumped = true;        // the reference cannot move without the other quarters: the block goes through its tiles again
-                }
-                float sum0 = 0.f, sum1 = 0.f, sq0 = 0.f, sq1 = 0.f;
-                uint32_t hi[16];
-#pragma unroll
-                for (int i = 0; i < 16; ++i) {
-                    float x0, x1;
-                    ffma2(x0, x1, s[2 * i], s[2 * i + 1], p.scale_log2, -m_used);
-                    const float e0 = fast_exp2(x0), e1 = fast_exp2(x1);
-                    fadd2(sum0, sum1, sum0, sum1, e0, e1);
-                    ffma2w(sq0, sq1, e0, e1, e0, e1, sq0, sq1);
-                    hi[i] = pack_bf16(e0, e1);
-                }
-                l_run += sum0 + sum1;
-                q_run += sq0 + sq1;
-                tmem_st16(lane_base + sb * 128 + cq * 32, hi);     // over the first 16 of this thread's own 32 S columns
-                tmem_wait_st();
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar(kBarPFull + sb));
-                if (tid == 0) HERALD_STAMP(8 + 4 * jg + 2);
-            }
-            // the verdict (the last PV is still running): row sums of e and e^2 over the four column quarters, exchanged as one
-            // bf16 pair per thread (the sum rounded down, the sum of squares rounded up: the test stays on the safe side)
-            {
+            l_run = 0.f, q_run = 0.f, jumped = false;
+            if (kTryFast && fast) {
+                softmax_pass(std::true_type{});
+                // the verdict (the last PV is still running): row sums of e and e^2 over the four column quarters, exchanged as one
+                // bf16 pair per thread (the sum rounded down, the sum of squares rounded up: the test stays on the safe side)
                 uint32_t* ex_pair = reinterpret_cast<uint32_t*>(ex_max);
                 const __nv_bfloat16 lb = __float2bfloat16_rd(l_run), qb = __float2bfloat16_ru(q_run);
                 ex_pair[cq * 128 + row] = (uint32_t)__bfloat16_as_ushort(lb) | ((uint32_t)__bfloat16_as_ushort(qb) << 16);
@@ -674,95 +713,31 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                     q_row += __uint_as_float(v & 0xffff0000u);
                 }
                 if (!(q_row <= kTcFastCmax * l_row * l_row)) jumped = true;
-            }
-        } else {
-            // =========================== softmax warps, exact pass ===========================
-            m_used = -INFINITY, l_run = 0.f;
-            for (int j = 0; j < nt; ++j) {
-                const int jg = HERALD_JB + j, sb = jg % kTcSBufs, eb = jg & 1;
-                mbar_wait(bar(kBarSFull + sb), (jg / kTcSBufs) & 1);
-                tc_fence_after();
-                if (tid == 0) { HERALD_STAMP(8 + 4 * jg + 1); if (jg == 0) HERALD_GSTAMP(62); }
-                float s[32];
-                tmem_ld32_async(lane_base + sb * 128 + cq * 32, s);
-                tmem_wait_ld();
-                const int valid = tile_valid(j);
-                if (valid < kTcBN) {
-#pragma unroll
-                    for (int i = 0; i < 32; ++i)
-                        if (cq * 32 + i >= valid) s[i] = -INFINITY;
-                }
-                float mx = fmax3(s[0], s[1], s[2]);
-#pragma unroll
-                for (int i = 3; i + 1 < 32; i += 2) mx = fmax3(mx, s[i], s[i + 1]);
-                mx = fmaxf(mx, s[31]);
-                // the row maximum only has to be common to the four column quarters and not below the true maximum:
-                // it is exchanged rounded up to bf16
-                ex_max[(eb * 4 + cq) * 128 + row] = __float2bfloat16_ru(mx);
-                named_bar_sync(1 + quarter, 128);                 // the four warps that hold these 32 rows
-                float mrow = __bfloat162float(ex_max[(eb * 4 + 0) * 128 + row]);
-#pragma unroll
-                for (int c = 1; c < 4; ++c) mrow = fmaxf(mrow, __bfloat162float(ex_max[(eb * 4 + c) * 128 + row]));
-                mrow *= p.scale_log2;
-                float alpha = 1.f;
-                bool need = false;
-                if (j == 0) {
-                    m_used = mrow;
-                } else if (mrow > m_used + kTcRescaleThreshold) {
-                    need = true;
-                    alpha = fast_exp2(m_used - mrow);
-                    m_used = mrow;
-                }
-                const bool any = __any_sync(0xffffffffu, need);
-                // P = P_hi + P_lo (bf16 pair: the PV product keeps the weights to ~2^-17 relative).  The exponentials (MUFU,
-                // 16 per clock and SM: the scarce unit) and the splitting arithmetic of earlier pairs share one unrolled loop
-                // so that the scheduler interleaves them.
-                float sum0 = 0.f, sum1 = 0.f;
-                uint32_t hi[16], lo[16];
-#pragma unroll
-                for (int i = 0; i < 16; ++i) {
-                    float x0, x1;
-                    ffma2(x0, x1, s[2 * i], s[2 * i + 1], p.scale_log2, -m_used);
-                    const float e0 = fast_exp2(x0), e1 = fast_exp2(x1);
-                    fadd2(sum0, sum1, sum0, sum1, e0, e1);
-                    hi[i] = pack_bf16(e0, e1);
-                    float r0, r1;
-                    ffma2v(r0, r1, __uint_as_float(hi[i] << 16), __uint_as_float(hi[i] & 0xffff0000u), -1.f, e0, e1);   // e - hi, exact
-                    lo[i] = pack_bf16(r0, r1);
-                }
-                l_run = l_run * alpha + (sum0 + sum1);
-                if (any) {   // rare: the running maximum of some row grew past the threshold -> rescale O in place
-                    mbar_wait(bar(kBarPvDone + ((jg - 1) % kTcSBufs)), ((jg - 1) / kTcSBufs) & 1);   // PV_{j-1} finished; PV_j waits for our arrive
-                    tc_fence_after();
-                    float o[32];
-                    tmem_ld32_async(lane_base + kTcTmemO + cq * 32, o);
-                    tmem_wait_ld();
-#pragma unroll
-                    for (int i = 0; i < 32; ++i) o[i] *= alpha;
-                    tmem_st32(lane_base + kTcTmemO + cq * 32, reinterpret_cast<const uint32_t*>(o));
-                }
-                // Both halves go to TMEM as the A operand of the PV MMA: row = lane, two keys per 32-bit column; P_hi in
-                // columns [0,64) of the S buffer, P_lo in [64,128), this thread's quarter row at [cq*16, cq*16+16) of each.
-                tmem_st16(lane_base + sb * 128 + cq * 16, hi);
-                tmem_st16(lane_base + sb * 128 + 64 + cq * 16, lo);
-                tmem_wait_st();
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar(kBarPFull + sb));
-                if (tid == 0) HERALD_STAMP(8 + 4 * jg + 2);
+            } else {
+                softmax_pass(std::false_type{});
             }
         }
-        // ---- end of a fast pass: one block-wide vote (every warp is here shortly after the last P was handed over) ----
-        if (kTryFast && fast) {
+        // ---- end of the first pass: one block-wide vote (every warp is here shortly after the last P was handed over) ----
+        if (pass == 0) {
             fast = false;
             if (__syncthreads_or(warp < kTcSoftmaxWarps && jumped ? 1 : 0)) {
+                // once more (the first PV of the pass overwrites O), with the hi + lo pair and the row maximum that this pass
+                // saw as the reference: nothing can rise above it
                 jb_rt += nt;
-                continue;         // once more, the exact way: the first PV of the pass overwrites O
+                if (warp < kTcSoftmaxWarps) {
+                    ex_max[cq * 128 + row] = __float2bfloat16_ru(mx_all);
+                    named_bar_sync(1 + quarter, 128);
+                    float mrow = __bfloat162float(ex_max[row]);
+#pragma unroll
+                    for (int c = 1; c < 4; ++c) mrow = fmaxf(mrow, __bfloat162float(ex_max[c * 128 + row]));
+                    m_used = mrow * p.scale_log2;
+                }
+                continue;
             }
         }
         break;
     }
-    const int n_passes = (kTryFast && jb_rt > 0) ? 2 : 1;
+    const int n_passes = jb_rt > 0 ? 2 : 1;
     if (kTryFast && tid == 0 && p.mode_hint && nt > 0) {
         // the note for this block's next launch.  One failed fast pass costs one redo and nothing more (on N(0,1)-like data a
         // row with a 6-sigma logit turns up in some block now and then, and a block that starts exact holds up its whole

@@ -49,6 +49,11 @@ __device__ __forceinline__ uint32_t find_threshold_bin(const uint32_t* hist, int
     return res[0];
 }
 
+#ifndef HERALD_TOPK_UNROLL
+#define HERALD_TOPK_UNROLL 4
+#endif
+constexpr int kTopkUnroll = HERALD_TOPK_UNROLL;
+
 struct TopkParams {
     const float* scores;       // [units][max_seq_len]
     const uint32_t* hist1;     // [units][kBins1]
@@ -100,31 +105,39 @@ __global__ void __launch_bounds__(kTopkThreads, 2) topk_kernel(const TopkParams 
         const int lane = tid & 31;
         for (int i = tid; i < n_words; i += kTopkThreads) { bitmap[i] = 0; tiemap[i] = 0; }
         __syncthreads();
-        for (int tile = 0; tile < L; tile += kTopkThreads * 4) {
-            const int i = tile + tid * 4;
-            float ve[4] = {0.f, 0.f, 0.f, 0.f};
-            if (i < L) {
-                const float4 v = *reinterpret_cast<const float4*>(sc + i);
-                ve[0] = v.x; ve[1] = v.y; ve[2] = v.z; ve[3] = v.w;
-            }
-            uint32_t above = 0;
+        // kTopkUnroll independent 16-byte loads per thread are issued before the first of them is used: at L = 131072
+        // the pass is 32 trips of one load each otherwise, and each trip waits for a whole L2 round trip
+        for (int tile = 0; tile < L; tile += kTopkThreads * 4 * kTopkUnroll) {
+            float4 vv[kTopkUnroll];
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const bool in = i + e < L;
-                const uint32_t key = score_key(ve[e]);
-                const uint32_t bin = key >> (32 - kBits1);
-                if (in && bin > b1) above |= 1u << e;
-                const bool is_c = in && bin == b1;
-                const uint32_t m = __ballot_sync(0xffffffffu, is_c);
-                if (m) {
-                    uint32_t base = 0;
-                    if (lane == 0) base = atomicAdd(&s_ncand, (uint32_t)__popc(m));
-                    base = __shfl_sync(0xffffffffu, base, 0);
-                    if (is_c) cand[base + __popc(m & ((1u << lane) - 1u))] = make_uint2(key, (uint32_t)(i + e));
-                }
+            for (int u = 0; u < kTopkUnroll; ++u) {
+                const int i = tile + (u * kTopkThreads + tid) * 4;
+                vv[u] = i < L ? *reinterpret_cast<const float4*>(sc + i) : make_float4(0.f, 0.f, 0.f, 0.f);
             }
-            // the 4 positions of a thread share one bitmap word (i is a multiple of 4)
-            if (above) atomicOr(&bitmap[i >> 5], above << (i & 31));
+#pragma unroll
+            for (int u = 0; u < kTopkUnroll; ++u) {
+                const int i = tile + (u * kTopkThreads + tid) * 4;
+                if (tile + u * kTopkThreads * 4 >= L) break;   // uniform over the block
+                const float ve[4] = {vv[u].x, vv[u].y, vv[u].z, vv[u].w};
+                uint32_t above = 0;
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const bool in = i + e < L;
+                    const uint32_t key = score_key(ve[e]);
+                    const uint32_t bin = key >> (32 - kBits1);
+                    if (in && bin > b1) above |= 1u << e;
+                    const bool is_c = in && bin == b1;
+                    const uint32_t m = __ballot_sync(0xffffffffu, is_c);
+                    if (m) {
+                        uint32_t base = 0;
+                        if (lane == 0) base = atomicAdd(&s_ncand, (uint32_t)__popc(m));
+                        base = __shfl_sync(0xffffffffu, base, 0);
+                        if (is_c) cand[base + __popc(m & ((1u << lane) - 1u))] = make_uint2(key, (uint32_t)(i + e));
+                    }
+                }
+                // the 4 positions of a thread share one bitmap word (i is a multiple of 4)
+                if (above) atomicOr(&bitmap[i >> 5], above << (i & 31));
+            }
         }
         __syncthreads();
         // levels 2 and 3 on the candidates: the k2 largest of the low 20 key bits

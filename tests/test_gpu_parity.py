@@ -925,8 +925,9 @@ def test_sparse_attn_precision_modes_match_oracle(H, cuda, case, precision, tuni
 
 def test_fast_pass_is_taken_on_flat_rows_and_refused_on_peaked_ones(H, cuda, tuning):
     """Long pools (>= 1536 keys per block), M = 224 rows: with N(0,1) queries every row is flat (sum p^2 ~ e/n) and the fast
-    pass is accepted -- the output then differs from the exact one by the bf16 rounding of the weights, ~1e-4, far inside the
-    bar; with queries scaled x6 the rows are peaked, the criterion refuses, and the result is the exact pass's, bit for bit."""
+    pass is accepted -- the output then carries the bf16 rounding of the weights, ~1e-4 from the oracle, far inside the bar but
+    an order of magnitude above the hi + lo pair's error; with queries scaled x6 the rows are peaked, the criterion refuses, and
+    the block's second pass gives the pair's accuracy again."""
     batch, B, Hq, Hkv, cap = 1, 32, 14, 2, 4000
     for q_scale, expect_fast in ((1.0, True), (6.0, False)):
         q, kb, vb, pk, pv, pl = _attn_case(cuda, batch, B, Hq, Hkv, cap, [[4000, 3000]], seed=99, q_scale=q_scale)
@@ -944,10 +945,44 @@ def test_fast_pass_is_taken_on_flat_rows_and_refused_on_peaked_ones(H, cuda, tun
         pv_clean[torch.isnan(pv_clean)] = 0
         ref, _ = O.sparse_attn(synth.to_u16(q), synth.to_u16(kb), synth.to_u16(vb), synth.to_u16(pk), synth.to_u16(pv_clean),
                                pl.cpu().numpy(), 128 ** -0.5)
-        for mode, out in outs.items():
-            assert np.abs(out.cpu().numpy() - ref).max() <= ATTN_TOL, (q_scale, mode)
-        same = torch.equal(outs[H.ATTN_EXACT], outs[H.ATTN_AUTO])
-        assert same != expect_fast, (q_scale, "fast pass " + ("not taken" if same else "taken"))
+        err = {mode: float(np.abs(out.cpu().numpy() - ref).max()) for mode, out in outs.items()}
+        for mode in outs:
+            assert err[mode] <= ATTN_TOL, (q_scale, mode, err)
         if expect_fast:
-            d = (outs[H.ATTN_EXACT] - outs[H.ATTN_AUTO]).abs().max().item()
-            assert d <= 5e-4, d
+            assert 4 * err[H.ATTN_EXACT] < err[H.ATTN_AUTO] <= 5e-4, (q_scale, "fast pass not taken?", err)
+        else:
+            assert err[H.ATTN_AUTO] <= 2 * err[H.ATTN_EXACT] + 1e-6, (q_scale, "fast pass taken on peaked rows?", err)
+
+
+@pytest.mark.parametrize("precision", ["exact", "auto"])
+@pytest.mark.parametrize("splits", [1, 2])
+def test_logits_far_above_the_first_tile_send_the_block_through_a_second_pass(H, cuda, tuning, precision, splits):
+    """The row reference of a pass is fixed on its first key tile.  Here the first 128 pool rows of every unit point away from
+    the queries (logits ~ -66) and the rest towards them (~ +66): 190 log2 units above the reference, past fp32.  The block must
+    notice, take the row maximum it has seen as the new reference and go through its tiles again; the result is the oracle's."""
+    batch, B, Hq, Hkv, cap = 1, 16, 8, 2, 2200
+    q, kb, vb, pk, pv, pl = _attn_case(cuda, batch, B, Hq, Hkv, cap, [[2200, 1700]], seed=4242)
+    u = torch.full((128,), 128 ** -0.5, device=cuda)
+    q = (q.float() + 30.0 * u).to(torch.bfloat16)
+    kf = pk.float()
+    for h in range(Hkv):
+        n = int(pl[0, h])
+        kf[0, h, :128] = -25.0 * u
+        kf[0, h, 128:n] = kf[0, h, 128:n] * 0.25 + 25.0 * u
+    pk = kf.to(torch.bfloat16)
+    kb = (kb.float() * 0.25 + 25.0 * u).to(torch.bfloat16)
+    shape = H.make_shape(batch, Hq, Hkv, B, 16, 1, cap)
+    ws = H.alloc_workspace(H.herald_attn_workspace_bytes(shape), cuda)
+    tuning(attn_precision=H.ATTN_EXACT if precision == "exact" else H.ATTN_AUTO, attn_splits=splits)
+    pv_clean = pv.clone()
+    pv_clean[torch.isnan(pv_clean)] = 0
+    ref, lse_ref = O.sparse_attn(synth.to_u16(q), synth.to_u16(kb), synth.to_u16(vb), synth.to_u16(pk), synth.to_u16(pv_clean),
+                                 pl.cpu().numpy(), 128 ** -0.5)
+    for launch in range(3):     # the note a block leaves for its next launch must not change the result
+        out = torch.full((batch, B, Hq, 128), float("nan"), dtype=torch.float32, device=cuda)
+        lse = torch.empty((batch, B, Hq), dtype=torch.float32, device=cuda)
+        H.herald_sparse_attn(shape, pk, pv, pl, q, kb, vb, out, lse, ws)
+        torch.cuda.synchronize()
+        err = np.abs(out.cpu().numpy().astype(np.float64) - ref).max()
+        assert np.isfinite(err) and err <= ATTN_TOL, (precision, splits, launch, err)
+        assert np.abs(lse.cpu().numpy() - lse_ref).max() <= 2e-3 * max(1.0, float(np.abs(lse_ref).max()) / 50)
