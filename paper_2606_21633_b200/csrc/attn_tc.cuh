@@ -101,7 +101,7 @@ static_assert(kTcBM * kTcRowFloats * 4 <= kTcStages * kTcTileBytes, "output stag
 // barrier slots (8 bytes each) inside the misc area
 enum { kBarKFull = 0, kBarVFull = kBarKFull + kTcStages,
        kBarSFull = kBarVFull + kTcStages, kBarPFull = kBarSFull + kTcSBufs, kBarPvDone = kBarPFull + kTcSBufs,
-       kBarQFull = kBarPvDone + kTcSBufs, kBarVTail, kBarMerge, kBarPeerReady, kBarQkDone, kBarCount };
+       kBarPvIssued = kBarPvDone + kTcSBufs, kBarQFull = kBarPvIssued + kTcSBufs, kBarVTail, kBarMerge, kBarPeerReady, kBarQkDone, kBarCount };
 constexpr int kTcMiscTmemPtr = 240;              // uint32
 constexpr int kTcMiscReady = 244;                // uint32: the word the peers' "receive buffer ready" signals land on
 constexpr int kTcMiscMax = 256;                  // bf16 [2 buffers][4 column quarters][128 rows]; float [4][128] for the row sums
@@ -554,8 +554,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
             // =========================== QK^T issuer ===========================
             // Two warps feed the tensor pipe, one per product: what an issuing warp does between its MMAs (barrier polls,
             // commits, descriptor set-up: about 1.1k cycles per tile next to 1.1k of issue) was longer than the pipe's own
-            // 1.56k per tile while one warp did both.  The pipe no longer orders S_j after the PV that read the same TMEM
-            // columns three tiles earlier, so this warp waits for that PV's completion barrier.
+            // 1.56k per tile while one warp did both.  S_j overwrites the TMEM columns PV_{j-3} reads its P from: this warp waits
+            // until the other one has ISSUED that PV (tcgen05.fence::before_thread_sync + arrive there, wait +
+            // fence::after_thread_sync here order the two groups of MMAs; the pipe executes them in that order) -- not until
+            // it has completed, which put a whole PV between a block's P_j and its S_{j+3}.
             constexpr uint32_t hi_k = umma_desc_hi(1024);
             const uint32_t q_lo = umma_desc_lo(sbase + kTcSmemQ, 16);
             if (pass == 0) {
@@ -565,7 +567,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
 #pragma unroll 1
             for (int j = 0; j < nt; ++j) {   // S_j = Q K_j^T into S buffer j % 3, which held P_{j-3}
                 const int jg = HERALD_JB + j, stage = jg % kTcStages, sb = jg % kTcSBufs;
-                if (jg >= kTcSBufs) mbar_wait(bar(kBarPvDone + sb), ((jg / kTcSBufs) - 1) & 1);
+                if (jg >= kTcSBufs) mbar_wait(bar(kBarPvIssued + sb), ((jg / kTcSBufs) - 1) & 1);
                 mbar_wait(bar(kBarKFull + stage), (jg / kTcStages) & 1);
                 tc_fence_after();
                 if (lane == 0) { HERALD_STAMP(8 + 4 * jg); if (jg == 0) HERALD_GSTAMP(58); }
@@ -622,6 +624,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                         }
                     }
                     umma_commit(bar(kBarPvDone + sb));               // P_j and V stage j % 3 have been read
+                    tc_fence_before();
+                    mbar_arrive(bar(kBarPvIssued + sb));             // the QK^T issuer may queue S_{j+3} behind these MMAs
                 }
                 __syncwarp();
             }
