@@ -101,7 +101,7 @@ static_assert(kTcBM * kTcRowFloats * 4 <= kTcStages * kTcTileBytes, "output stag
 // barrier slots (8 bytes each) inside the misc area
 enum { kBarKFull = 0, kBarVFull = kBarKFull + kTcStages,
        kBarSFull = kBarVFull + kTcStages, kBarPFull = kBarSFull + kTcSBufs, kBarPvDone = kBarPFull + kTcSBufs,
-       kBarPvIssued = kBarPvDone + kTcSBufs, kBarQFull = kBarPvIssued + kTcSBufs, kBarVTail, kBarMerge, kBarPeerReady, kBarQkDone, kBarCount };
+       kBarPvIssued = kBarPvDone + kTcSBufs, kBarQFull = kBarPvIssued + kTcSBufs, kBarVTail, kBarMerge, kBarPeerReady, kBarAck, kBarQkDone, kBarCount };
 constexpr int kTcMiscTmemPtr = 240;              // uint32
 constexpr int kTcMiscReady = 244;                // uint32: the word the peers' "receive buffer ready" signals land on
 constexpr int kTcMiscMax = 256;                  // bf16 [2 buffers][4 column quarters][128 rows]; float [4][128] for the row sums
@@ -217,6 +217,11 @@ __device__ __forceinline__ void st_async_u32(uint32_t addr, uint32_t v, uint32_t
 __device__ __forceinline__ void st_async_f2(uint32_t addr, float a, float b, uint32_t bar_cluster) {
     asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];"
                  ::"r"(addr), "f"(a), "f"(b), "r"(bar_cluster) : "memory");
+}
+// bulk copy own shared memory -> a peer's shared memory; completes bytes on the peer's mbarrier
+__device__ __forceinline__ void bulk_copy_to_peer(uint32_t dst_cluster, uint32_t src_cta, uint32_t bytes, uint32_t bar_cluster) {
+    asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst_cluster), "r"(src_cta), "r"(bytes), "r"(bar_cluster) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive_remote(uint32_t bar_cluster) {
     asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster) : "memory");
@@ -371,7 +376,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     const int rows_own = (rows_box + S - 1) / S;             // tile rows merged and written by each CTA of the cluster (zero rows past the box are nobody's)
     const int ml_stride = (rows_own + 1) & ~1;               // float2 per source, padded to 16 bytes
     const int n_own = max(0, min(rows_own, rows_box - split * rows_own));   // rows of the box this CTA merges
-    const int merge_bytes = (S - 1) * n_own * (kHeadDim * 4 + 8);   // partial rows and (m, l) the other CTAs send to this one
+    const int merge_bytes = (S - 1) * n_own * (kTcRowFloats * 4 + 8);   // partial rows and (m, l) the other CTAs send to this one
     const int g_inv = (65536 + G - 1) / G;                   // (r * g_inv) >> 16 == r / G for r < 128, G <= 8
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) { HERALD_STAMP(0); HERALD_GSTAMP(60); }
@@ -400,6 +405,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
             // ... and the 4-byte "my receive buffer is ready" signals of the S - 1 peers (asynchronous stores as well: a remote
             // mbarrier arrive with release semantics compiles to a device-wide memory barrier)
             if (S > 1) mbar_arrive_expect_tx(bar(kBarPeerReady), (uint32_t)(S - 1) * 4u);
+            if (S > 1) mbar_arrive_expect_tx(bar(kBarAck), (uint32_t)(S - 1) * 4u);
         }
         if (lane < 5) {
             const CUtensorMap* tm = lane == 0 ? &tm_q : lane == 1 ? &tm_k : lane == 2 ? &tm_v : lane == 3 ? &tm_kb : &tm_vb;
@@ -793,16 +799,32 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
             for (int i = 0; i < 32; ++i) o[i] = 0.f;
         }
         if (tid == 0) HERALD_STAMP(6);
-        if (owner != split && row < rows_box) {
-            // this quarter row (unnormalised) and (m, l) go straight into the owner's receive buffer; slots skip the owner itself
-            mbar_wait_cluster(bar(kBarPeerReady), 0);
-            const int src_slot = split < owner ? split : split - 1;
-            const uint32_t bar_owner = map_to_cta(bar(kBarMerge), owner);
-            const uint32_t dst = map_to_cta(sbase + kTcRecvO + ((src_slot * rows_own + row_l) * kTcRowFloats + cq * 32) * 4, owner);
+        if (S > 1) {
+            if (owner != split && row < rows_box) {
+                float4* stg = reinterpret_cast<float4*>(sgen + kTcStageO + (row * kTcRowFloats + cq * 32) * 4);
 #pragma unroll
-            for (int i = 0; i < 8; ++i) st_async_f4(dst + 16 * i, o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3], bar_owner);
-            if (cq == 0)   // an empty split sends (-inf, 0) and zero rows
-                st_async_f2(map_to_cta(sbase + kTcRecvML + (src_slot * ml_stride + row_l) * 8, owner), nt > 0 ? m_used : -INFINITY, l_tot, bar_owner);
+                for (int i = 0; i < 8; ++i) stg[i] = make_float4(o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
+                if (cq == 0) {
+                    mbar_wait_cluster(bar(kBarPeerReady), 0);
+                    const int src_slot = split < owner ? split : split - 1;
+                    st_async_f2(map_to_cta(sbase + kTcRecvML + (src_slot * ml_stride + row_l) * 8, owner), nt > 0 ? m_used : -INFINITY, l_tot,
+                                map_to_cta(bar(kBarMerge), owner));
+                }
+            }
+            fence_proxy_async_smem();
+            named_bar_sync(1 + quarter, 128);
+            if (cq == 0 && lane == 0) {
+                mbar_wait_cluster(bar(kBarPeerReady), 0);
+                const int r0 = quarter * 32, r1 = min(r0 + 32, rows_box);
+                for (int o2 = 0; o2 < S; ++o2) {
+                    if (o2 == split) continue;
+                    const int ra = max(r0, o2 * rows_own), rb = min(r1, (o2 + 1) * rows_own);
+                    if (ra >= rb) continue;
+                    const int src_slot = split < o2 ? split : split - 1;
+                    bulk_copy_to_peer(map_to_cta(sbase + kTcRecvO + ((src_slot * rows_own + (ra - o2 * rows_own)) * kTcRowFloats) * 4, o2),
+                                      sbase + kTcStageO + ra * kTcRowFloats * 4, (uint32_t)(rb - ra) * kTcRowFloats * 4, map_to_cta(bar(kBarMerge), o2));
+                }
+            }
         }
     }
     if (tid == 0) HERALD_STAMP(5);
@@ -834,7 +856,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
             }
             const float inv = 1.f / den;
             // the V ring is dead (this thread has seen the last PV of the CTA complete): it stages the finished rows
-            float4* dst = reinterpret_cast<float4*>(sgen + kTcStageO + (row_l * kTcRowFloats + cq * 32) * 4);
+            float4* dst = reinterpret_cast<float4*>(sgen + kTcStageO + (row * kTcRowFloats + cq * 32) * 4);
 #pragma unroll
             for (int i = 0; i < 8; ++i) dst[i] = make_float4(o[4 * i] * inv, o[4 * i + 1] * inv, o[4 * i + 2] * inv, o[4 * i + 3] * inv);
             if (p.lse && cq == 0) {
@@ -846,6 +868,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
         if (tid == 0) HERALD_STAMP(7);
     }
     __syncthreads();
+    if (S > 1 && tid < S - 1) {   // every partial row addressed to this CTA has landed: its senders may let go of their staging rows
+        const uint32_t peer = tid < split ? tid : tid + 1;
+        st_async_u32(map_to_cta(misc + kTcMiscReady + 4, peer), 1u, map_to_cta(bar(kBarAck), peer));
+    }
     {
         // coalesced copy of this CTA's finished rows: one warp writes one 512-byte row per instruction
         const float* stage = reinterpret_cast<const float*>(sgen + kTcStageO);
@@ -853,12 +879,12 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
         for (int rl = warp; rl < r_end - r_begin; rl += kTcThreads / 32) {
             const int r = r_begin + rl, bi = (r * g_inv) >> 16;   // r / G
             const int64_t orow = ((int64_t)b * B + i0 + bi) * p.n_q_heads + h * G + (r - bi * G);
-            *reinterpret_cast<float4*>(p.out + orow * kHeadDim + lane * 4) = *reinterpret_cast<const float4*>(stage + rl * kTcRowFloats + lane * 4);
+            *reinterpret_cast<float4*>(p.out + orow * kHeadDim + lane * 4) = *reinterpret_cast<const float4*>(stage + r * kTcRowFloats + lane * 4);
         }
     }
     // a CTA may not exit while a peer can still arrive on its barriers: every peer has announced its receive buffer by now
     // (the partial rows addressed to this CTA have landed: the merge waited for them)
-    if (S > 1 && tid == 0) mbar_wait_cluster(bar(kBarPeerReady), 0);
+    if (S > 1 && tid == 0) { mbar_wait_cluster(bar(kBarPeerReady), 0); mbar_wait_cluster(bar(kBarAck), 0); }
     if (tid == 0) { HERALD_STAMP(4); HERALD_GSTAMP(63); }
 
     // ---- teardown ----
