@@ -346,6 +346,11 @@ __device__ __forceinline__ float fmax3(float a, float b, float c) {
     return r;
 }
 
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* v) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x8.b32 [%8], {%0, %1, %2, %3, %4, %5, %6, %7};"
+        ::"r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(taddr) : "memory");
+}
 __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* v) {
     asm volatile(
         "tcgen05.st.sync.aligned.32x32b.x16.b32 [%16], "
@@ -677,28 +682,33 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
                     }
                     // The exponentials (MUFU, 16 per clock and SM: the scarce unit) and the splitting arithmetic of earlier
                     // pairs share one unrolled loop so that the scheduler interleaves them.
+                    // A operand of the PV MMA: row = lane, two keys per 32-bit column.  The weights leave for TMEM eight columns at
+                    // a time, so that at most 16 of them sit in registers next to the logits still to be exponentiated.
                     float sum0 = 0.f, sum1 = 0.f, sq0 = 0.f, sq1 = 0.f;
-                    uint32_t hi[16], lo[kSingle ? 1 : 16];
 #pragma unroll
-                    for (int i = 0; i < 16; ++i) {
-                        float x0, x1;
-                        ffma2(x0, x1, s[2 * i], s[2 * i + 1], p.scale_log2, -m_used);
-                        const float e0 = fast_exp2(x0), e1 = fast_exp2(x1);
-                        fadd2(sum0, sum1, sum0, sum1, e0, e1);
-                        hi[i] = pack_bf16(e0, e1);
-                        if (kSingle) {
-                            ffma2w(sq0, sq1, e0, e1, e0, e1, sq0, sq1);
-                        } else {
-                            float r0, r1;
-                            ffma2v(r0, r1, __uint_as_float(hi[i] << 16), __uint_as_float(hi[i] & 0xffff0000u), -1.f, e0, e1);   // e - hi, exact
-                            lo[i] = pack_bf16(r0, r1);
+                    for (int half = 0; half < 2; ++half) {
+                        uint32_t hi[8], lo[kSingle ? 1 : 8];
+#pragma unroll
+                        for (int ii = 0; ii < 8; ++ii) {
+                            const int i = half * 8 + ii;
+                            float x0, x1;
+                            ffma2(x0, x1, s[2 * i], s[2 * i + 1], p.scale_log2, -m_used);
+                            const float e0 = fast_exp2(x0), e1 = fast_exp2(x1);
+                            fadd2(sum0, sum1, sum0, sum1, e0, e1);
+                            hi[ii] = pack_bf16(e0, e1);
+                            if (kSingle) {
+                                ffma2w(sq0, sq1, e0, e1, e0, e1, sq0, sq1);
+                            } else {
+                                float r0, r1;
+                                ffma2v(r0, r1, __uint_as_float(hi[ii] << 16), __uint_as_float(hi[ii] & 0xffff0000u), -1.f, e0, e1);   // e - hi, exact
+                                lo[ii] = pack_bf16(r0, r1);
+                            }
                         }
+                        tmem_st8(lane_base + sb * 128 + cq * 32 + half * 8, hi);
+                        if (!kSingle) tmem_st8(lane_base + sb * 128 + cq * 32 + 16 + half * 8, lo);
                     }
                     l_run += sum0 + sum1;
                     if (kSingle) q_run += sq0 + sq1;
-                    // A operand of the PV MMA: row = lane, two keys per 32-bit column
-                    tmem_st16(lane_base + sb * 128 + cq * 32, hi);
-                    if (!kSingle) tmem_st16(lane_base + sb * 128 + cq * 32 + 16, lo);
                     tmem_wait_st();
                     tc_fence_before();
                     __syncwarp();
