@@ -144,6 +144,23 @@ int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, cons
                   const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, float* scores_out,
                   void* ws, size_t ws_bytes, herald_stream_t stream);
 
+/* herald_select for callers that may not allocate device memory (code under CUDA-graph capture, serving loops, harnesses
+ * that forbid cudaMalloc): the same selection, with the workspace -- level-1 histograms and the score plane -- in a
+ * file-scope __device__ array of HERALD_SELECT_STATIC_BYTES inside the library instead of a caller's buffer.  The library
+ * allocates nothing here either: every GPU that loads it holds the array until the process exits.
+ *   Arguments, output layout and errors are herald_select's, without scores_out / ws / ws_bytes.
+ *   Limit: herald_select_workspace_bytes(shape) <= HERALD_SELECT_STATIC_BYTES (mode 0: about batch * H_kv * (max_seq_len + 4096)
+ *   * 4 bytes -- BASELINE C1, C2 and C3 fit, C4 and C5 do not); a larger shape returns HERALD_ERR_WORKSPACE_TOO_SMALL and
+ *   enqueues nothing.
+ *   Every call on a device shares the one array, which keeps the previous call's contents (the call clears the histograms
+ *   itself).  Two herald_select_static calls that overlap on the GPU (different streams, or graphs replayed side by side)
+ *   race on it: keep them on one stream.  Calls that bring their own workspace (herald_select, herald_pipeline_step) do
+ *   not touch the array and may run beside it. */
+#define HERALD_SELECT_STATIC_BYTES (16u << 20)
+size_t herald_select_static_max_bytes(void);      /* host-only: HERALD_SELECT_STATIC_BYTES */
+int herald_select_static(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep,
+                         const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, herald_stream_t stream);
+
 /* Selection scored by x queries per sequence instead of one (PAPER.md:137 Fig. 8, :143, :161: the selection kernel as
  * the query count goes from B = 32 down to 1).  The paper does not say how the x
  * queries' scores combine into one ranking (reading 25): this entry takes the maximum,

@@ -533,6 +533,47 @@ int herald_select(const herald_shape_t* shape, const herald_cache_t* cache, cons
     return select_impl(shape, cache, q_rep, k_per_seq, sel_idx, sel_cnt, scores_out, ws, ws_bytes, stream_, kSelectAll, 0);
 }
 
+// ---- herald_select with its workspace inside the library (callers that may not allocate) -------------------------------
+// The array's name is a device symbol: host code may not pass it to a kernel, it asks the runtime for its device address,
+// once per device and with that device current.
+static __device__ __align__(256) uint8_t g_select_scratch[HERALD_SELECT_STATIC_BYTES];
+
+static int select_scratch_ptr(void** out) {
+    static void* ptr[kMaxDevices] = {nullptr};
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    if (dev < 0 || dev >= kMaxDevices) return fail(HERALD_ERR_UNSUPPORTED, "herald_select_static: device %d >= %d", dev, kMaxDevices);
+    if (!ptr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_select_scratch);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(select scratch)");
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255u)) return fail(HERALD_ERR_CUDA, "herald_select_static: scratch symbol at %p", p);
+        ptr[dev] = p;
+    }
+    *out = ptr[dev];
+    return HERALD_OK;
+}
+
+size_t herald_select_static_max_bytes(void) { return HERALD_SELECT_STATIC_BYTES; }
+
+int herald_select_static(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_rep,
+                         const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, herald_stream_t stream_) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    const size_t need = select_ws_layout(shape).total;
+    if (need > (size_t)HERALD_SELECT_STATIC_BYTES)
+        return fail(HERALD_ERR_WORKSPACE_TOO_SMALL,
+                    "herald_select_static: this shape needs %zu bytes of scratch, the library holds %zu (batch * H_kv * (max_seq_len + %d) * 4 "
+                    "must fit, mode 0); use herald_select with a caller-owned workspace", need, (size_t)HERALD_SELECT_STATIC_BYTES, kBins1);
+    void* ws = nullptr;
+    rc = select_scratch_ptr(&ws);
+    if (rc) return rc;
+    // the level-1 histograms must start at zero and the array keeps the last call's contents: select_impl clears them on the
+    // stream before the scan, as it does for a caller's workspace; the score plane is fully rewritten for t < seq_lens[b]
+    return select_impl(shape, cache, q_rep, k_per_seq, sel_idx, sel_cnt, nullptr, ws, (size_t)HERALD_SELECT_STATIC_BYTES, stream_, kSelectAll, 0);
+}
+
 int herald_select_xq(const herald_shape_t* shape, const herald_cache_t* cache, const void* q_x, int32_t x,
                      const int32_t* k_per_seq, int32_t* sel_idx, int32_t* sel_cnt, float* scores_out, void* ws,
                      size_t ws_bytes, herald_stream_t stream_) {

@@ -24,7 +24,8 @@ OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE_TOO_SMALL, ERR_CUDA = 0, -1,
 AGG_MAX_LOGIT, AGG_SOFTMAX_SUM = 0, 1
 
 EXPORTS = ("herald_last_error", "herald_set_tuning", "herald_budget_rows", "herald_select_workspace_bytes",
-           "herald_attn_workspace_bytes", "herald_attn_grid_ctas", "herald_select", "herald_select_xq", "herald_gather", "herald_sparse_attn", "herald_sparse_attn_groups",
+           "herald_attn_workspace_bytes", "herald_attn_grid_ctas", "herald_select", "herald_select_static",
+           "herald_select_static_max_bytes", "herald_select_xq", "herald_gather", "herald_sparse_attn", "herald_sparse_attn_groups",
            "herald_dense_attn", "herald_rep_attn_workspace_bytes", "herald_rep_attn",
            "herald_select_rep_workspace_bytes", "herald_select_rep",
            "herald_cache_write_block", "herald_pool_append_block",
@@ -108,6 +109,10 @@ _lib.herald_attn_grid_ctas.argtypes = [C.POINTER(Shape)]
 _lib.herald_select.restype = C.c_int
 _lib.herald_select.argtypes = [C.POINTER(Shape), C.POINTER(Cache), C.c_void_p, C.c_void_p, C.c_void_p,
                                C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
+_lib.herald_select_static_max_bytes.restype = C.c_size_t
+_lib.herald_select_static_max_bytes.argtypes = []
+_lib.herald_select_static.restype = C.c_int
+_lib.herald_select_static.argtypes = [C.POINTER(Shape), C.POINTER(Cache), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.herald_select_xq.restype = C.c_int
 _lib.herald_select_xq.argtypes = [C.POINTER(Shape), C.POINTER(Cache), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p,
                                   C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
@@ -223,6 +228,16 @@ def herald_select(shape, cache, q_rep, k_per_seq, sel_idx, sel_cnt, scores_out, 
     ws_ptr, ws_bytes = _ws(ws)
     _check(_lib.herald_select(C.byref(shape), C.byref(cache), _ptr(q_rep), _ptr(k_per_seq), _ptr(sel_idx),
                               _ptr(sel_cnt), _ptr(scores_out), ws_ptr, ws_bytes, _stream(stream)))
+
+
+def herald_select_static_max_bytes() -> int:
+    return int(_lib.herald_select_static_max_bytes())
+
+
+def herald_select_static(shape, cache, q_rep, k_per_seq, sel_idx, sel_cnt, stream=None):
+    """herald_select with the workspace held inside the library (no allocation anywhere; include/herald.h)."""
+    _check(_lib.herald_select_static(C.byref(shape), C.byref(cache), _ptr(q_rep), _ptr(k_per_seq), _ptr(sel_idx),
+                                     _ptr(sel_cnt), _stream(stream)))
 
 
 def herald_select_xq(shape, cache, q_x, x, k_per_seq, sel_idx, sel_cnt, scores_out, ws, stream=None):
