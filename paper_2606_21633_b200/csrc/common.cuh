@@ -29,6 +29,13 @@ __device__ __forceinline__ uint4 ldg_stream_u4(const void* p) {
     return r;
 }
 
+// 32 bytes per lane (sm_100: 256-bit global loads); p must be 32-byte aligned
+__device__ __forceinline__ void ldg_stream_u8(const void* p, uint32_t* r) {
+    asm volatile("ld.global.nc.L1::no_allocate.L2::128B.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "l"(p));
+}
+
 __device__ __forceinline__ uint4 ldg_u4(const void* p) { return __ldg(reinterpret_cast<const uint4*>(p)); }
 
 // D(16x8, fp32) += A(16x16, bf16, row) * B(16x8, bf16, col)

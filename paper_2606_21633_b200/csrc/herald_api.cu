@@ -491,10 +491,21 @@ static int select_impl(const herald_shape_t* shape, const herald_cache_t* cache,
         if (shape->agg_mode == HERALD_AGG_MAX_LOGIT && Hkv <= 8 && kScanWarps % Hkv == 0 && !g_tune.scan_head_major) {
             // page-major order: the warps next to each other read the head tiles of one page (whole pages for DRAM)
             const size_t smem = (size_t)Hkv * kBins1 * sizeof(uint32_t);
-            static bool pm_attr[kMaxDevices] = {false};
-            e = ensure_smem(scan_pm_kernel, 8 * kBins1 * (int)sizeof(uint32_t), pm_attr);
+            static bool pm_attr[kMaxDevices] = {false}, pm_wide_attr[kMaxDevices] = {false};
+            // A scan on less than half of the SMs (beside the attention) is bound by what one SM can draw, not by HBM: it takes
+            // 32-byte loads (rows must be 32-byte aligned; the contract asks for 16) and prefetches the next page into L2 (pages
+            // must be token-major and whole: the prefetched range [page, page + 16 token rows) then belongs to the page).
+            const bool few = 2 * scan_ctas <= sm_count() && (kScanPmWideThreads / 32) % Hkv == 0;
+            const bool wide = few && reinterpret_cast<uintptr_t>(sp.k_pages) % 32 == 0 && sp.page_stride % 16 == 0 && sp.token_stride % 16 == 0 &&
+                              sp.head_stride % 16 == 0;
+            if (wide && sp.token_stride >= (int64_t)Hkv * sp.head_stride && sp.head_stride >= kHeadDim &&
+                sp.page_stride >= kPageSize * sp.token_stride && kPageSize * sp.token_stride * 2 <= (1 << 20))
+                sp.l2_prefetch = (int32_t)(kPageSize * sp.token_stride * 2);
+            e = wide ? ensure_smem(scan_pm_kernel<true, kScanPmWideThreads>, 8 * kBins1 * (int)sizeof(uint32_t), pm_wide_attr)
+                     : ensure_smem(scan_pm_kernel<false, kScanThreads>, 8 * kBins1 * (int)sizeof(uint32_t), pm_attr);
             if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(scan)");
-            scan_pm_kernel<<<grid, kScanThreads, smem, stream>>>(sp);
+            if (wide) scan_pm_kernel<true, kScanPmWideThreads><<<grid, kScanPmWideThreads, smem, stream>>>(sp);
+            else scan_pm_kernel<false, kScanThreads><<<grid, kScanThreads, smem, stream>>>(sp);
         } else if (shape->agg_mode == HERALD_AGG_MAX_LOGIT) {
             scan_kernel<0><<<grid, kScanThreads, 0, stream>>>(sp);
         } else {

@@ -30,6 +30,8 @@ struct ScanParams {
     float2* stats_part;   // [batch*H_kv][G][gridDim.x] (m, l)       (mode 1)
     uint32_t* hist1;      // [batch*H_kv][kBins1]                    (mode 0)
     int32_t batch, n_q_heads, n_kv_heads, max_seq_len, max_pages;
+    int32_t l2_prefetch;        // page-major scan with 32-byte loads: bytes of a page to prefetch into L2 one iteration ahead (0 = off); set for grids of
+                                // a few CTAs, where latency and not HBM bounds the stream (it costs 6 % when every SM scans)
     int32_t part_lo, part_hi;   // this launch covers [part_lo, part_hi) thousandths of the tile space (0, 1000 = all of it): the
                                 // pipeline runs a head part on every SM before the denoising steps and the rest beside them
     float sm_scale;
@@ -205,22 +207,35 @@ __global__ void __launch_bounds__(kScanThreads, 1) scan_kernel(const ScanParams 
 // tiles of the same page at the same time, so DRAM sees whole 4-16 KB pages instead of 256-byte pieces 1 KB apart
 // (+6 % bandwidth on B200).  Work = the pages of the batch in sequence-major order, cut into gridDim.x equal
 // contiguous ranges; a CTA keeps one histogram per KV head in shared memory (H_kv x 16 KB, dynamic).
-__global__ void __launch_bounds__(kScanThreads, 1) scan_pm_kernel(const ScanParams p) {
+//
+// kWide (rows 32-byte aligned): a lane loads 32 bytes at a time (ld.global.v8.b32, sm_100), so the four lanes that share a
+// token row cover one whole 128-byte line per load instruction.  The SM's load pipe handles one line per clock whether a warp
+// uses 64 or 128 bytes of it: with 16-byte loads (8 rows x 64 B per instruction) ncu shows the L1 data pipe 76 % busy on the
+// SMs of a 20-CTA scan and the SM streams at 78 GB/s (a load-only kernel with this pattern: 118); with 32-byte loads the
+// same pattern reaches 170 GB/s per SM.  That is what the retrieval stream has beside the attention.
+// 768 threads there: the tile of a lane is 32 registers + 16 of q; at 1024 threads (64 registers) that kernel spills and gains
+// nothing, at 512 too few bytes are in flight.  When every SM scans, HBM is the bound and bytes in flight are what counts: the
+// launcher then takes the 16-byte loads with 1024 threads (76.6 against 73.8 % of 8 TB/s on C2).
+constexpr int kScanPmWideThreads = 768;
+
+template <bool kWide, int kThreads>
+__global__ void __launch_bounds__(kThreads, 1) scan_pm_kernel(const ScanParams p) {
+    constexpr int kScanPmThreads = kThreads, kScanPmWarps = kThreads / 32;
     extern __shared__ uint32_t s_hist_pm[];   // [H_kv][kBins1]
     __shared__ int64_t s_total;
 
     const int G = p.n_q_heads / p.n_kv_heads, H = p.n_kv_heads;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = lane >> 2, tig = lane & 3;
-    const int h = warp % H;                    // fixed per warp: 32 % H == 0
-    const int pages_per_iter = kScanWarps / H;
+    const int h = warp % H;                    // fixed per warp: H divides the warp count
+    const int pages_per_iter = kScanPmWarps / H;
 
     if (threadIdx.x == 0) {
         int64_t total = 0;
         for (int b = 0; b < p.batch; ++b) total += seq_pages(p, b);
         s_total = total;
     }
-    for (int i = threadIdx.x; i < H * kBins1; i += kScanThreads) s_hist_pm[i] = 0;
+    for (int i = threadIdx.x; i < H * kBins1; i += kScanPmThreads) s_hist_pm[i] = 0;
     __syncthreads();
     const int64_t total = s_total;
     const int64_t g0 = cta_part_begin(total, p.part_lo, p.part_hi, blockIdx.x, gridDim.x);
@@ -237,34 +252,56 @@ __global__ void __launch_bounds__(kScanThreads, 1) scan_pm_kernel(const ScanPara
         if (lo >= hi) continue;                            // block-uniform
         const int page_lo = (int)(lo - (seq_begin - n_pages)), page_hi = (int)(hi - (seq_begin - n_pages));
         const int32_t* pt = p.page_table + (int64_t)b * p.max_pages;
-        uint4 qf[4];
+        // B operand: query head g of this KV head's group (zeros for g >= G), channel-permuted like A: register 4i + r of the
+        // lane holds channels [32 i + 8 tig + 2r, +2) (16-byte loads) or register 8j + r channels [64 j + 16 tig + 2r, +2) (32-byte)
+        uint32_t qf[16];
         {
-            const __nv_bfloat16* qrow = p.q_rep + ((int64_t)b * p.n_q_heads + h * G + g) * kHeadDim + 8 * tig;
+            const __nv_bfloat16* qrow = p.q_rep + ((int64_t)b * p.n_q_heads + h * G + g) * kHeadDim + (kWide ? 16 : 8) * tig;
 #pragma unroll
-            for (int i = 0; i < 4; ++i) qf[i] = (g < G) ? ldg_u4(qrow + 32 * i) : make_uint4(0, 0, 0, 0);
+            for (int i = 0; i < 4; ++i) {
+                const uint4 v = (g < G) ? ldg_u4(kWide ? qrow + 64 * (i >> 1) + 8 * (i & 1) : qrow + 32 * i) : make_uint4(0, 0, 0, 0);
+                qf[4 * i] = v.x, qf[4 * i + 1] = v.y, qf[4 * i + 2] = v.z, qf[4 * i + 3] = v.w;
+            }
         }
         float* score_row = p.scores + (int64_t)(b * H + h) * p.max_seq_len;
 
+        // wide kernel: page ids run two iterations ahead of the loads, so that the id of the next page is in a register when its
+        // prefetch is issued (the 64-register kernel has no register for that and looks one iteration ahead)
         int page = page_lo + warp / H;
         int phys = page < page_hi ? __ldg(pt + page) : 0;
+        int phys_next = kWide && page + pages_per_iter < page_hi ? __ldg(pt + page + pages_per_iter) : 0;
         while (page < page_hi) {
             const int next = page + pages_per_iter;
-            const int phys_next = next < page_hi ? __ldg(pt + next) : 0;
-            const __nv_bfloat16* base = p.k_pages + (int64_t)phys * p.page_stride + (int64_t)h * p.head_stride + 8 * tig;
+            int phys_next2 = 0;
+            if (kWide) {
+                phys_next2 = next + pages_per_iter < page_hi ? __ldg(pt + next + pages_per_iter) : 0;
+                // the page of the next iteration is pulled into L2 while this one is multiplied (one request per page: its H head
+                // tiles are contiguous): the loads then find it there, and the few SMs of an overlapped scan need fewer bytes in flight
+                if (p.l2_prefetch && h == 0 && lane == 0 && next < page_hi)
+                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p.k_pages + (int64_t)phys_next * p.page_stride), "r"((uint32_t)p.l2_prefetch) : "memory");
+            } else {
+                phys_next = next < page_hi ? __ldg(pt + next) : 0;
+            }
+            const __nv_bfloat16* base = p.k_pages + (int64_t)phys * p.page_stride + (int64_t)h * p.head_stride + (kWide ? 16 : 8) * tig;
             const __nv_bfloat16* r0 = base + (int64_t)g * p.token_stride;
             const __nv_bfloat16* r1 = base + (int64_t)(g + 8) * p.token_stride;
-            uint4 a[4], c[4];
+            uint32_t a[16], c[16];   // token rows g and g + 8
+            if (kWide) {
+                ldg_stream_u8(r0, a);
+                ldg_stream_u8(r1, c);
+                ldg_stream_u8(r0 + 64, a + 8);
+                ldg_stream_u8(r1 + 64, c + 8);
+            } else {
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                a[i] = ldg_stream_u4(r0 + 32 * i);
-                c[i] = ldg_stream_u4(r1 + 32 * i);
+                for (int i = 0; i < 4; ++i) {
+                    const uint4 va = ldg_stream_u4(r0 + 32 * i), vc = ldg_stream_u4(r1 + 32 * i);
+                    a[4 * i] = va.x, a[4 * i + 1] = va.y, a[4 * i + 2] = va.z, a[4 * i + 3] = va.w;
+                    c[4 * i] = vc.x, c[4 * i + 1] = vc.y, c[4 * i + 2] = vc.z, c[4 * i + 3] = vc.w;
+                }
             }
             float acc[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                mma_bf16_16816(acc, a[i].x, c[i].x, a[i].y, c[i].y, qf[i].x, qf[i].y);
-                mma_bf16_16816(acc, a[i].z, c[i].z, a[i].w, c[i].w, qf[i].z, qf[i].w);
-            }
+            for (int i = 0; i < 8; ++i) mma_bf16_16816(acc, a[2 * i], c[2 * i], a[2 * i + 1], c[2 * i + 1], qf[2 * i], qf[2 * i + 1]);
             float m0 = fmaxf(v0 ? acc[0] : -INFINITY, v1 ? acc[1] : -INFINITY);
             float m1 = fmaxf(v0 ? acc[2] : -INFINITY, v1 ? acc[3] : -INFINITY);
             m0 = fmaxf(m0, __shfl_xor_sync(0xffffffffu, m0, 1));
@@ -279,11 +316,12 @@ __global__ void __launch_bounds__(kScanThreads, 1) scan_pm_kernel(const ScanPara
             }
             page = next;
             phys = phys_next;
+            if (kWide) phys_next = phys_next2;
         }
         // ---- end of this CTA's share of sequence b: flush the H histograms ----
         __syncthreads();
         uint32_t* gh = p.hist1 + (int64_t)b * H * kBins1;   // units b*H .. b*H + H-1 are contiguous
-        for (int i = threadIdx.x; i < H * kBins1; i += kScanThreads) {
+        for (int i = threadIdx.x; i < H * kBins1; i += kScanPmThreads) {
             const uint32_t v = s_hist_pm[i];
             if (v) {
                 atomicAdd(gh + i, v);

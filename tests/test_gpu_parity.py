@@ -124,10 +124,15 @@ def test_select_xq_matches_oracle(H, cuda, case, x, path, tuning):
             assert np.all(sel_g[b, h, int(cnt_g[b, h]):] == -7), "entries past sel_cnt must stay untouched"
     units = w.batch * w.n_kv_heads
     assert differing <= max(1, units // 4), f"{differing} in-band swaps over {units} units is more than rounding explains"
-    if x == 1 and path != "tcgen05":      # one query on the mma.sync kernel: bit-identical to herald_select's mode-0 plane
+    if x == 1 and path != "tcgen05":
+        # one query on the mma.sync kernel: herald_select's mode-0 plane up to the order of the 128 fp32 additions (the two
+        # kernels walk the channels in different orders since herald_select's scan loads 32 bytes per lane; SURVEY.md 8(c)'s
+        # error budget: <= 128 * 2^-24 * sum|q_c k_c| * d^-1/2 ~ 5e-5 worst case, ~1e-6 typical).  Both index sets are checked
+        # against the oracle's band (above and in test_select_matches_oracle).
         _, _, _, sel1, cnt1, sc1 = run_select(H, w, inp, ks, 0)
-        assert torch.equal(sc1[:, :, :max_seq].nan_to_num(0.0), scores[:, :, :max_seq].nan_to_num(0.0))
-        assert torch.equal(sel1, sel_idx) and torch.equal(cnt1, sel_cnt)
+        diff = (sc1[:, :, :max_seq].nan_to_num(0.0) - scores[:, :, :max_seq].nan_to_num(0.0)).abs().max().item()
+        assert diff <= 5e-5, diff
+        assert torch.equal(cnt1, sel_cnt)
 
 
 @pytest.mark.parametrize("ctas", [1, 5, 37])
