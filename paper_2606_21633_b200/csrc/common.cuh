@@ -17,8 +17,8 @@ constexpr int kBins1 = 1 << kBits1, kBins2 = 1 << kBits2, kBins3 = 1 << kBits3;
 // Order-preserving map fp32 -> u32 (larger float <=> larger key).  -0 is canonicalised to +0 first
 // so that equal floats have equal keys (ties are broken by position, reading 7).
 __device__ __forceinline__ uint32_t score_key(float x) {
-    uint32_t u = __float_as_uint(x + 0.0f);
-    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+    const uint32_t u = __float_as_uint(x + 0.0f);
+    return u ^ ((uint32_t)((int32_t)u >> 31) | 0x80000000u);   // negative: all bits flipped; non-negative: the sign bit set
 }
 
 __device__ __forceinline__ uint4 ldg_stream_u4(const void* p) {

@@ -88,7 +88,14 @@ __global__ void __launch_bounds__(kTopkThreads, 2) topk_kernel(const TopkParams 
     const int tid = threadIdx.x;
 
     if (tid == 0) { s_res[0] = 0; s_res[1] = 0; s_ncand = 0; }
-    for (int i = tid; i < kBins1; i += kTopkThreads) s_hist[i] = p.hist1[(int64_t)unit * kBins1 + i];
+    {   // the level-1 histogram: all loads of a thread in flight at once
+        static_assert(kBins1 % kTopkThreads == 0, "histogram load");
+        uint32_t hv[kBins1 / kTopkThreads];
+#pragma unroll
+        for (int j = 0; j < kBins1 / kTopkThreads; ++j) hv[j] = __ldg(p.hist1 + (int64_t)unit * kBins1 + j * kTopkThreads + tid);
+#pragma unroll
+        for (int j = 0; j < kBins1 / kTopkThreads; ++j) s_hist[j * kTopkThreads + tid] = hv[j];
+    }
     __syncthreads();
     uint32_t above1, above2, above3;
     const uint32_t b1 = find_threshold_bin(s_hist, kBins1, (uint32_t)kk, s_warp, s_res, &above1);
@@ -103,10 +110,14 @@ __global__ void __launch_bounds__(kTopkThreads, 2) topk_kernel(const TopkParams 
         uint32_t* tiemap = bitmap + p.bitmap_words;                                          // positions with key == T
         const int n_words = (L + 31) >> 5;
         const int lane = tid & 31;
-        for (int i = tid; i < n_words; i += kTopkThreads) { bitmap[i] = 0; tiemap[i] = 0; }
+        for (int i = tid; i < n_words; i += kTopkThreads) tiemap[i] = 0;
+        const uint32_t k_lo = b1 << (32 - kBits1), k_top = k_lo | ((1u << (32 - kBits1)) - 1u);   // the keys of the threshold bin
         __syncthreads();
         // kTopkUnroll independent 16-byte loads per thread are issued before the first of them is used: at L = 131072
-        // the pass is 32 trips of one load each otherwise, and each trip waits for a whole L2 round trip
+        // the pass is 32 trips of one load each otherwise, and each trip waits for a whole L2 round trip.
+        // The candidates among the 4 * kTopkUnroll scores of a trip are appended with ONE shared-memory atomic per warp: a
+        // ballot + atomic + shuffle per score made the pass a chain of ~30 atomic round trips per warp on one address.
+        // The order of the candidate list does not matter.
         for (int tile = 0; tile < L; tile += kTopkThreads * 4 * kTopkUnroll) {
             float4 vv[kTopkUnroll];
 #pragma unroll
@@ -114,29 +125,57 @@ __global__ void __launch_bounds__(kTopkThreads, 2) topk_kernel(const TopkParams 
                 const int i = tile + (u * kTopkThreads + tid) * 4;
                 vv[u] = i < L ? *reinterpret_cast<const float4*>(sc + i) : make_float4(0.f, 0.f, 0.f, 0.f);
             }
+            uint32_t cmask = 0;                    // bit 4u + e: score e of load u lies in the threshold bin [k_lo, k_top]
 #pragma unroll
             for (int u = 0; u < kTopkUnroll; ++u) {
                 const int i = tile + (u * kTopkThreads + tid) * 4;
                 if (tile + u * kTopkThreads * 4 >= L) break;   // uniform over the block
                 const float ve[4] = {vv[u].x, vv[u].y, vv[u].z, vv[u].w};
-                uint32_t above = 0;
+                uint32_t above = 0, cm = 0;
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
-                    const bool in = i + e < L;
                     const uint32_t key = score_key(ve[e]);
-                    const uint32_t bin = key >> (32 - kBits1);
-                    if (in && bin > b1) above |= 1u << e;
-                    const bool is_c = in && bin == b1;
-                    const uint32_t m = __ballot_sync(0xffffffffu, is_c);
-                    if (m) {
-                        uint32_t base = 0;
-                        if (lane == 0) base = atomicAdd(&s_ncand, (uint32_t)__popc(m));
-                        base = __shfl_sync(0xffffffffu, base, 0);
-                        if (is_c) cand[base + __popc(m & ((1u << lane) - 1u))] = make_uint2(key, (uint32_t)(i + e));
+                    above |= (key > k_top ? 1u : 0u) << e;
+                    cm |= (key >= k_lo ? 1u : 0u) << e;
+                }
+                cm &= ~above;
+                if (i + 3 >= L) {                  // the last load of the plane: positions past L do not count
+                    const uint32_t valid = i < L ? (1u << (L - i)) - 1u : 0u;
+                    above &= valid;
+                    cm &= valid;
+                }
+                cmask |= cm << (4 * u);
+                // 8 neighbouring lanes hold the 32 positions of one bitmap word (bit 4 * (lane & 7) + e): the word is put
+                // together with three shuffles and written once by the first of them -- no atomics, and every word below
+                // n_words is written, so none needs clearing
+                uint32_t word = above << (4 * (lane & 7));
+                word |= __shfl_xor_sync(0xffffffffu, word, 1);
+                word |= __shfl_xor_sync(0xffffffffu, word, 2);
+                word |= __shfl_xor_sync(0xffffffffu, word, 4);
+                if ((lane & 7) == 0 && i < L) bitmap[i >> 5] = word;
+            }
+            if (__any_sync(0xffffffffu, cmask != 0)) {
+                // warp-inclusive scan of the candidate counts, one atomic for the warp's total of the trip
+                const uint32_t mine = __popc(cmask);
+                uint32_t incl = mine;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t n = __shfl_up_sync(0xffffffffu, incl, o);
+                    if (lane >= o) incl += n;
+                }
+                uint32_t base = 0;
+                if (lane == 31) base = atomicAdd(&s_ncand, incl);
+                base = __shfl_sync(0xffffffffu, base, 31) + incl - mine;
+#pragma unroll
+                for (int u = 0; u < kTopkUnroll; ++u) {
+                    if ((cmask >> (4 * u)) & 15u) {
+                        const int i = tile + (u * kTopkThreads + tid) * 4;
+                        const float ve[4] = {vv[u].x, vv[u].y, vv[u].z, vv[u].w};
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            if (cmask & (1u << (4 * u + e))) cand[base++] = make_uint2(score_key(ve[e]), (uint32_t)(i + e));
                     }
                 }
-                // the 4 positions of a thread share one bitmap word (i is a multiple of 4)
-                if (above) atomicOr(&bitmap[i >> 5], above << (i & 31));
             }
         }
         __syncthreads();
