@@ -1266,9 +1266,10 @@ int herald_pipeline_tune(herald_pipeline_t* p, int32_t reps, herald_schedule_t* 
         return HERALD_OK;
     };
     // 1. the scan grid beside the denoising steps: around the SMs the attention grid leaves free; every SM; every SM after the last step
-    const int grids[3] = {spare - 2, spare, n_sm / 8};
-    for (int i = 0; i < 3 && rc == HERALD_OK; ++i) {
-        bool dup = grids[i] < 8 && grids[i] != spare;
+    // (a multi-wave attention grid has no hard number of free SMs: a few more for the scan can pay, C5 takes 56 rather than 40)
+    const int grids[5] = {spare - 2, spare, n_sm / 8, spare + n_sm / 16, spare + n_sm / 8};
+    for (int i = 0; i < 5 && rc == HERALD_OK; ++i) {
+        bool dup = (grids[i] < 8 && grids[i] != spare) || grids[i] >= n_sm;
         for (int j = 0; j < i; ++j) dup = dup || grids[j] == grids[i];
         if (!dup && grids[i] >= 1) rc = time_one(grids[i], start0, 0);
     }
