@@ -84,6 +84,38 @@ def test_select_matches_oracle(H, cuda, case, agg_mode):
                     assert len(planted - set(sel_g[b, h, :ks[b]].tolist())) <= max(1, len(planted) // 8)
 
 
+@pytest.mark.parametrize("aligned32", [True, False])
+@pytest.mark.parametrize("ctas", [3, 37])
+@pytest.mark.parametrize("case", ["tiny_ragged", "g7_ragged", "g8_h8", "C1"])
+def test_select_on_few_sms_matches_oracle(H, cuda, case, ctas, aligned32, tuning):
+    """A scan grid of at most half the SMs (what the retrieval stream has beside the attention) takes the kernel with 32-byte
+    loads and the L2 prefetch of the next page; a cache whose rows are only 16-byte aligned must fall back to 16-byte loads."""
+    c = SELECT_CASES[case]
+    w = c["w"]
+    inp = synth.make_inputs(w, seed=700 + len(case), device=cuda, spare_pages=c["spare"], hostile_tails=c["hostile"])
+    if not aligned32:
+        for name in ("k_pages", "v_pages"):
+            t = inp[name]
+            big = torch.empty(t.numel() + 16, dtype=t.dtype, device=cuda)
+            off = 8 if big.data_ptr() % 32 == 0 else 0          # 8 bf16 = 16 bytes past a 32-byte boundary
+            view = big[off:off + t.numel()].view(t.shape)
+            view.copy_(t)
+            assert view.data_ptr() % 32 == 16
+            inp[name] = view
+    ks = [O.budget_rows(L, w.permille) for L in w.seq_lens]
+    tuning(scan_ctas=ctas)
+    shape, cache, k_per_seq, sel_idx, sel_cnt, scores = run_select(H, w, inp, ks, 0)
+    oi = oracle_inputs(inp)
+    _, sc_o = O.select(oi["q_rep"], oi["k_pages"], oi["page_table"], oi["seq_lens"], ks, w.n_kv_heads, 128 ** -0.5, 0)
+    sel_g, cnt_g, sc_g = sel_idx.cpu().numpy(), sel_cnt.cpu().numpy(), scores.cpu().numpy()
+    differing = 0
+    for b, L in enumerate(w.seq_lens):
+        for h in range(w.n_kv_heads):
+            assert np.abs(sc_g[b, h, :L] - sc_o[b][h]).max() <= 1e-4, (case, ctas, b, h)
+            differing += check_selection(sel_g[b, h], int(cnt_g[b, h]), sc_o[b][h], ks[b], L, f"{case} ctas{ctas} b{b} h{h}")
+    assert differing <= max(1, w.batch * w.n_kv_heads // 4)
+
+
 XQ_CASES = [("tiny_ragged", 1), ("tiny_ragged", 3), ("one_token", 2), ("g7_ragged", 4), ("g7_ragged", 32), ("g8_h8", 32), ("g1", 5),
             ("h3_g5", 7), ("h6_g2", 20)]
 
