@@ -498,9 +498,11 @@ static int select_impl(const herald_shape_t* shape, const herald_cache_t* cache,
             const bool few = 2 * scan_ctas <= sm_count() && (kScanPmWideThreads / 32) % Hkv == 0;
             const bool wide = few && reinterpret_cast<uintptr_t>(sp.k_pages) % 32 == 0 && sp.page_stride % 16 == 0 && sp.token_stride % 16 == 0 &&
                               sp.head_stride % 16 == 0;
+            // (the range ends with the last row the scan itself reads from the page, so it never leaves the caller's allocation)
+            const int64_t page_span = ((kPageSize - 1) * sp.token_stride + (Hkv - 1) * sp.head_stride + kHeadDim) * 2;   // bytes
             if (wide && sp.token_stride >= (int64_t)Hkv * sp.head_stride && sp.head_stride >= kHeadDim &&
-                sp.page_stride >= kPageSize * sp.token_stride && kPageSize * sp.token_stride * 2 <= (1 << 20))
-                sp.l2_prefetch = (int32_t)(kPageSize * sp.token_stride * 2);
+                sp.page_stride >= kPageSize * sp.token_stride && page_span <= (1 << 20))
+                sp.l2_prefetch = (int32_t)page_span;
             e = wide ? ensure_smem(scan_pm_kernel<true, kScanPmWideThreads>, 8 * kBins1 * (int)sizeof(uint32_t), pm_wide_attr)
                      : ensure_smem(scan_pm_kernel<false, kScanThreads>, 8 * kBins1 * (int)sizeof(uint32_t), pm_attr);
             if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(scan)");
