@@ -295,7 +295,7 @@ typedef struct herald_pipeline {
     int32_t scan_head_permille; /* 0..1000: that many thousandths of the (first sparse layer's) score scan run with one block per
                                  SM BEFORE the main stream's next denoising step starts (the main stream waits for them), the rest
                                  with scan_ctas blocks beside the steps.  The retrieval stream needs a fixed amount of SM time
-                                 (an SM draws ~77 GB/s from L2/HBM); when the SMs the attention grid leaves free cannot deliver it
+                                 (an SM draws ~100 GB/s from L2/HBM with the scan's access pattern); when the SMs the attention grid leaves free cannot deliver it
                                  inside the denoising window, a head start costs less than a retrieval stream that outlasts the
                                  window.  0 = everything beside the steps (max-logit aggregation only;
                                  ignored with HERALD_AGG_SOFTMAX_SUM) */
