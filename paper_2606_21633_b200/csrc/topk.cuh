@@ -198,15 +198,18 @@ __global__ void __launch_bounds__(kTopkThreads, 2) topk_kernel(const TopkParams 
         const uint32_t b3f = find_threshold_bin(s_hist, kBins3, k3f, s_warp, s_res, &above3f);
         const uint32_t need_f = k3f - above3f;          // exact ties (key == T) to keep, lowest positions first
         const uint32_t T = (b1 << (32 - kBits1)) | (b2f << kBits3) | b3f;
+        // the level-3 count of the threshold bin is the number of scores equal to T: when all of them are kept (the usual case:
+        // one score sits on the threshold) they go straight into the bitmap and the tie phase with its block scan is skipped
+        const bool all_ties = s_hist[b3f] == need_f;
         for (uint32_t c = tid; c < n_c; c += kTopkThreads) {
             const uint2 kc = cand[c];
-            if (kc.x > T) atomicOr(&bitmap[kc.y >> 5], 1u << (kc.y & 31));
+            if (kc.x > T || (all_ties && kc.x == T)) atomicOr(&bitmap[kc.y >> 5], 1u << (kc.y & 31));
             else if (kc.x == T) atomicOr(&tiemap[kc.y >> 5], 1u << (kc.y & 31));
         }
         __syncthreads();
         const int wpt = (n_words + kTopkThreads - 1) / kTopkThreads;   // words per thread (<= 8), contiguous
         const int w0 = tid * wpt, w1 = min(n_words, w0 + wpt);
-        {   // ties: keep the first need_f in position order
+        if (!all_ties) {   // ties: keep the first need_f in position order (block-uniform branch)
             uint32_t cnt = 0;
             for (int wd = w0; wd < w1; ++wd) cnt += __popc(tiemap[wd]);
             uint32_t total;
@@ -221,19 +224,26 @@ __global__ void __launch_bounds__(kTopkThreads, 2) topk_kernel(const TopkParams 
                 }
                 bitmap[wd] |= keep;                     // this thread owns word wd in this phase
             }
+            __syncthreads();
         }
-        __syncthreads();
-        {   // emit the set positions in ascending order
+        {   // emit the set positions in ascending order: staged in the candidate list's memory (dead by now) when they fit, so
+            // that the global stores are coalesced instead of ~6 consecutive ints per thread
             uint32_t cnt = 0;
             for (int wd = w0; wd < w1; ++wd) cnt += __popc(bitmap[wd]);
             uint32_t total;
             uint32_t at = block_exclusive_scan(cnt, s_warp, &total);
+            const bool staged = kk <= 2 * p.cand_cap;       // block-uniform
+            int32_t* dst = staged ? reinterpret_cast<int32_t*>(cand) : out;
             for (int wd = w0; wd < w1; ++wd) {
                 uint32_t t = bitmap[wd];
                 while (t) {
-                    out[at++] = wd * 32 + __ffs(t) - 1;
+                    dst[at++] = wd * 32 + __ffs(t) - 1;
                     t &= t - 1;
                 }
+            }
+            if (staged) {
+                __syncthreads();
+                for (int i = tid; i < kk; i += kTopkThreads) out[i] = dst[i];
             }
         }
         if (tid == 0) p.sel_cnt[unit] = kk;
